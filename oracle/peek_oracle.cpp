@@ -1,0 +1,290 @@
+// peek_oracle.cpp — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, obviously-correct CPU implementation of what the PEEK hot path
+// computes (arxiv/paper_2607_02525).  Only tests/, __graft_entry__.smoke() and
+// bench.py's cpu_baseline / --impl reference legs may build, load or call this
+// file.  It shares no code, header, table or constant generator with the CUDA
+// path under paper_2607_02525_b200/csrc/, and neither includes the other.
+//
+// Every function is the plain definition written out (the paper's dual-walk,
+// Alg. 1, reaches the per-request longest prefix match exactly,
+// PAPER.md:73-82 "H[r] <- max(H[r], h)", "a partial match
+// terminates the branch"), so there is no blocking, fusion or reordering here.
+// Readings of silent / garbled passages are DESIGN.md "Readings" R1..R14
+// (= SURVEY.md section 8(c) O1-O5, S1-S26).
+//
+// Pins (tests/test_oracle_*.py, run with -m "not gpu"):
+//   orc_block_hash    splitmix64 known-answer stream + survey-computed vectors
+//                     (tests/golden/hash_vectors.txt), python big-int restatement
+//   orc_lpm_radix     brute force max-LCP over all cached sequences; std::mismatch
+//                     reduction for a one-sequence cache; planted structure
+//   orc_lpm_hash      python set of chained keys; mirror identity hit_hash =
+//                     B*floor(hit_radix/B)
+//   orc_pending_tree  python sorted() of tuples, O(N^2 nb) cluster definition,
+//                     paper worked example PAPER.md:55 (sizes 3/3/2), Fig. 6(a)
+//   orc_demand        nested-loop count; root-block demand = N
+//   orc_clpm_order    python sorted() of tuples; worked-example order
+// No function here is "parity unpinned".
+//
+// Threading: the per-request loops (hash, radix walk, hash probes) carry an
+// OpenMP "parallel for"; results do not depend on the thread count.  The sorts
+// and the demand map are single-threaded.
+
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <numeric>
+#include <unordered_map>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef uint64_t u64;
+typedef int64_t i64;
+typedef int32_t i32;
+
+static const u64 ORC_EMPTY = 0xFFFFFFFFFFFFFFFFull;  // table EMPTY sentinel (R5)
+
+// ---------------------------------------------------------------------------
+// O1. Chained block hash.  PAPER.md:596  k_i = hash(k_{i-1}, tuple(s[iB:(i+1)B])),
+// B = 16; "hashes each block by token content and prefix position via
+// chained hashing".  The paper names no hash function (R1): this is the
+// splitmix64 finaliser over an order-sensitive multiply-add of the block.
+// ---------------------------------------------------------------------------
+static inline u64 orc_mix64(u64 x) {
+    x ^= x >> 30;
+    x *= 0xBF58476D1CE4E5B9ull;
+    x ^= x >> 27;
+    x *= 0x94D049BB133111EBull;
+    x ^= x >> 31;
+    return x;
+}
+
+extern "C" u64 orc_mix64_export(u64 x) { return orc_mix64(x); }
+
+// M_j = mix64(j+1) | 1   (odd per-position multiplier)
+extern "C" u64 orc_position_multiplier(i32 j) { return orc_mix64((u64)j + 1) | 1ull; }
+
+extern "C" int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+extern "C" void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+// blk_off[r] = sum_{q<r} floor(len_q / B); trailing partial block not hashed (R3).
+// hashes must have room for blk_off[N] words.  Returns NB.
+extern "C" i64 orc_block_hash(const i32* tokens, const i64* tok_off, i64 N, i32 B, u64 seed,
+                              i64* blk_off, u64* hashes) {
+    blk_off[0] = 0;
+    for (i64 r = 0; r < N; ++r) blk_off[r + 1] = blk_off[r] + (tok_off[r + 1] - tok_off[r]) / B;
+    if (!hashes) return blk_off[N];
+    std::vector<u64> M(B);
+    for (i32 j = 0; j < B; ++j) M[j] = orc_position_multiplier(j);
+#pragma omp parallel for schedule(dynamic, 64)
+    for (i64 r = 0; r < N; ++r) {
+        const i32* s = tokens + tok_off[r];
+        i64 nb = blk_off[r + 1] - blk_off[r];
+        u64 k = seed;  // k_{-1} = seed (R2)
+        for (i64 i = 0; i < nb; ++i) {
+            u64 S = 0;
+            for (i32 j = 0; j < B; ++j) {
+                u64 t = (u64)(uint32_t)s[i * B + j];  // bit pattern as u32, widened (R6)
+                S += (t + 1) * M[j];
+            }
+            u64 c = orc_mix64(S);
+            k = orc_mix64(k ^ c);
+            if (k == ORC_EMPTY) k = 0xFFFFFFFFFFFFFFFEull;  // remapped value stored AND carried (R5)
+            hashes[blk_off[r] + i] = k;
+        }
+    }
+    return blk_off[N];
+}
+
+// ---------------------------------------------------------------------------
+// O2a. LPM against the radix cache (the result of Alg. 1): for
+// each request independently walk from the root; a partial edge match ends the
+// walk.  Token-granular, not rounded to B, not capped at len-1
+// (R9, R10).  Children of node v are edges n_child_off[v] .. n_child_off[v+1];
+// the child is found by linear scan on e_first_tok (R11).
+// ---------------------------------------------------------------------------
+extern "C" void orc_lpm_radix(const i32* tokens, const i64* tok_off, i64 N,
+                              const i32* c_tokens, const i64* n_tok_off, const i32* n_tok_len,
+                              const i32* n_child_off, const i32* e_first_tok, const i32* e_child,
+                              i32* hit_radix) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (i64 r = 0; r < N; ++r) {
+        const i32* s = tokens + tok_off[r];
+        i64 len = tok_off[r + 1] - tok_off[r];
+        i32 v = 0;
+        i64 d = 0;
+        for (;;) {
+            if (d == len) break;
+            i32 u = -1;
+            for (i32 e = n_child_off[v]; e < n_child_off[v + 1]; ++e)
+                if (e_first_tok[e] == s[d]) { u = e_child[e]; break; }
+            if (u < 0) break;
+            const i32* lab = c_tokens + n_tok_off[u];
+            i64 L = n_tok_len[u];
+            i64 m = 0;
+            while (m < L && d + m < len && lab[m] == s[d + m]) ++m;
+            d += m;
+            if (m < L) break;
+            v = u;
+        }
+        hit_radix[r] = (i32)d;
+    }
+}
+
+// ---------------------------------------------------------------------------
+// O2b. LPM against the flat block-hash table ("per-request
+// find_longest_cache_hit", O(N x b)).  Scan to the FIRST miss (R12).  Table:
+// open addressing, linear probing, home = key & (S-1), EMPTY = all ones (R13).
+// ---------------------------------------------------------------------------
+static inline bool orc_lookup(const u64* t_keys, i64 S, u64 key) {
+    i64 p = (i64)(key & (u64)(S - 1));
+    while (t_keys[p] != ORC_EMPTY) {
+        if (t_keys[p] == key) return true;
+        p = (p + 1) & (S - 1);
+    }
+    return false;
+}
+
+extern "C" void orc_lpm_hash(const u64* hashes, const i64* blk_off, i64 N, i32 B,
+                             const u64* t_keys, i64 S, i32* hit_hash) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (i64 r = 0; r < N; ++r) {
+        const u64* k = hashes + blk_off[r];
+        i64 nb = blk_off[r + 1] - blk_off[r];
+        i64 i = 0;
+        while (i < nb && orc_lookup(t_keys, S, k[i])) ++i;
+        hit_hash[r] = (i32)(B * i);
+    }
+}
+
+// ---------------------------------------------------------------------------
+// O3. Pending radix tree at block granularity (R7): the
+// sorted order of the hash chains is the DFS order of the compressed trie,
+// adjacent LCPs are its branching depths.
+// ---------------------------------------------------------------------------
+struct OrcChainLess {
+    const u64* hashes;
+    const i64* blk_off;
+    // word-by-word unsigned compare; a proper prefix sorts first; equal chains
+    // are "not less" either way so stable_sort keeps ascending request index.
+    bool operator()(i32 a, i32 b) const {
+        const u64* ka = hashes + blk_off[a];
+        const u64* kb = hashes + blk_off[b];
+        i64 na = blk_off[a + 1] - blk_off[a], nb = blk_off[b + 1] - blk_off[b];
+        i64 m = na < nb ? na : nb;
+        for (i64 i = 0; i < m; ++i) {
+            if (ka[i] != kb[i]) return ka[i] < kb[i];
+        }
+        return na < nb;
+    }
+};
+
+extern "C" void orc_pending_tree(const u64* hashes, const i64* blk_off, i64 N,
+                                 i32* order, i32* lcp, i32* group_id, i32* group_size,
+                                 i32* cluster_depth, i32* cluster_size, i64* cluster_id,
+                                 i32* n_groups) {
+    // O3.1 order
+    for (i64 r = 0; r < N; ++r) order[r] = (i32)r;
+    OrcChainLess less{hashes, blk_off};
+    std::stable_sort(order, order + N, less);
+    // O3.2 adjacent LCP in blocks, lcp[0] = 0; sentinel lcp[N] = 0 kept locally
+    std::vector<i32> L(N + 1, 0);
+    for (i64 j = 1; j < N; ++j) {
+        i32 a = order[j - 1], b = order[j];
+        const u64* ka = hashes + blk_off[a];
+        const u64* kb = hashes + blk_off[b];
+        i64 na = blk_off[a + 1] - blk_off[a], nb = blk_off[b + 1] - blk_off[b];
+        i64 m = na < nb ? na : nb, i = 0;
+        while (i < m && ka[i] == kb[i]) ++i;
+        L[j] = (i32)i;
+    }
+    for (i64 j = 0; j < N; ++j) lcp[j] = L[j];
+    // O3.3 flat groups: a new group starts at j iff lcp[j] == 0 (root-child
+    // subtrees, the ones has_sharing looks at)
+    i32 g = -1;
+    std::vector<i32> gsize;
+    for (i64 j = 0; j < N; ++j) {
+        if (L[j] == 0) { ++g; gsize.push_back(0); }
+        group_id[order[j]] = g;
+        gsize[g] += 1;
+    }
+    for (i64 j = 0; j < N; ++j) group_size[order[j]] = gsize[group_id[order[j]]];
+    *n_groups = g + 1;
+    // O3.4 cluster = deepest node on the request's path with pending_count >= 2
+    // (PAPER.md:94, :287); pending_count includes requests ending at the node (R8).
+    for (i64 j = 0; j < N; ++j) {
+        i32 r = order[j];
+        i32 cd = L[j] > L[j + 1] ? L[j] : L[j + 1];
+        if (cd == 0) {
+            cluster_depth[r] = 0;
+            cluster_size[r] = 1;
+            cluster_id[r] = (i64)((u64)j << 32);
+            continue;
+        }
+        i64 a = j;
+        while (!(L[a] < cd)) --a;  // largest p <= j with lcp[p] < cd (lcp[0] = 0 < cd)
+        i64 b = j;
+        while (!(L[b + 1] < cd)) ++b;  // smallest q >= j with lcp[q+1] < cd (lcp[N] = 0)
+        cluster_depth[r] = cd;
+        cluster_size[r] = (i32)(b - a + 1);
+        cluster_id[r] = (i64)(((u64)a << 32) | (u64)(uint32_t)cd);
+    }
+}
+
+// ---------------------------------------------------------------------------
+// O4. Per-table-slot pending demand (PAPER.md:281 inverted index
+// block_hash -> demand; pending_count in Eq. 2).  Independent of
+// hit lengths.  demand[p] = 0 for EMPTY slots.
+// ---------------------------------------------------------------------------
+extern "C" void orc_demand(const u64* hashes, const i64* blk_off, i64 N,
+                           const u64* t_keys, i64 S, i32* demand) {
+    std::unordered_map<u64, i64> slot_of;
+    slot_of.reserve((size_t)S);
+    for (i64 p = 0; p < S; ++p) {
+        demand[p] = 0;
+        if (t_keys[p] != ORC_EMPTY) slot_of.emplace(t_keys[p], p);
+    }
+    i64 NB = blk_off[N];
+    for (i64 x = 0; x < NB; ++x) {
+        auto it = slot_of.find(hashes[x]);
+        if (it != slot_of.end()) demand[it->second] += 1;
+    }
+}
+
+// ---------------------------------------------------------------------------
+// O5. cLPM order: the (-h, -|cluster|, arrival) sub-key of Eq. 1
+// with the request index as the last tie-break (R14).  arrival == NULL => index.
+// ---------------------------------------------------------------------------
+extern "C" void orc_clpm_order(const i32* hit, const i32* cluster_size, const i32* arrival,
+                               i64 N, i32* clpm_order) {
+    for (i64 r = 0; r < N; ++r) clpm_order[r] = (i32)r;
+    std::sort(clpm_order, clpm_order + N, [&](i32 a, i32 b) {
+        if (hit[a] != hit[b]) return hit[a] > hit[b];
+        if (cluster_size[a] != cluster_size[b]) return cluster_size[a] > cluster_size[b];
+        i32 aa = arrival ? arrival[a] : a, ab = arrival ? arrival[b] : b;
+        if (aa != ab) return aa < ab;
+        return a < b;
+    });
+}
+
+// has_sharing guard: true iff some root child has pending_count >= 2.
+extern "C" i32 orc_has_sharing(const i32* group_size, i64 N) {
+    for (i64 r = 0; r < N; ++r)
+        if (group_size[r] >= 2) return 1;
+    return 0;
+}
