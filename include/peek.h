@@ -1,0 +1,178 @@
+/* peek.h — C ABI of libpeek.so: the data-parallel hot path behind PEEK
+ * (arxiv/paper_2607_02525, "Predictive Queue-Informed KV Cache Management for LLM
+ * Serving"), as hand-written sm_100a CUDA kernels.
+ *
+ * Four calls (BASELINE.json north_star):
+ *   peek_block_hash    chained per-block hashes of CSR int32 token sequences
+ *                      ("k_i = hash(k_{i-1}, tuple(s[iB:(i+1)B]))", B = 16)
+ *   peek_pending_tree  the pending radix tree as a batch build: lexicographic order of the
+ *                      requests' hash chains, adjacent LCP, groups and clusters
+ *                      (PAPER.md:94 section 3.1, :287 section A.1.3, :125 has_sharing)
+ *   peek_lpm           per-request hit length against the engine's prefix cache: a radix cache
+ *                      (Alg. 1) and/or a flat block-hash table
+ *                      ("per-request find_longest_cache_hit")
+ *   peek_demand_rank   per-cached-block pending demand for the eviction hook (PAPER.md:115-119
+ *                      Eq. 2 pending_count; :281 inverted index block_hash -> demand) and the cLPM
+ *                      admission order, sub-key (-h, -|cluster|, arrival) of Eq. 1
+ *
+ * Conventions (the paper is silent on all of them):
+ *   Pointers   every array pointer is caller-owned DEVICE memory unless marked [host]; it must
+ *              stay valid until the work enqueued on `stream` has completed.  The library keeps
+ *              no state between calls, allocates no device memory and frees none.
+ *   Workspace  `ws` is caller-allocated device scratch of at least peek_workspace_bytes(...)
+ *              bytes, 256-byte aligned; contents undefined before and after.  Too small ->
+ *              PEEK_ERR_WORKSPACE, nothing enqueued.
+ *   Stream     `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *              Calls only enqueue work: no device synchronisation, no device->host copy.
+ *   Errors     return code only (0 = PEEK_OK, < 0 = error); peek_last_error() gives a
+ *              thread-local detail string.  Argument errors are detected on the host before
+ *              anything is enqueued.  Contents of device arrays are trusted (monotone offsets,
+ *              valid child indices, >= 1 EMPTY table slot) and not validated.
+ *   Sizes      N = 0 is PEEK_OK and touches nothing.  N < 2^31 - 1.  block_size must be 16
+ *              (every config) else PEEK_ERR_UNSUPPORTED.
+ *   Aliasing   inputs and outputs never alias each other or `ws`.
+ *   Determinism outputs are a pure function of the inputs (no dependence on atomics order).
+ *   There is no CPU fallback anywhere in this library.
+ */
+#ifndef PEEK_H_
+#define PEEK_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int32_t peek_status;
+enum {
+    PEEK_OK = 0,
+    PEEK_ERR_INVALID_ARG = -1,   /* NULL where required, negative size, S not a power of two, ... */
+    PEEK_ERR_CAPACITY = -2,      /* an output capacity the host can check is too small */
+    PEEK_ERR_WORKSPACE = -3,     /* ws NULL / misaligned / smaller than peek_workspace_bytes */
+    PEEK_ERR_CUDA = -4,          /* a CUDA runtime call failed; see peek_last_error() */
+    PEEK_ERR_UNSUPPORTED = -5,   /* block_size != 16 */
+    PEEK_ERR_UNIMPLEMENTED = -6
+};
+
+/* Table EMPTY sentinel: no chained hash ever equals it (peek_block_hash remaps). */
+#define PEEK_EMPTY_KEY 0xFFFFFFFFFFFFFFFFull
+
+/* Static strings, never freed.  peek_last_error is thread-local, "" if none. */
+const char* peek_status_string(peek_status s);
+const char* peek_last_error(void);
+int32_t peek_version(void); /* major*10000 + minor*100 + patch */
+
+/* ---- workspace -------------------------------------------------------------------------- */
+enum {
+    PEEK_CALL_BLOCK_HASH = 0,
+    PEEK_CALL_LPM = 1,
+    PEEK_CALL_PENDING_TREE = 2,
+    PEEK_CALL_DEMAND_RANK = 3
+};
+/* Bytes of device scratch `call_id` needs for the given sizes [host out].  N requests, T tokens,
+ * NB hashed blocks, S table slots, V radix nodes; pass 0 for sizes a call does not use. */
+peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t T, int64_t NB, int64_t S,
+                                 int64_t V, int64_t* out_bytes);
+
+/* ---- a1: chained block hash ----------------------------------------- */
+/* tokens  int32[T]  CSR token pool, request r = tokens[tok_off[r] .. tok_off[r+1])
+ * tok_off int64[N+1] monotone, tok_off[0] >= 0
+ * seed    k_{-1} of every chain
+ * blk_off int64[N+1] OUT exclusive prefix sum of nb_r = floor(len_r / block_size)
+ * hashes  uint64[NB] OUT k^r_i at hashes[blk_off[r] + i]; the trailing partial block of a request
+ *                    is not hashed.  hashes_capacity = number of uint64 the buffer holds; the
+ *                    caller computes NB = sum floor(len_r/B) on the host (it owns tok_off);
+ *                    kernels never write at or beyond hashes_capacity.
+ * Hash function (the paper names none; R1): tokens as uint32 bit patterns,
+ *   S_i = sum_j (tok[iB+j] + 1) * M_j,  M_j = mix64(j+1)|1,  c_i = mix64(S_i),
+ *   k_i = mix64(k_{i-1} ^ c_i), remapped to 0xFF..FE if it equals PEEK_EMPTY_KEY (remapped value
+ *   is stored and carried); mix64 = the splitmix64 finaliser. */
+peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok_off, int64_t N,
+                            int32_t block_size, uint64_t seed, int64_t* blk_off, uint64_t* hashes,
+                            int64_t hashes_capacity, void* ws, int64_t ws_bytes, void* stream);
+
+/* ---- the engine's prefix cache, read-only --------------------------------- */
+/* Radix cache flattened to arrays.  Node 0 is the root (empty label).  Node u's label is
+ * c_tokens[n_tok_off[u] .. + n_tok_len[u]).  The children of node v are edges
+ * n_child_off[v] .. n_child_off[v+1]; within a node edges are sorted ascending by e_first_tok
+ * (signed int32), first tokens are distinct, and e_first_tok[e] == first label token of
+ * e_child[e] ("children keyed by the first edge token"). */
+typedef struct {
+    const int32_t* c_tokens;    /* int32[CT] */
+    int64_t CT;
+    const int64_t* n_tok_off;   /* int64[V] */
+    const int32_t* n_tok_len;   /* int32[V] */
+    const int32_t* n_child_off; /* int32[V+1] */
+    int32_t V;
+    const int32_t* e_first_tok; /* int32[E] */
+    const int32_t* e_child;     /* int32[E] */
+    int32_t E;
+} peek_radix;
+
+/* Flat block-hash cache: open addressing, linear probing, home = key & (S-1), S a power of two,
+ * empty slots hold PEEK_EMPTY_KEY, each key at most once, no tombstones, >= 1 empty slot. */
+typedef struct {
+    const uint64_t* t_keys; /* uint64[S] */
+    int64_t S;
+} peek_table;
+
+/* Optional accelerator for peek_lpm: outputs of peek_pending_tree over the SAME hashes/blk_off.
+ * order/lcp are by sorted position.  With it, peek_lpm co-descends: a request whose sorted
+ * predecessor's hit ends inside their common prefix copies that hit without touching the cache;
+ * otherwise it resumes at the common depth (Alg. 1 "one cache walk per pending edge",
+ * PAPER.md:73-82, :96).  Results are identical with and without it. */
+typedef struct {
+    const int32_t* order; /* int32[N] */
+    const int32_t* lcp;   /* int32[N] */
+} peek_tree_view;
+
+/* ---- a5/a6: longest prefix match (Alg. 1; hash mode PAPER.md:87-89) -- */
+/* hit_radix int32[N] OUT (NULL to skip; needs radix, tokens, tok_off): tokens of request r matched
+ *           from the root; a partial edge match ends the walk; token-granular; not capped at len-1.
+ * hit_hash  int32[N] OUT (NULL to skip; needs table, hashes, blk_off): block_size * number of
+ *           leading blocks whose chained hash is in the table, scanning to the FIRST miss.
+ * tree      optional (NULL = naive per-request walk; needs hashes/blk_off as given to
+ *           peek_pending_tree). */
+peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, const uint64_t* hashes,
+                     const int64_t* blk_off, int64_t N, int32_t block_size,
+                     const peek_radix* radix /*host struct*/, const peek_table* table /*host struct*/,
+                     const peek_tree_view* tree /*host struct*/, int32_t* hit_radix,
+                     int32_t* hit_hash, void* ws, int64_t ws_bytes, void* stream);
+
+/* ---- a2-a4: pending radix tree at block granularity ------------ */
+/* order         int32[N] OUT sorted position -> request; chains compared word by word as unsigned
+ *               64-bit, a proper prefix first, identical chains by ascending request index
+ * lcp           int32[N] OUT lcp[0] = 0; lcp[j] = leading equal hash words of order[j-1], order[j]
+ * group_id      int32[N] OUT by request: dense id (in sorted order) of the root-child subtree;
+ *               a new group starts at sorted position j iff lcp[j] == 0
+ * group_size    int32[N] OUT by request: members of its group   (has_sharing <=> max >= 2)
+ * cluster_depth int32[N] OUT by request: depth in blocks of the deepest node on its path with
+ *               pending_count >= 2 (0 = none: singleton)
+ * cluster_size  int32[N] OUT by request: that node's pending_count (1 for singletons)
+ * cluster_id    int64[N] OUT by request: (first sorted position under the node << 32) | depth;
+ *               (sorted position << 32) for singletons
+ * n_groups      int32[1] OUT device scalar
+ * Any of group_id .. n_groups may be NULL (skipped); order and lcp are required.
+ * Relies on the chain property "k_i equal => k_j equal for all j < i" (true unless two distinct
+ * blocks collide in 64 bits; R15). */
+peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* blk_off, int64_t N,
+                              int32_t* order, int32_t* lcp, int32_t* group_id, int32_t* group_size,
+                              int32_t* cluster_depth, int32_t* cluster_size, int64_t* cluster_id,
+                              int32_t* n_groups, void* ws, int64_t ws_bytes, void* stream);
+
+/* ---- a7/a8: eviction demand and cLPM order (Eq. 1) */
+/* demand     int32[S] OUT (NULL to skip; needs hashes, blk_off, order, lcp, table): for an occupied
+ *            slot the number of (request, block) pairs whose chained hash equals its key, 0 for
+ *            empty slots.  Independent of hit lengths.
+ * clpm_order int32[N] OUT (NULL to skip; needs hit, cluster_size): request indices sorted ascending
+ *            by (-hit[r], -cluster_size[r], arrival[r], r); arrival NULL => arrival[r] = r. */
+peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* blk_off, int64_t N,
+                             const int32_t* order, const int32_t* lcp,
+                             const peek_table* table /*host struct*/, const int32_t* hit,
+                             const int32_t* cluster_size, const int32_t* arrival, int32_t* demand,
+                             int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PEEK_H_ */

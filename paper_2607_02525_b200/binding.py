@@ -1,0 +1,236 @@
+"""Thin ctypes binding over libpeek.so (include/peek.h): argument marshalling only.
+
+Same four names as the C ABI.  PyTorch supplies device memory and the current CUDA stream; every
+step of the path runs in the library's kernels.  There is no fallback: if libpeek.so is missing or
+a call fails, this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpeek.so")
+_lib = None
+
+CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
+EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
+           "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank"]
+
+
+class PeekError(RuntimeError):
+    pass
+
+
+class _Radix(ctypes.Structure):
+    _fields_ = [("c_tokens", ctypes.c_void_p), ("CT", ctypes.c_int64),
+                ("n_tok_off", ctypes.c_void_p), ("n_tok_len", ctypes.c_void_p),
+                ("n_child_off", ctypes.c_void_p), ("V", ctypes.c_int32),
+                ("e_first_tok", ctypes.c_void_p), ("e_child", ctypes.c_void_p),
+                ("E", ctypes.c_int32)]
+
+
+class _Table(ctypes.Structure):
+    _fields_ = [("t_keys", ctypes.c_void_p), ("S", ctypes.c_int64)]
+
+
+class _TreeView(ctypes.Structure):
+    _fields_ = [("order", ctypes.c_void_p), ("lcp", ctypes.c_void_p)]
+
+
+def lib():
+    """Load libpeek.so; raise loudly if it has not been built (python -m paper_2607_02525_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise PeekError("libpeek.so not found at %s: build it with "
+                            "`python -m paper_2607_02525_b200.build` (no CPU fallback exists)" % LIB_PATH)
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, i32, u64 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_uint64
+        L.peek_status_string.restype = ctypes.c_char_p
+        L.peek_status_string.argtypes = [i32]
+        L.peek_last_error.restype = ctypes.c_char_p
+        L.peek_version.restype = i32
+        L.peek_workspace_bytes.restype = i32
+        L.peek_workspace_bytes.argtypes = [i32, i64, i64, i64, i64, i64, ctypes.POINTER(i64)]
+        L.peek_block_hash.restype = i32
+        L.peek_block_hash.argtypes = [vp, vp, i64, i32, u64, vp, vp, i64, vp, i64, vp]
+        L.peek_lpm.restype = i32
+        L.peek_lpm.argtypes = [vp, vp, vp, vp, i64, i32, ctypes.POINTER(_Radix), ctypes.POINTER(_Table),
+                               ctypes.POINTER(_TreeView), vp, vp, vp, i64, vp]
+        L.peek_pending_tree.restype = i32
+        L.peek_pending_tree.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp]
+        L.peek_demand_rank.restype = i32
+        L.peek_demand_rank.argtypes = [vp, vp, i64, vp, vp, ctypes.POINTER(_Table), vp, vp, vp, vp, vp,
+                                       vp, i64, vp]
+        _lib = L
+    return _lib
+
+
+def _check(st: int, what: str):
+    if st != 0:
+        L = lib()
+        raise PeekError("%s: %s (%s)" % (what, L.peek_status_string(st).decode(),
+                                         L.peek_last_error().decode()))
+
+
+def _ptr(t: Optional[torch.Tensor], dtype=None):
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise PeekError("expected a CUDA tensor (the library has no CPU path)")
+    if not t.is_contiguous():
+        raise PeekError("expected a contiguous tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise PeekError("expected dtype %s, got %s" % (dtype, t.dtype))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+_ws_cache = {}
+
+
+def workspace_bytes(call_id: int, N=0, T=0, NB=0, S=0, V=0) -> int:
+    out = ctypes.c_int64(0)
+    _check(lib().peek_workspace_bytes(call_id, N, T, NB, S, V, ctypes.byref(out)), "peek_workspace_bytes")
+    return int(out.value)
+
+
+def _ws(call_id, device, **sizes):
+    need = workspace_bytes(call_id, **sizes)
+    key = (str(device), call_id)
+    buf = _ws_cache.get(key)
+    if buf is None or buf.numel() < need:
+        buf = torch.empty(need, dtype=torch.uint8, device=device)
+        _ws_cache[key] = buf
+    return buf, need
+
+
+U64 = torch.uint64
+
+
+@dataclass
+class Radix:
+    """Flattened radix cache on the device (include/peek.h peek_radix)."""
+    c_tokens: torch.Tensor     # int32[CT]
+    n_tok_off: torch.Tensor    # int64[V]
+    n_tok_len: torch.Tensor    # int32[V]
+    n_child_off: torch.Tensor  # int32[V+1]
+    e_first_tok: torch.Tensor  # int32[E]
+    e_child: torch.Tensor      # int32[E]
+
+    def _c(self) -> _Radix:
+        V = int(self.n_tok_len.shape[0])
+        E = int(self.e_child.shape[0])
+        return _Radix(_ptr(self.c_tokens, torch.int32) if self.c_tokens.numel() else None,
+                      int(self.c_tokens.shape[0]), _ptr(self.n_tok_off, torch.int64),
+                      _ptr(self.n_tok_len, torch.int32), _ptr(self.n_child_off, torch.int32), V,
+                      _ptr(self.e_first_tok, torch.int32) if E else None,
+                      _ptr(self.e_child, torch.int32) if E else None, E)
+
+
+@dataclass
+class PendingTree:
+    order: torch.Tensor
+    lcp: torch.Tensor
+    group_id: torch.Tensor
+    group_size: torch.Tensor
+    cluster_depth: torch.Tensor
+    cluster_size: torch.Tensor
+    cluster_id: torch.Tensor
+    n_groups: torch.Tensor  # int32[1] on the device
+
+
+def peek_block_hash(tokens: torch.Tensor, tok_off: torch.Tensor, NB: int, block_size: int = 16,
+                    seed: int = 0, blk_off: Optional[torch.Tensor] = None,
+                    hashes: Optional[torch.Tensor] = None):
+    """a1.  NB = sum floor(len_r / block_size), computed by the caller from its
+    host copy of tok_off.  Returns (blk_off int64[N+1], hashes uint64[NB])."""
+    N = int(tok_off.shape[0]) - 1
+    dev = tok_off.device
+    if blk_off is None:
+        blk_off = torch.empty(N + 1, dtype=torch.int64, device=dev)
+    if hashes is None:
+        hashes = torch.empty(max(NB, 1), dtype=U64, device=dev)
+    ws, nbytes = _ws(CALL_BLOCK_HASH, dev, N=N)
+    st = lib().peek_block_hash(_ptr(tokens, torch.int32) if tokens.numel() else None,
+                               _ptr(tok_off, torch.int64), N, block_size, ctypes.c_uint64(seed),
+                               _ptr(blk_off, torch.int64), _ptr(hashes, U64), NB, _ptr(ws), nbytes, _stream())
+    _check(st, "peek_block_hash")
+    return blk_off, hashes[:NB]
+
+
+def peek_pending_tree(hashes: torch.Tensor, blk_off: torch.Tensor, signals: bool = True) -> PendingTree:
+    """a2-a4."""
+    N = int(blk_off.shape[0]) - 1
+    dev = blk_off.device
+    e32 = lambda: torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N]
+    t = PendingTree(e32(), e32(), e32(), e32(), e32(), e32(),
+                    torch.empty(max(N, 1), dtype=torch.int64, device=dev)[:N],
+                    torch.zeros(1, dtype=torch.int32, device=dev))
+    ws, nbytes = _ws(CALL_PENDING_TREE, dev, N=N)
+    sig = (lambda x: _ptr(x)) if signals else (lambda x: None)
+    st = lib().peek_pending_tree(_ptr(hashes, U64) if hashes.numel() else None, _ptr(blk_off, torch.int64),
+                                 N, _ptr(t.order), _ptr(t.lcp), sig(t.group_id), sig(t.group_size),
+                                 sig(t.cluster_depth), sig(t.cluster_size), sig(t.cluster_id),
+                                 sig(t.n_groups), _ptr(ws), nbytes, _stream())
+    _check(st, "peek_pending_tree")
+    return t
+
+
+def peek_lpm(tokens=None, tok_off=None, hashes=None, blk_off=None, radix: Optional[Radix] = None,
+             t_keys: Optional[torch.Tensor] = None, tree: Optional[PendingTree] = None,
+             block_size: int = 16, want_radix: Optional[bool] = None, want_hash: Optional[bool] = None):
+    """a5/a6 (Alg. 1).  Returns (hit_radix | None, hit_hash | None)."""
+    ref = tok_off if tok_off is not None else blk_off
+    N = int(ref.shape[0]) - 1
+    dev = ref.device
+    want_radix = radix is not None if want_radix is None else want_radix
+    want_hash = t_keys is not None if want_hash is None else want_hash
+    hr = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N] if want_radix else None
+    hh = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N] if want_hash else None
+    cr = radix._c() if radix is not None else None
+    ct = _Table(_ptr(t_keys, U64), int(t_keys.shape[0])) if t_keys is not None else None
+    cv = _TreeView(_ptr(tree.order, torch.int32), _ptr(tree.lcp, torch.int32)) if tree is not None else None
+    ws, nbytes = _ws(CALL_LPM, dev, N=N)
+    if tokens is not None and tokens.numel() == 0:  # all requests empty: still a valid pointer
+        tokens = torch.zeros(4, dtype=torch.int32, device=dev)
+    st = lib().peek_lpm(_ptr(tokens), _ptr(tok_off),
+                        _ptr(hashes) if hashes is not None and hashes.numel() else None, _ptr(blk_off), N,
+                        block_size, ctypes.byref(cr) if cr is not None else None,
+                        ctypes.byref(ct) if ct is not None else None,
+                        ctypes.byref(cv) if cv is not None else None, _ptr(hr), _ptr(hh), _ptr(ws), nbytes,
+                        _stream())
+    _check(st, "peek_lpm")
+    return hr, hh
+
+
+def peek_demand_rank(hashes=None, blk_off=None, tree: Optional[PendingTree] = None,
+                     t_keys: Optional[torch.Tensor] = None, hit: Optional[torch.Tensor] = None,
+                     cluster_size: Optional[torch.Tensor] = None, arrival: Optional[torch.Tensor] = None,
+                     want_demand: Optional[bool] = None, want_order: Optional[bool] = None):
+    """a7/a8 (Eq. 1).  Returns (demand | None, clpm_order | None)."""
+    ref = blk_off if blk_off is not None else hit
+    N = int(ref.shape[0]) - (1 if blk_off is not None else 0)
+    dev = ref.device
+    want_demand = t_keys is not None if want_demand is None else want_demand
+    want_order = hit is not None if want_order is None else want_order
+    S = int(t_keys.shape[0]) if t_keys is not None else 0
+    demand = torch.empty(S, dtype=torch.int32, device=dev) if want_demand else None
+    out = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N] if want_order else None
+    ct = _Table(_ptr(t_keys, U64), S) if t_keys is not None else None
+    ws, nbytes = _ws(CALL_DEMAND_RANK, dev, N=N, S=S)
+    st = lib().peek_demand_rank(_ptr(hashes) if hashes is not None and hashes.numel() else None,
+                                _ptr(blk_off), N, _ptr(tree.order) if tree is not None else None,
+                                _ptr(tree.lcp) if tree is not None else None,
+                                ctypes.byref(ct) if ct is not None else None, _ptr(hit), _ptr(cluster_size),
+                                _ptr(arrival), _ptr(demand), _ptr(out), _ptr(ws), nbytes, _stream())
+    _check(st, "peek_demand_rank")
+    return demand, out

@@ -1,0 +1,123 @@
+// peek_common.cuh — shared host/device helpers of libpeek.so (sm_100a only).
+// Nothing here is shared with oracle/: the constants and the mixer below are this
+// library's own statement of DESIGN.md R1.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/peek.h"
+
+typedef uint64_t u64;
+typedef int64_t i64;
+typedef int32_t i32;
+typedef uint32_t u32;
+
+namespace peek {
+
+// ---- host side ---------------------------------------------------------------------------
+void set_error(const char* fmt, ...);
+peek_status cuda_fail(cudaError_t e, const char* what);
+int sm_count();  // SMs of the current device (148 on B200)
+
+#define PEEK_CUDA(call)                                            \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) return peek::cuda_fail(e__, #call); \
+    } while (0)
+
+static inline i64 align_up(i64 x, i64 a) { return (x + a - 1) / a * a; }
+
+// Bump allocator over the caller's workspace (256-byte aligned pieces).
+struct Arena {
+    char* base;
+    i64 used;
+    explicit Arena(void* p) : base((char*)p), used(0) {}
+    template <typename T>
+    T* take(i64 n) {
+        T* r = (T*)(base ? base + used : nullptr);
+        used += align_up((n > 0 ? n : 1) * (i64)sizeof(T), 256);
+        return r;
+    }
+};
+
+// ---- device side -------------------------------------------------------------------------
+#define PEEK_EMPTY 0xFFFFFFFFFFFFFFFFull
+
+__host__ __device__ constexpr u64 mix64(u64 x) {  // splitmix64 finaliser
+    x ^= x >> 30;
+    x *= 0xBF58476D1CE4E5B9ull;
+    x ^= x >> 27;
+    x *= 0x94D049BB133111EBull;
+    x ^= x >> 31;
+    return x;
+}
+__host__ __device__ constexpr u64 pos_mult(int j) { return mix64((u64)j + 1) | 1ull; }
+
+__device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+
+// streaming 128-bit load that does not allocate in L1 (read-once data)
+__device__ __forceinline__ int4 ld_stream_v4(const void* p) {
+    int4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+__device__ __forceinline__ u32 ld_acquire_u32(const u32* p) {
+    u32 v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// Grid-wide barrier for persistent kernels launched with cudaLaunchCooperativeKernel (all CTAs
+// co-resident).  `ctr` is a zero-initialised device word that only ever grows; `epoch` is the
+// caller's running target (starts at 0, same in every thread).  The gpu-scope fences publish
+// this CTA's writes and drop stale L1 lines before the next phase reads other CTAs' data.
+__device__ __forceinline__ void grid_barrier(u32* ctr, u32& epoch) {
+    epoch += gridDim.x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(ctr, 1u);
+        while (ld_acquire_u32(ctr) < epoch) __nanosleep(32);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ int bits_for(u64 maxval) {  // bits needed to hold 0..maxval
+    return maxval == 0 ? 1 : 64 - __clzll((long long)maxval);
+}
+
+// CTA-wide exclusive scan of one i64 per thread (blockDim.x <= 1024, multiple of 32).
+// `smem` holds >= 33 i64.  Returns the exclusive prefix; *total gets the CTA sum.
+__device__ __forceinline__ i64 block_exscan_i64(i64 v, i64* smem, i64* total) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    i64 inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        i64 t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) smem[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        i64 s = lane < nw ? smem[lane] : 0;
+        i64 si = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            i64 t = __shfl_up_sync(0xffffffffu, si, o);
+            if (lane >= o) si += t;
+        }
+        if (lane < nw) smem[lane] = si - s;
+        if (lane == 31) smem[32] = si;
+    }
+    __syncthreads();
+    i64 r = smem[w] + inc - v;
+    *total = smem[32];
+    __syncthreads();
+    return r;
+}
+
+}  // namespace peek

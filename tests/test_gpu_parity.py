@@ -1,0 +1,181 @@
+"""-m gpu: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element, bit-exact (every output is integer / index work), on the same seeded inputs.
+Sizes span several sort tiles (2048), scan chunks and ragged tails."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2607_02525_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda:0"
+
+
+def _b():
+    from paper_2607_02525_b200 import binding
+    return binding
+
+
+def _dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.view(dtype)
+    return t.to(DEV)
+
+
+def _np(t, dtype=None):
+    a = t.cpu()
+    if a.dtype == torch.uint64:
+        return a.view(torch.int64).numpy().view(np.uint64)
+    return a.numpy()
+
+
+def _radix_dev(r):
+    b = _b()
+    return b.Radix(_dev(r.c_tokens), _dev(r.n_tok_off), _dev(r.n_tok_len), _dev(r.n_child_off),
+                   _dev(r.e_first_tok), _dev(r.e_child))
+
+
+def _orc_radix(r):
+    return oracle.Radix(r.c_tokens, r.n_tok_off, r.n_tok_len, r.n_child_off, r.e_first_tok, r.e_child)
+
+
+def run_pipeline(toks, off, radix, t_keys, arrival, check_tree_free=True):
+    """GPU pipeline vs oracle on CSR tokens (numpy).  radix: workloads.RadixArrays or None."""
+    b = _b()
+    N = off.shape[0] - 1
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    NB = int(o_bo[-1])
+    d_tok = _dev(toks) if toks.shape[0] else torch.zeros(0, dtype=torch.int32, device=DEV)
+    d_off = _dev(off)
+    g_bo, g_h = b.peek_block_hash(d_tok, d_off, NB)
+    assert np.array_equal(_np(g_bo), o_bo)
+    assert np.array_equal(_np(g_h), o_h)
+
+    ot = oracle.pending_tree(o_h, o_bo)
+    gt = b.peek_pending_tree(g_h, g_bo)
+    assert np.array_equal(_np(gt.order), ot.order)
+    assert np.array_equal(_np(gt.lcp), ot.lcp)
+    assert np.array_equal(_np(gt.group_id), ot.group_id)
+    assert np.array_equal(_np(gt.group_size), ot.group_size)
+    assert int(gt.n_groups.item()) == ot.n_groups
+    assert np.array_equal(_np(gt.cluster_depth), ot.cluster_depth)
+    assert np.array_equal(_np(gt.cluster_size), ot.cluster_size)
+    assert np.array_equal(_np(gt.cluster_id), ot.cluster_id)
+
+    d_keys = _dev(t_keys.view(np.int64), torch.uint64) if t_keys is not None else None
+    d_radix = _radix_dev(radix) if radix is not None else None
+    o_hr = oracle.lpm_radix(toks, off, _orc_radix(radix)) if radix is not None else None
+    o_hh = oracle.lpm_hash(o_h, o_bo, t_keys) if t_keys is not None else None
+    # co-descent (tree view) and the naive per-request walk must both equal the oracle
+    for tree in ([gt, None] if check_tree_free else [gt]):
+        g_hr, g_hh = b.peek_lpm(d_tok, d_off, g_h, g_bo, radix=d_radix, t_keys=d_keys, tree=tree)
+        if radix is not None:
+            assert np.array_equal(_np(g_hr), o_hr), "hit_radix tree=%s" % (tree is not None)
+        if t_keys is not None:
+            assert np.array_equal(_np(g_hh), o_hh), "hit_hash tree=%s" % (tree is not None)
+
+    hit_np = o_hr if o_hr is not None else o_hh
+    d_hit = _dev(hit_np)
+    d_arr = _dev(arrival) if arrival is not None else None
+    g_dem, g_ord = b.peek_demand_rank(g_h, g_bo, tree=gt, t_keys=d_keys, hit=d_hit,
+                                      cluster_size=gt.cluster_size, arrival=d_arr)
+    if t_keys is not None:
+        assert np.array_equal(_np(g_dem), oracle.demand(o_h, o_bo, t_keys))
+    assert np.array_equal(_np(g_ord), oracle.clpm_order(hit_np, ot.cluster_size, arrival))
+    torch.cuda.synchronize()
+    return dict(N=N, NB=NB)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("seed", [42, 142])
+def test_small_configs(cfg, seed):
+    wl = W.make(cfg, seed=seed, small=True)
+    toks, off = wl.queue.materialize_np()
+    cache = W.build_cache(wl, lambda t, o: oracle.block_hash(t, o, 16, 0))
+    run_pipeline(toks, off, cache.radix, cache.t_keys, wl.arrival)
+
+
+def _csr(seqs):
+    off = np.zeros(len(seqs) + 1, dtype=np.int64)
+    off[1:] = np.cumsum([len(s) for s in seqs])
+    toks = np.concatenate([np.asarray(s, dtype=np.int32) for s in seqs]) if off[-1] else np.zeros(0, np.int32)
+    return toks.astype(np.int32), off
+
+
+def _cache_from(seqs, slots):
+    toks, off = _csr(seqs)
+    n = len(seqs)
+    pcs = W.Pieces(toks, off[:-1].copy(), np.diff(off), np.arange(n + 1, dtype=np.int64))
+    radix, _ = W.build_radix(pcs, 16, 0)
+    _, keys = oracle.block_hash(toks, off, 16, 0)
+    return radix, W.build_table(keys, slots)
+
+
+def test_edge_cases_tiny_vocab():
+    """Tiny vocab so prefixes collide at every depth; empty, sub-block, duplicate and
+    prefix-of-another requests; arrival = NULL."""
+    rng = np.random.default_rng(5)
+    stems = [rng.integers(0, 3, size=int(rng.integers(1, 200))).astype(np.int32) for _ in range(6)]
+    reqs = [np.zeros(0, np.int32), np.zeros(5, np.int32), np.zeros(16, np.int32), np.zeros(16, np.int32)]
+    for _ in range(700):
+        s = stems[int(rng.integers(0, 6))]
+        cut = int(rng.integers(0, len(s) + 1))
+        tail = rng.integers(0, 3, size=int(rng.integers(0, 60))).astype(np.int32)
+        reqs.append(np.concatenate([s[:cut], tail]))
+    reqs += [reqs[10].copy(), reqs[10][: len(reqs[10]) // 2].copy(), reqs[11].copy()]
+    toks, off = _csr(reqs)
+    radix, t_keys = _cache_from([s for s in stems] + [reqs[20], reqs[21]], 1 << 10)
+    run_pipeline(toks, off, radix, t_keys, None)
+
+
+def test_empty_cache_and_self_cache():
+    rng = np.random.default_rng(9)
+    reqs = [rng.integers(0, 1000, size=int(rng.integers(0, 300))).astype(np.int32) for _ in range(300)]
+    toks, off = _csr(reqs)
+    # empty cache: V = 1, all-EMPTY table
+    radix, _ = W.build_radix(None, 16, 0)
+    t_keys = np.full(64, W.EMPTY, dtype=np.uint64)
+    run_pipeline(toks, off, radix, t_keys, None)
+    # the cache is the requests themselves: hit_radix = len, hit_hash = 16 * nb
+    radix, t_keys = _cache_from([r for r in reqs if len(r)], 1 << 14)
+    run_pipeline(toks, off, radix, t_keys, rng.permutation(len(reqs)).astype(np.int32))
+
+
+def test_single_and_identical():
+    one = [np.arange(100, dtype=np.int32)]
+    toks, off = _csr(one)
+    radix, t_keys = _cache_from(one, 64)
+    run_pipeline(toks, off, radix, t_keys, None)
+    same = [np.arange(64, dtype=np.int32)] * 2500
+    toks, off = _csr(same)
+    run_pipeline(toks, off, radix, t_keys, None)
+
+
+def test_wide_root_fanout_and_long_edges():
+    """Root with thousands of children (32-ary child search) and a 40k-token edge."""
+    rng = np.random.default_rng(11)
+    cached = [np.concatenate([[i * 7], rng.integers(0, 128256, size=30)]).astype(np.int32) for i in range(5000)]
+    long = rng.integers(0, 128256, size=40000).astype(np.int32)
+    cached.append(long)
+    reqs = [c[: int(rng.integers(1, 32))] for c in cached[:800]]
+    reqs += [np.concatenate([long[: int(rng.integers(1, 40000))], rng.integers(0, 9, size=40)]).astype(np.int32)
+             for _ in range(40)]
+    reqs += [rng.integers(-5, 128256, size=50).astype(np.int32) for _ in range(100)]
+    toks, off = _csr(reqs)
+    radix, t_keys = _cache_from(cached, 1 << 18)
+    run_pipeline(toks, off, radix, t_keys, rng.permutation(len(reqs)).astype(np.int32))
+
+
+def test_arg_errors():
+    b = _b()
+    L = b.lib()
+    assert L.peek_block_hash(None, None, -1, 16, 0, None, None, 0, None, 0, None) == -1
+    assert L.peek_block_hash(None, None, 4, 8, 0, None, None, 0, None, 0, None) == -5
+    assert L.peek_block_hash(None, None, 0, 16, 0, None, None, 0, None, 0, None) == 0
+    assert L.peek_pending_tree(None, None, 0, None, None, None, None, None, None, None, None, None, 0, None) == 0
+    off = torch.zeros(5, dtype=torch.int64, device=DEV)
+    with pytest.raises(b.PeekError):
+        b.peek_lpm(None, off, None, off, radix=None, t_keys=torch.zeros(6, dtype=torch.uint64, device=DEV))
