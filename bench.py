@@ -1,0 +1,450 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the PEEK hot path on B200 (contract in DESIGN.md "Measurement").
+
+A step = one pass of the whole hot path over one batch of pending requests, through the C ABI:
+peek_block_hash -> peek_pending_tree -> peek_lpm (radix + hash mode, co-descent) ->
+peek_demand_rank.  Default workload: BASELINE.json configs[4] (agentic multi-turn, 1 048 576
+pending requests, ~4.3e9 tokens), the "largest config" north_star's target is quoted on.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl peek|reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2607_02525_b200 import workloads as W  # noqa: E402
+
+METRIC = "lpm_queries_per_s"
+UNIT = "queries/s"
+CONFIG_NAMES = {1: "configs[0] tiny_shared_prompt_chat", 2: "configs[1] shared_prompt_chat_at_scale",
+                3: "configs[2] long_prefix_rag", 4: "configs[3] singleton_chat_table_only",
+                5: "configs[4] agentic_multi_turn_at_scale"}
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def parse():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=5)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--config", type=int, default=5)
+    p.add_argument("--seed", type=int, default=42)
+    p.add_argument("--impl", default="peek", choices=["peek", "reference"])
+    p.add_argument("--small", action="store_true", help="reduced sizes (tests)")
+    p.add_argument("--e2e-steps", type=int, default=2)
+    p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--cpu-seconds", type=float, default=15.0)
+    return p.parse_args()
+
+
+# ------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v == "Active":
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------
+# inputs
+# ------------------------------------------------------------------------------------------
+class Inputs:
+    pass
+
+
+def gpu_hash_fn(dev):
+    """hash_fn for workloads.build_cache: the CUDA call (the product path never touches oracle/)."""
+    from paper_2607_02525_b200 import binding as B
+
+    def fn(toks, off):
+        nb = int((np.diff(off) // 16).sum())
+        t = torch.from_numpy(np.ascontiguousarray(toks)).to(dev)
+        o = torch.from_numpy(np.ascontiguousarray(off)).to(dev)
+        bo, h = B.peek_block_hash(t, o, nb)
+        torch.cuda.synchronize()
+        return bo.cpu().numpy(), h.cpu().view(torch.int64).numpy().view(np.uint64)
+    return fn
+
+
+def build_inputs(cfg: int, seed: int, small: bool, dev) -> Inputs:
+    from paper_2607_02525_b200 import binding as B
+    t0 = time.time()
+    wl = W.make(cfg, seed=seed, small=small)
+    inp = Inputs()
+    inp.wl = wl
+    inp.N = wl.N
+    lens = wl.queue.seq_lens()
+    inp.T = int(lens.sum())
+    inp.NB = int((lens // 16).sum())
+    inp.tok, inp.off = wl.queue.materialize(dev)
+    log("[bench] config %d: N=%d T=%d NB=%d generated+uploaded in %.1fs" % (cfg, inp.N, inp.T, inp.NB, time.time() - t0))
+    t0 = time.time()
+    cache = W.build_cache(wl, gpu_hash_fn(dev))
+    inp.cache = cache
+    up = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    inp.radix = None
+    if cache.radix is not None:
+        r = cache.radix
+        inp.radix = B.Radix(up(r.c_tokens), up(r.n_tok_off), up(r.n_tok_len), up(r.n_child_off),
+                            up(r.e_first_tok), up(r.e_child))
+    inp.keys = up(cache.t_keys.view(np.int64)).view(torch.uint64)
+    inp.S = int(cache.t_keys.shape[0])
+    inp.arrival = up(wl.arrival)
+    inp.bo_buf = torch.empty(inp.N + 1, dtype=torch.int64, device=dev)
+    inp.h_buf = torch.empty(max(inp.NB, 1), dtype=torch.uint64, device=dev)
+    log("[bench] cache: V=%s keys=%d S=%d built in %.1fs" % (
+        cache.radix.V if cache.radix is not None else None, cache.n_keys, inp.S, time.time() - t0))
+    return inp
+
+
+def step(inp: Inputs, tok=None, off=None):
+    """One pass of the hot path; every stage is a libpeek.so call."""
+    from paper_2607_02525_b200 import binding as B
+    tok = inp.tok if tok is None else tok
+    off = inp.off if off is None else off
+    bo, h = B.peek_block_hash(tok, off, inp.NB, blk_off=inp.bo_buf, hashes=inp.h_buf)
+    tree = B.peek_pending_tree(h, bo)
+    hr, hh = B.peek_lpm(tok, off, h, bo, radix=inp.radix, t_keys=inp.keys, tree=tree)
+    hit = hr if hr is not None else hh
+    dem, order = B.peek_demand_rank(h, bo, tree=tree, t_keys=inp.keys, hit=hit,
+                                    cluster_size=tree.cluster_size, arrival=inp.arrival)
+    return dict(bo=bo, h=h, tree=tree, hit_radix=hr, hit_hash=hh, hit=hit, demand=dem, clpm=order)
+
+
+def algorithmic_bytes(inp: Inputs, out: dict) -> dict:
+    """SURVEY.md section 8(d) B_alg per call, from by-products of one step (reporting only)."""
+    N, T, NB, S = inp.N, inp.T, inp.NB, inp.S
+    tree = out["tree"]
+    order = tree.order.long()
+    lcp = tree.lcp.long()
+    nb = (out["bo"][1:] - out["bo"][:-1])[order]
+    res = {"hash": 4 * T + 8 * NB + 16 * N, "hash.content": 4 * T + 8 * NB + 16 * N, "hash.chain": 16 * NB + 16 * N}
+    lc = torch.minimum(16 * (lcp + 1), 64 * torch.ceil(torch.log2(nb.double() + 2)).long()).sum().item()
+    res["tree"] = int(32 * N + 192 * N + lc + 32 * N)
+    U = int((nb - lcp).sum().item())
+    for name, key, unit in (("lpm.radix", "hit_radix", 1), ("lpm.hash", "hit_hash", 16)):
+        if out[key] is None:
+            continue
+        hs = out[key].long()[order]
+        prev = torch.cat([torch.zeros(1, dtype=torch.long, device=hs.device), hs[:-1]])
+        R = int(((prev // 16 >= lcp) | (lcp == 0)).sum().item())
+        if name == "lpm.radix":
+            ht = int(torch.clamp(hs - 16 * lcp, min=0).sum().item())
+            res[name] = 8 * ht + 96 * R + 16 * N
+        else:
+            hb = int(torch.clamp(hs // 16 - lcp, min=0).sum().item())
+            res[name] = 40 * (hb + R) + 16 * N
+    dplus = int((out["demand"] > 0).sum().item()) if out["demand"] is not None else 0
+    res["demand"] = 40 * U + 32 * dplus + 4 * S
+    res["rank"] = 208 * N
+    res["_U"] = U
+    return res
+
+
+SLOT_TO_CALL = {"hash.nb_scan": "hash", "hash.content": "hash.content", "hash.chain": "hash.chain",
+                "tree.persistent": "tree", "lpm.radix_walk": "lpm.radix", "lpm.hash_probe": "lpm.hash",
+                "lpm.resolve_scan": None, "demand.count": "demand", "rank.clpm_sort": "rank"}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(workload: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        return json.load(open(p)).get(workload)
+    except Exception:
+        return None
+
+
+# ------------------------------------------------------------------------------------------
+# the oracle as the CPU baseline / reference arm (the only code here that touches oracle/)
+# ------------------------------------------------------------------------------------------
+def oracle_pass(wl, cache, n_sample: int):
+    """The oracle as it stands, on the first n_sample requests of the workload against the same
+    cache.  Returns seconds for one pass of the whole path."""
+    import oracle
+    sub = wl.queue.select(np.arange(n_sample))
+    toks, off = sub.materialize_np()
+    arrival = np.ascontiguousarray(wl.arrival[:n_sample])
+    radix = None
+    if cache.radix is not None:
+        r = cache.radix
+        radix = oracle.Radix(r.c_tokens, r.n_tok_off, r.n_tok_len, r.n_child_off, r.e_first_tok, r.e_child)
+    t0 = time.perf_counter()
+    bo, h = oracle.block_hash(toks, off, 16, 0)
+    tree = oracle.pending_tree(h, bo)
+    hr = oracle.lpm_radix(toks, off, radix) if radix is not None else None
+    hh = oracle.lpm_hash(h, bo, cache.t_keys)
+    oracle.demand(h, bo, cache.t_keys)
+    oracle.clpm_order(hr if hr is not None else hh, tree.cluster_size, arrival)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(wl, cache, budget_s: float):
+    import oracle
+    n = min(wl.N, 2048)
+    dt = oracle_pass(wl, cache, n)
+    # scale the sample to the time budget (the fixed cost of the demand map does not scale)
+    if wl.N > n:
+        n2 = int(min(wl.N, max(n, n * budget_s / max(dt, 1e-3) * 0.5)))
+        if n2 > n:
+            n = n2
+            dt = oracle_pass(wl, cache, n)
+    return {"value": n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "first %d of %d requests of the same workload, same cache, one pass of "
+                      "hash+tree+lpm(radix,hash)+demand+rank in %.2f s" % (n, wl.N, dt)}
+
+
+def cpu_inputs(cfg, seed, small):
+    """Workload + cache built with the oracle's hash (reference arm: no CUDA anywhere)."""
+    import oracle
+    wl = W.make(cfg, seed=seed, small=small)
+    cache = W.build_cache(wl, lambda t, o: oracle.block_hash(t, o, 16, 0))
+    return wl, cache
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    wl, cache = cpu_inputs(args.config, args.seed, args.small)
+    n = min(wl.N, 2048)
+    dt = oracle_pass(wl, cache, n)
+    n = int(min(wl.N, max(n, n * 4.0 / max(dt, 1e-3) * 0.5)))  # ~4 s per step
+    for _ in range(args.warmup):
+        oracle_pass(wl, cache, n)
+    t = 0.0
+    for _ in range(args.steps):
+        t += oracle_pass(wl, cache, n)
+    value = n * args.steps / t
+    sample = "each step = the oracle on the first %d of %d requests" % (n, wl.N)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64/int32",
+            "data": "synthetic", "gpu_launches": 0,
+            "config": {"workload": CONFIG_NAMES[args.config] + (" (small)" if args.small else ""),
+                       "N": wl.N, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(),
+                             "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------
+def run_peek(args):
+    import torch.distributed as dist
+    from paper_2607_02525_b200 import binding as B
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl peek needs a CUDA device (there is no CPU path)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    B.lib()  # fail loudly now if libpeek.so is missing
+
+    # each rank owns an independent batch (its own queue and cache replica): weak scaling, no
+    # data-path collective
+    inp = build_inputs(args.config, args.seed + 1000 * rank, args.small, dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 1)):
+        out = step(inp)
+    torch.cuda.synchronize()
+    launches0 = B.launch_count()
+    B.profile_enable(True)
+    B.profile_read(reset=True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    evs = []
+    for _ in range(args.steps):
+        flush.zero_()  # L2 flush between timed iterations, outside the event pairs
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        out = step(inp)
+        e1.record()
+        evs.append((e0, e1))
+    barrier()
+    t_ms = sum(a.elapsed_time(b) for a, b in evs)
+    prof = B.profile_read(reset=True)
+    B.profile_enable(False)
+    launches = (B.launch_count() - launches0) // max(args.steps, 1)
+    # keep the same load running ~1.5 s more so the clock sampler sees it (not timed)
+    t_end = time.time() + 1.5
+    while time.time() < t_end:
+        step(inp)
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+    tt = torch.tensor([t_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_ms = float(tt.item())
+    sum_hit = int(out["hit"].long().sum().item())
+
+    # end to end: host buffers in, results out, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        h_tok = inp.tok.cpu().pin_memory()
+        h_off = inp.off.cpu().pin_memory()
+        d_tok = torch.empty_like(inp.tok)
+        d_off = torch.empty_like(inp.off)
+        h_hit = torch.empty(inp.N, dtype=torch.int32).pin_memory()
+        h_ord = torch.empty(inp.N, dtype=torch.int32).pin_memory()
+        h_dem = torch.empty(inp.S, dtype=torch.int32).pin_memory()
+
+        def e2e_step():
+            d_tok.copy_(h_tok, non_blocking=True)
+            d_off.copy_(h_off, non_blocking=True)
+            o = step(inp, d_tok, d_off)
+            h_hit.copy_(o["hit"], non_blocking=True)
+            h_ord.copy_(o["clpm"], non_blocking=True)
+            h_dem.copy_(o["demand"], non_blocking=True)
+        e2e_step()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        e1.record()
+        barrier()
+        te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * inp.N * args.e2e_steps / (float(te.item()) * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(h_tok.numel() * 4 + h_off.numel() * 8),
+               "d2h_bytes_per_step": int(inp.N * 8 + inp.S * 4), "steps": args.e2e_steps,
+               "ms_per_step": float(te.item()) / args.e2e_steps}
+        del h_tok, d_tok
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # roofline of the dominant kernel group
+    balg = algorithmic_bytes(inp, out)
+    peak, peak_src = measured_peak()
+    calls = {}
+    for slot, (ms, groups) in prof.items():
+        call = SLOT_TO_CALL.get(slot)
+        per = ms / max(groups, 1) * (groups / max(args.steps, 1)) if groups else 0.0  # ms per step
+        calls[slot] = {"ms_per_step": per, "share": ms / t_ms if t_ms else None}
+        if call and call in balg and per > 0:
+            calls[slot]["alg_bytes"] = balg[call]
+            calls[slot]["alg_GBps"] = balg[call] / (per * 1e-3) / 1e9
+    dom = max(prof, key=lambda s: prof[s][0])
+    dom_call = SLOT_TO_CALL.get(dom)
+    dom_ms = prof[dom][0] / max(prof[dom][1], 1)
+    achieved = balg.get(dom_call, 0) / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
+    wname = CONFIG_NAMES[args.config] + (" (small)" if args.small else "")
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic(wname),
+                "alg_bytes_per_launch": balg.get(dom_call), "ms_per_launch": dom_ms}
+    line = {"metric": METRIC, "value": world * inp.N * args.steps / (t_ms * 1e-3), "unit": UNIT,
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64/int32",
+            "data": "synthetic",
+            "config": {"workload": wname, "N_per_gpu": inp.N, "tokens_per_gpu": inp.T, "blocks_per_gpu": inp.NB,
+                       "table_slots": inp.S, "radix_nodes": inp.cache.radix.V if inp.cache.radix is not None else 0,
+                       "block_size": 16, "parallelism": "independent batches per GPU, no collective",
+                       "l2": "256 MB buffer written between timed steps; inputs %.1f GB" % (inp.T * 4 / 1e9)},
+            "tokens_matched_per_s": world * sum_hit * args.steps / (t_ms * 1e-3),
+            "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roofline, "calls": calls}
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(inp.wl, inp.cache, args.cpu_seconds)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_peek(args)
+
+
+if __name__ == "__main__":
+    main()

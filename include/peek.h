@@ -172,6 +172,18 @@ peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* blk_off, int
                              const int32_t* cluster_size, const int32_t* arrival, int32_t* demand,
                              int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream);
 
+/* ---- tracing (CUDA events per kernel group) --------------------------- */
+/* Off by default.  When on, every kernel group a call enqueues is bracketed by a pair of CUDA
+ * events on the caller's stream (up to 512 pairs per slot between reads; later ones are dropped).
+ * peek_profile_read synchronises on the recorded events of `slot`, returns their summed elapsed
+ * milliseconds and the number of bracketed groups [host out], and optionally resets the slot.
+ * peek_launch_count: kernels this library has launched in this process (always counted). */
+void peek_profile_enable(int32_t on);
+int32_t peek_profile_slots(void);
+const char* peek_profile_name(int32_t slot);
+peek_status peek_profile_read(int32_t slot, double* total_ms, int64_t* groups, int32_t reset);
+int64_t peek_launch_count(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,6 +19,8 @@ _lib = None
 
 CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
+           "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
+           "peek_launch_count",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank"]
 
 
@@ -234,3 +236,32 @@ def peek_demand_rank(hashes=None, blk_off=None, tree: Optional[PendingTree] = No
                                 _ptr(arrival), _ptr(demand), _ptr(out), _ptr(ws), nbytes, _stream())
     _check(st, "peek_demand_rank")
     return demand, out
+
+
+# ---- tracing (include/peek.h "tracing") ---------------------------------------------------
+def profile_enable(on: bool) -> None:
+    L = lib()
+    L.peek_profile_enable.argtypes = [ctypes.c_int32]
+    L.peek_profile_enable(1 if on else 0)
+
+
+def profile_read(reset: bool = True) -> dict:
+    """{slot name: (total_ms, groups)} for the kernel groups recorded since the last reset."""
+    L = lib()
+    L.peek_profile_name.restype = ctypes.c_char_p
+    L.peek_profile_name.argtypes = [ctypes.c_int32]
+    L.peek_profile_read.restype = ctypes.c_int32
+    L.peek_profile_read.argtypes = [ctypes.c_int32, ctypes.POINTER(ctypes.c_double),
+                                    ctypes.POINTER(ctypes.c_int64), ctypes.c_int32]
+    out = {}
+    for s in range(int(L.peek_profile_slots())):
+        ms, n = ctypes.c_double(0), ctypes.c_int64(0)
+        _check(L.peek_profile_read(s, ctypes.byref(ms), ctypes.byref(n), 1 if reset else 0), "peek_profile_read")
+        out[L.peek_profile_name(s).decode()] = (float(ms.value), int(n.value))
+    return out
+
+
+def launch_count() -> int:
+    L = lib()
+    L.peek_launch_count.restype = ctypes.c_int64
+    return int(L.peek_launch_count())

@@ -27,6 +27,40 @@ int sm_count() {
     return n;
 }
 
+// ---- tracing ---------------------------------------------------------------------------
+static const char* const g_prof_names[PROF_NSLOTS] = {
+    "hash.nb_scan", "hash.content", "hash.chain", "tree.persistent", "lpm.radix_walk", "lpm.hash_probe",
+    "lpm.resolve_scan", "demand.count", "rank.clpm_sort"};
+static constexpr int PROF_RING = 512;
+struct ProfSlotState {
+    cudaEvent_t ev[PROF_RING][2];
+    int created, used;
+};
+static ProfSlotState g_prof[PROF_NSLOTS];
+static bool g_prof_on = false;
+static long long g_launches = 0;
+
+void prof_begin(int slot, cudaStream_t st) {
+    if (!g_prof_on) return;
+    ProfSlotState& p = g_prof[slot];
+    if (p.used >= PROF_RING) return;
+    if (p.used >= p.created) {
+        if (cudaEventCreate(&p.ev[p.created][0]) != cudaSuccess) return;
+        if (cudaEventCreate(&p.ev[p.created][1]) != cudaSuccess) return;
+        p.created++;
+    }
+    cudaEventRecord(p.ev[p.used][0], st);
+}
+
+void prof_end(int slot, cudaStream_t st, int launches) {
+    g_launches += launches;
+    if (!g_prof_on) return;
+    ProfSlotState& p = g_prof[slot];
+    if (p.used >= PROF_RING || p.used >= p.created) return;
+    cudaEventRecord(p.ev[p.used][1], st);
+    p.used++;
+}
+
 i64 block_hash_ws_bytes(i64 N);
 i64 lpm_ws_bytes(i64 N);
 i64 pending_tree_ws_bytes(i64 N);
@@ -70,3 +104,28 @@ extern "C" peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t 
     if (*out_bytes < 256) *out_bytes = 256;
     return PEEK_OK;
 }
+
+extern "C" void peek_profile_enable(int32_t on) { peek::g_prof_on = on != 0; }
+extern "C" int32_t peek_profile_slots(void) { return peek::PROF_NSLOTS; }
+extern "C" const char* peek_profile_name(int32_t slot) {
+    return (slot >= 0 && slot < peek::PROF_NSLOTS) ? peek::g_prof_names[slot] : "";
+}
+extern "C" peek_status peek_profile_read(int32_t slot, double* total_ms, int64_t* groups, int32_t reset) {
+    if (slot < 0 || slot >= peek::PROF_NSLOTS || !total_ms || !groups) {
+        peek::set_error("peek_profile_read: bad argument");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    peek::ProfSlotState& p = peek::g_prof[slot];
+    double tot = 0;
+    for (int i = 0; i < p.used; ++i) {
+        PEEK_CUDA(cudaEventSynchronize(p.ev[i][1]));
+        float ms = 0;
+        PEEK_CUDA(cudaEventElapsedTime(&ms, p.ev[i][0], p.ev[i][1]));
+        tot += ms;
+    }
+    *total_ms = tot;
+    *groups = p.used;
+    if (reset) p.used = 0;
+    return PEEK_OK;
+}
+extern "C" int64_t peek_launch_count(void) { return peek::g_launches; }

@@ -20,6 +20,20 @@ void set_error(const char* fmt, ...);
 peek_status cuda_fail(cudaError_t e, const char* what);
 int sm_count();  // SMs of the current device (148 on B200)
 
+// tracing slots (peek_profile_*)
+enum ProfSlot {
+    PROF_HASH_SCAN = 0, PROF_HASH_CONTENT, PROF_HASH_CHAIN, PROF_TREE, PROF_LPM_RADIX, PROF_LPM_HASH,
+    PROF_LPM_RESOLVE, PROF_DEMAND, PROF_RANK, PROF_NSLOTS
+};
+void prof_begin(int slot, cudaStream_t st);
+void prof_end(int slot, cudaStream_t st, int launches);
+struct Prof {  // brackets the kernels launched during its lifetime
+    int slot, launches;
+    cudaStream_t st;
+    Prof(int s, cudaStream_t stream, int n) : slot(s), launches(n), st(stream) { prof_begin(slot, st); }
+    ~Prof() { prof_end(slot, st, launches); }
+};
+
 #define PEEK_CUDA(call)                                            \
     do {                                                           \
         cudaError_t e__ = (call);                                  \

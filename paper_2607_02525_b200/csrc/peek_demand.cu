@@ -169,6 +169,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
     if (demand) {
         MinTree mt;
         mintree_layout(mt, lcp, N, mt_buf);
+        Prof pr(PROF_DEMAND, st, mt.levels);
         for (int k = 1; k < mt.levels; ++k) {
             i64 warps = mt.n[k];
             unsigned grid = (unsigned)((warps * 32 + 255) / 256);
@@ -186,6 +187,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
         if (want < grid) grid = (int)(want < 1 ? 1 : want);
         PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, sizeof(RankCtl), st));
         void* params[] = {&A};
+        Prof pr(PROF_RANK, st, 1);
         PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort, dim3(grid), dim3(PK_THREADS), params, 0, st));
     }
     PEEK_CUDA(cudaGetLastError());

@@ -212,17 +212,26 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
     Arena a(ws);
     i64 nchunks = (N + SCAN_CHUNK - 1) / SCAN_CHUNK;
     i64* partial = a.take<i64>(nchunks + 1);
-    k_nb_partial<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial);
-    k_scan_partials<<<1, 1024, 0, st>>>(partial, nchunks);
-    k_nb_apply<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial, blk_off);
+    {
+        Prof pr(PROF_HASH_SCAN, st, 3);
+        k_nb_partial<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial);
+        k_scan_partials<<<1, 1024, 0, st>>>(partial, nchunks);
+        k_nb_apply<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial, blk_off);
+    }
     if (hashes_capacity > 0) {
         // NB is only known on the device; the grid is sized for the caller's capacity (>= NB).
         i64 warps = (hashes_capacity + TILE_BLOCKS - 1) / TILE_BLOCKS;
         i64 ctas = (warps * 32 + HB_THREADS - 1) / HB_THREADS;
-        k_block_content<<<(unsigned)ctas, HB_THREADS, 0, st>>>(tokens, tok_off, blk_off, N, hashes,
-                                                              hashes_capacity);
-        k_block_chain<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(blk_off, N, seed, hashes,
+        {
+            Prof pr(PROF_HASH_CONTENT, st, 1);
+            k_block_content<<<(unsigned)ctas, HB_THREADS, 0, st>>>(tokens, tok_off, blk_off, N, hashes,
                                                                   hashes_capacity);
+        }
+        {
+            Prof pr(PROF_HASH_CHAIN, st, 1);
+            k_block_chain<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(blk_off, N, seed, hashes,
+                                                                      hashes_capacity);
+        }
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;

@@ -324,19 +324,27 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
     if (hit_radix) {
         RadixDev R{radix->c_tokens, radix->n_tok_off, radix->n_tok_len,
                    radix->n_child_off, radix->e_first_tok, radix->e_child};
-        k_lpm_radix<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, order, lcp,
-                                                       tree ? Wr : hit_radix);
+        {
+            Prof pr(PROF_LPM_RADIX, st, 1);
+            k_lpm_radix<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, order, lcp,
+                                                           tree ? Wr : hit_radix);
+        }
         if (tree) {
+            Prof pr(PROF_LPM_RESOLVE, st, 3);
             k_resolve_partial<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(lcp, Wr, N, partial);
             k_resolve_scan<<<1, 1024, 0, st>>>(partial, nchunks);
             k_resolve_apply<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(order, lcp, Wr, N, partial, hit_radix);
         }
     }
     if (hit_hash) {
-        k_lpm_hash<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys,
-                                                      (u64)(table->S - 1), order, lcp,
-                                                      tree ? Wh : hit_hash);
+        {
+            Prof pr(PROF_LPM_HASH, st, 1);
+            k_lpm_hash<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys,
+                                                          (u64)(table->S - 1), order, lcp,
+                                                          tree ? Wh : hit_hash);
+        }
         if (tree) {
+            Prof pr(PROF_LPM_RESOLVE, st, 3);
             k_resolve_partial<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(lcp, Wh, N, partial);
             k_resolve_scan<<<1, 1024, 0, st>>>(partial, nchunks);
             k_resolve_apply<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(order, lcp, Wh, N, partial, hit_hash);

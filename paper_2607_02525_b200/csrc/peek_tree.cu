@@ -347,6 +347,7 @@ extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* 
     tree_layout(a, N, MAX_GRID, A);
     PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, sizeof(TreeCtl), st));
     void* params[] = {&A};
+    Prof pr(PROF_TREE, st, 1);
     PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(PK_THREADS), params, 0, st));
     return PEEK_OK;
 }
