@@ -75,7 +75,8 @@ peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t T, int64_t 
                                  int64_t V, int64_t* out_bytes);
 
 /* ---- a1: chained block hash ----------------------------------------- */
-/* tokens  int32[T]  CSR token pool, request r = tokens[tok_off[r] .. tok_off[r+1])
+/* tokens  int32[T]  CSR token pool, request r = tokens[tok_off[r] .. tok_off[r+1]); the pointer must
+ *                    be 16-byte aligned (the kernel stages tokens with 16-byte bulk copies)
  * tok_off int64[N+1] monotone, tok_off[0] >= 0
  * seed    k_{-1} of every chain
  * blk_off int64[N+1] OUT exclusive prefix sum of nb_r = floor(len_r / block_size)

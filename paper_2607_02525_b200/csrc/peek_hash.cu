@@ -1,13 +1,9 @@
 // peek_hash.cu — a1 peek_block_hash: chained per-block hashes (R1).
 //
-// Three steps, all HBM-streaming:
-//   nb_scan      blk_off = exclusive prefix sum of floor(len_r / B)      (3 small launches)
-//   content      S_i = sum_j (tok+1) * M_j for EVERY block, flattened over the global block
-//                index so the token stream is read with coalesced 128-bit loads regardless of
-//                request lengths; 4 lanes per 16-token block, 2-step shuffle reduce
-//   chain        k_i = mix64(k_{i-1} ^ mix64(S_i)) in place, one thread per request (the chain is
-//                inherently serial per request; both mixers run here so the streaming kernel
-//                stays far below the integer-issue ceiling)
+// Two steps:
+//   nb_scan   blk_off = exclusive prefix sum of floor(len_r / B)                 (3 small launches)
+//   fused     k_block_hash_fused: tokens -> per-block sums -> chained hashes in ONE pass over HBM
+//             (1-D bulk TMA staging, thread-per-block sums, lane-per-request chain; see below)
 #include "peek_common.cuh"
 
 namespace peek {
@@ -43,8 +39,10 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_nb_partial(const i64* __restri
 }
 
 // single CTA: exclusive scan of partial[0..n) in place
-__global__ void __launch_bounds__(1024) k_scan_partials(i64* __restrict__ partial, i64 n) {
+__global__ void __launch_bounds__(1024) k_scan_partials(i64* __restrict__ partial, i64 n,
+                                                        unsigned long long* __restrict__ counter) {
     __shared__ i64 sm[34];
+    if (threadIdx.x == 0) *counter = 0;  // request queue head of k_block_hash_fused
     i64 carry = 0;
     for (i64 b = 0; b < n; b += 1024) {
         i64 i = b + threadIdx.x;
@@ -81,111 +79,289 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_nb_apply(const i64* __restrict
     }
 }
 
-// ---- content ---------------------------------------------------------------------------
-static constexpr int HB_THREADS = 256;
-static constexpr int TILE_BLOCKS = 128;  // token blocks per warp tile (8 KB of tokens)
-static constexpr int UNROLL = 4;         // warp steps (8 blocks each) in flight
+// ---- fused content + chain ----------------------------------------------------------------
+// One persistent kernel, HF_WARPS independent warps per CTA, one CTA per SM.  Lane l of a warp owns
+// one request at a time (taken from a global counter) and carries its chain state k in a register.
+// A round of a warp:
+//   A  for every owning lane q: the next chunk of <= 32 blocks (<= 2 KB of tokens) of q's request is
+//      staged in shared memory by ONE 1-D bulk TMA copy (cp.async.bulk + mbarrier, HF_STAGES deep
+//      ring per warp), then lane j computes block j of the chunk on its own: 16 multiply-adds from
+//      four conflict-free 128-bit shared loads, no cross-lane reduction; c = mix64(S) goes to the
+//      warp's c-buffer in shared memory
+//   B  every lane runs the serial chain k = mix64(k ^ c) over ITS request's chunk (32 requests per
+//      warp in parallel - the chain is inherently serial per request, so lanes = requests)
+//   C  the chunk's k values are written to `hashes` with coalesced 256-byte stores
+// so tokens are read from HBM once and only the final hashes are written: 4T + 8NB bytes.
+//
+// Alignment: a request starts at an arbitrary token, so a chunk starts `a` = 0..3 words past a
+// 16-byte boundary.  The copy fetches the 16-byte aligned superset; row j = staged bytes
+// [64j, 64j+64).  Block j is words a..15 of row j plus words 0..a-1 of row j+1; lane j computes
+// both parts of ITS row (U_j for block j, Q_j for block j-1) with the multipliers rotated by a,
+// and S_j = U_j + Q_{j+1} takes one shuffle.
+// Bank conflicts: rows are 64 bytes apart, so lane j reads its four 16-byte vectors in the rotated
+// order (c + (j>>1)) & 3 and keeps its multipliers pre-rotated the same way (M[c][e] below).
+static constexpr int HF_WARPS = 12;
+static constexpr int HF_THREADS = HF_WARPS * 32;
+static constexpr int HF_STAGES = 4;
+static constexpr int HF_STAGE_BYTES = 2176;          // 2048 + 16 rounded up to a multiple of 128
+static constexpr int HF_CROW = 33;                   // c-buffer row pitch in u64 (32 + 1: no conflicts)
+static constexpr int HF_WARP_BYTES = HF_STAGES * HF_STAGE_BYTES + 32 * HF_CROW * 8 + 64;
+static constexpr int HF_SMEM_BYTES = HF_WARPS * HF_WARP_BYTES + 128;
 
-// 4 tokens of this lane's quarter-block, from up to two 16-byte aligned vectors
-__device__ __forceinline__ void pick4(const int4& v, const int4& n, int a, u32 t[4]) {
-    if (a == 0) { t[0] = v.x; t[1] = v.y; t[2] = v.z; t[3] = v.w; }
-    else if (a == 1) { t[0] = v.y; t[1] = v.z; t[2] = v.w; t[3] = n.x; }
-    else if (a == 2) { t[0] = v.z; t[1] = v.w; t[2] = n.x; t[3] = n.y; }
-    else { t[0] = v.w; t[1] = n.x; t[2] = n.y; t[3] = n.z; }
+__device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(u32 bar, u32 count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(u32 bar, u32 bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(u32 dst, const void* src, u32 bytes, u32 bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u32 bar, u32 parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(u32 addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
 }
 
-__global__ void __launch_bounds__(HB_THREADS) k_block_content(const i32* __restrict__ tokens,
-                                                             const i64* __restrict__ tok_off,
-                                                             const i64* __restrict__ blk_off, i64 N,
-                                                             u64* __restrict__ hashes, i64 cap) {
-    const int lane = threadIdx.x & 31;
-    const int quad = lane >> 2, p = lane & 3;
-    const i64 NB = blk_off[N];
-    const i64 warp = ((i64)blockIdx.x * HB_THREADS + threadIdx.x) >> 5;
-    i64 x = warp * TILE_BLOCKS;
-    if (x >= NB) return;
-    const i64 x_end = min(x + TILE_BLOCKS, NB);
-    const u64 m0 = c_M[4 * p], m1 = c_M[4 * p + 1], m2 = c_M[4 * p + 2], m3 = c_M[4 * p + 3];
-
-    // request holding global block x: largest r with blk_off[r] <= x (warp-uniform search)
-    i64 lo = 0, hi = N;  // invariant blk_off[lo] <= x < blk_off[hi]
-    while (hi - lo > 1) {
-        i64 mid = (lo + hi) >> 1;
-        if (blk_off[mid] <= x) lo = mid; else hi = mid;
-    }
-    i64 r = lo;
-    while (x < x_end) {
-        i64 rb = blk_off[r], re = blk_off[r + 1];
-        while (re <= x) { ++r; rb = re; re = blk_off[r + 1]; }  // skip requests with no blocks left
-        const i64 cnt = min(re, x_end) - x;                       // blocks of request r in this tile
-        const i32* src = tokens + tok_off[r] + (x - rb) * B16;   // first token of block x
-        const int a = (int)(((uintptr_t)src >> 2) & 3);          // misalignment in tokens
-        const int4* vbase = (const int4*)(src - a);              // 16-byte aligned
-        for (i64 s0 = 0; s0 < cnt; s0 += 8 * UNROLL) {
-            int4 v[UNROLL], n[UNROLL];
+// Sum over this lane's 64-byte row with the multipliers rotated by A words: returns U (the part
+// of block j) and *qown (the part of block j-1: the first A words of the row).  V[c] is the row's
+// physical vector (c + x) & 3, M[c][e] = pos_mult(4 * ((c + x) & 3) + e), c0 = (4 - x) & 3 is the
+// register that holds physical vector 0.
+template <int A>
+__device__ __forceinline__ u64 row_sum(const uint4 (&V)[4], const u64 (&M)[4][4], int c0, u64* qown) {
+    u64 acc0 = 0, acc1 = 0;
+    u64 W[4] = {0, 0, 0, 0};
 #pragma unroll
-            for (int u = 0; u < UNROLL; ++u) {
-                i64 b = s0 + u * 8 + quad;  // block within the run
-                bool act = b < cnt;
-                v[u] = make_int4(0, 0, 0, 0);
-                n[u] = make_int4(0, 0, 0, 0);
-                if (act) v[u] = ld_stream_v4(vbase + b * 4 + p);
-            }
-            if (a != 0) {
+    for (int c = 0; c < 4; ++c) {
+        const u32 w[4] = {V[c].x, V[c].y, V[c].z, V[c].w};
 #pragma unroll
-                for (int u = 0; u < UNROLL; ++u) {
-                    i64 b = s0 + u * 8 + quad;
-                    bool act = b < cnt;
-                    n[u].x = __shfl_down_sync(0xffffffffu, v[u].x, 1);
-                    n[u].y = __shfl_down_sync(0xffffffffu, v[u].y, 1);
-                    n[u].z = __shfl_down_sync(0xffffffffu, v[u].z, 1);
-                    bool nxt_act = (s0 + u * 8 + ((lane + 1) >> 2)) < cnt;
-                    if (act && (lane == 31 || !nxt_act)) {
-                        int4 e = ld_stream_v4(vbase + b * 4 + p + 1);
-                        n[u].x = e.x; n[u].y = e.y; n[u].z = e.z;
-                    }
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < UNROLL; ++u) {
-                i64 b = s0 + u * 8 + quad;
-                u32 t[4];
-                pick4(v[u], n[u], a, t);
-                u64 s = (u64)t[0] * m0 + (u64)t[1] * m1 + (u64)t[2] * m2 + (u64)t[3] * m3;
-                s += __shfl_xor_sync(0xffffffffu, s, 1);
-                s += __shfl_xor_sync(0xffffffffu, s, 2);
-                if (p == 0 && b < cnt && x + b < cap) hashes[x + b] = s + SUM_M;
+        for (int e = 0; e < 4; ++e) {
+            if (e >= A) {
+                if (e & 1) acc1 += (u64)w[e] * M[c][e - A];
+                else acc0 += (u64)w[e] * M[c][e - A];
+            } else {
+                W[c] += (u64)w[e] * M[(c + 3) & 3][4 + e - A];
             }
         }
-        x += cnt;
     }
+    u64 tot = acc0 + acc1;
+    if (A > 0) {
+        u64 q = c0 == 0 ? W[0] : (c0 == 1 ? W[1] : (c0 == 2 ? W[2] : W[3]));
+        tot += (W[0] + W[1]) + (W[2] + W[3]) - q;
+        *qown = q;
+    } else {
+        *qown = 0;
+    }
+    return tot;
 }
 
-// ---- chain -----------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_block_chain(const i64* __restrict__ blk_off, i64 N, u64 seed,
-                                                    u64* __restrict__ hashes, i64 cap) {
-    i64 r = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= N) return;
-    i64 b = blk_off[r], e = min(blk_off[r + 1], cap);
-    u64 k = seed;
-    for (; b + 4 <= e; b += 4) {
-        u64 s0 = hashes[b], s1 = hashes[b + 1], s2 = hashes[b + 2], s3 = hashes[b + 3];
-        u64 c0 = mix64(s0), c1 = mix64(s1), c2 = mix64(s2), c3 = mix64(s3);
-        k = mix64(k ^ c0); if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1; hashes[b] = k;
-        k = mix64(k ^ c1); if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1; hashes[b + 1] = k;
-        k = mix64(k ^ c2); if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1; hashes[b + 2] = k;
-        k = mix64(k ^ c3); if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1; hashes[b + 3] = k;
+// S - SUM_M of block `lane` of the staged chunk: own row's part plus the next row's first A words.
+template <int A>
+__device__ __forceinline__ u64 block_sum(const uint4 (&V)[4], const u64 (&M)[4][4], int c0, u32 sbase,
+                                         int lane, int n) {
+    u64 qown;
+    u64 U = row_sum<A>(V, M, c0, &qown);
+    if (A > 0) {
+        u64 qn = __shfl_down_sync(0xffffffffu, qown, 1);
+        if (lane == 31 && n == 32) {
+            // row 32 belongs to no lane: its first A words carry positions 16-A..15, which for
+            // lane 31 (x = 3) are M[0][4-A..3]
+            uint4 X = lds128(sbase + 2048u);
+            const u32 w[4] = {X.x, X.y, X.z, X.w};
+            qn = 0;
+#pragma unroll
+            for (int e = 0; e < A; ++e) qn += (u64)w[e] * M[0][4 - A + e];
+        }
+        U += qn;
     }
-    for (; b < e; ++b) {
-        k = mix64(k ^ mix64(hashes[b]));
-        if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1;
-        hashes[b] = k;
+    return U;
+}
+
+struct HashArgs {
+    const i32* tokens;
+    const i64* tok_off;
+    const i64* blk_off;
+    i64 N;
+    u64 seed;
+    u64* hashes;
+    i64 cap;
+    unsigned long long* counter;  // next request to hand out (zeroed by k_scan_partials)
+    int lanes_cap;                // owning lanes per warp (spreads few long requests over all warps)
+};
+
+__global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) {
+    extern __shared__ __align__(128) unsigned char hf_smem[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned FULL = 0xffffffffu;
+    const unsigned lt = (1u << lane) - 1u;
+    unsigned char* wbase = hf_smem + (size_t)wid * HF_WARP_BYTES;
+    const u32 stage0 = smem_u32(wbase);
+    u64* cbuf = (u64*)(wbase + HF_STAGES * HF_STAGE_BYTES);
+    const u32 bar0 = smem_u32(wbase + HF_STAGES * HF_STAGE_BYTES + 32 * HF_CROW * 8);
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < HF_STAGES; ++s) mbar_init(bar0 + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncwarp();
+
+    const int x = (lane >> 1) & 3, c0 = (4 - x) & 3;
+    u64 M[4][4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) M[c][e] = pos_mult(4 * ((c + x) & 3) + e);
+    const u32 rowoff = 64u * lane;
+    u32 voff[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) voff[c] = rowoff + 16u * ((c + x) & 3);
+
+    const char* pool_end = (const char*)(A.tokens + A.tok_off[A.N]);
+    const char* pool_end16 = (const char*)((uintptr_t)pool_end & ~(uintptr_t)15);
+
+    // lane state
+    bool own = false;
+    i32 pos = 0, nb = 0;
+    const char* tptr = nullptr;  // first token of the request
+    i64 obase = 0;
+    u64 k = 0;
+    bool exhausted = false;
+    u32 parity = 0;  // bit s = parity to wait for on stage s
+    int sI = 0, sC = 0;
+
+    for (;;) {
+        // ---- refill: lanes without a request take the next ones from the global counter ----
+        bool need = !own && lane < A.lanes_cap && !exhausted;
+        for (;;) {
+            unsigned m = __ballot_sync(FULL, need);
+            if (!m) break;
+            unsigned long long base = 0;
+            if (lane == 0) base = atomicAdd(A.counter, (unsigned long long)__popc(m));
+            base = __shfl_sync(FULL, base, 0);
+            if ((i64)base >= A.N) { exhausted = true; need = false; break; }
+            if (need) {
+                i64 r = (i64)base + __popc(m & lt);
+                if (r < A.N) {
+                    i64 b0 = A.blk_off[r], b1 = A.blk_off[r + 1];
+                    if (b1 > b0) {
+                        own = true; need = false;
+                        pos = 0; nb = (i32)(b1 - b0); obase = b0; k = A.seed;
+                        tptr = (const char*)(A.tokens + A.tok_off[r]);
+                    }
+                } else {
+                    need = false;
+                }
+            }
+        }
+        const unsigned active = __ballot_sync(FULL, own);
+        if (!active) break;
+        const i32 n_l = own ? min(32, nb - pos) : 0;
+        const char* a_l = tptr + (size_t)pos * 64;  // first token byte of this lane's chunk
+
+        // ---- phase A: stage chunks by TMA (HF_STAGES deep), one thread per block ----
+        auto issue = [&](int q) {
+            const i32 n = __shfl_sync(FULL, n_l, q);
+            const uintptr_t ad = (uintptr_t)__shfl_sync(FULL, (unsigned long long)(uintptr_t)a_l, q);
+            if (lane == 0) {
+                const u32 a4 = (u32)(ad & 15);
+                const char* src = (const char*)(ad - a4);
+                u32 bytes = 64u * n + (a4 ? 16u : 0u);
+                if (src + bytes > pool_end16) bytes = src < pool_end16 ? (u32)(pool_end16 - src) : 0u;
+                const u32 bar = bar0 + 8 * sI;
+                mbar_expect_tx(bar, bytes);
+                if (bytes) tma_load_1d(stage0 + sI * HF_STAGE_BYTES, src, bytes, bar);
+            }
+            sI = sI + 1 == HF_STAGES ? 0 : sI + 1;
+        };
+        unsigned im = active, cm = active;
+#pragma unroll
+        for (int s = 0; s < HF_STAGES - 1; ++s) {
+            if (im) { int q = __ffs(im) - 1; im &= im - 1; issue(q); }
+        }
+        while (cm) {
+            if (im) { int q = __ffs(im) - 1; im &= im - 1; issue(q); }
+            const int q = __ffs(cm) - 1;
+            cm &= cm - 1;
+            const i32 n = __shfl_sync(FULL, n_l, q);
+            const uintptr_t ad = (uintptr_t)__shfl_sync(FULL, (unsigned long long)(uintptr_t)a_l, q);
+            const int a = (int)((ad & 15) >> 2);
+            const u32 sbase = stage0 + sC * HF_STAGE_BYTES;
+            mbar_wait(bar0 + 8 * sC, (parity >> sC) & 1u);
+            parity ^= 1u << sC;
+            sC = sC + 1 == HF_STAGES ? 0 : sC + 1;
+            {   // the copy stops at the last 16-byte boundary inside the pool: fetch the rest by hand
+                const char* need_end = (const char*)ad + (size_t)n * 64;
+                if (need_end > pool_end16) {
+                    const char* src = (const char*)(ad - (ad & 15));
+                    const int words = (int)((need_end - pool_end16) >> 2);  // 1..3
+                    if (lane < words) {
+                        u32 v = *(const u32*)(pool_end16 + 4 * lane);
+                        asm volatile("st.shared.u32 [%0], %1;" ::"r"(sbase + (u32)(pool_end16 - src) + 4u * lane), "r"(v) : "memory");
+                    }
+                    __syncwarp();
+                }
+            }
+            uint4 V[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) V[c] = lds128(sbase + voff[c]);
+            u64 U;
+            switch (a) {
+                case 0: U = block_sum<0>(V, M, c0, sbase, lane, n); break;
+                case 1: U = block_sum<1>(V, M, c0, sbase, lane, n); break;
+                case 2: U = block_sum<2>(V, M, c0, sbase, lane, n); break;
+                default: U = block_sum<3>(V, M, c0, sbase, lane, n); break;
+            }
+            if (lane < n) cbuf[q * HF_CROW + lane] = mix64(U + SUM_M);
+            __syncwarp();  // stage sC-1 fully read before it is refilled; cbuf row visible
+        }
+
+        // ---- phase B: serial chain, lane = request ----
+        const i32 nmax = __reduce_max_sync(FULL, n_l);
+        u64* crow = cbuf + lane * HF_CROW;
+        for (i32 s = 0; s < nmax; ++s) {
+            if (s < n_l) {
+                k = mix64(k ^ crow[s]);
+                if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1;
+                crow[s] = k;
+            }
+        }
+        __syncwarp();
+
+        // ---- phase C: coalesced stores of the chunk's hashes ----
+        unsigned om = active;
+        while (om) {
+            const int q = __ffs(om) - 1;
+            om &= om - 1;
+            const i32 n = __shfl_sync(FULL, n_l, q);
+            const i64 ob = __shfl_sync(FULL, obase + pos, q);
+            if (lane < n && ob + lane < A.cap) A.hashes[ob + lane] = cbuf[q * HF_CROW + lane];
+        }
+        __syncwarp();
+        if (own) {
+            pos += n_l;
+            if (pos == nb) own = false;
+        }
     }
 }
 
 i64 block_hash_ws_bytes(i64 N) {
     Arena a(nullptr);
     a.take<i64>((N + SCAN_CHUNK - 1) / SCAN_CHUNK + 1);
+    a.take<unsigned long long>(1);
     return a.used;
 }
 
@@ -204,6 +380,10 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
         set_error("peek_block_hash: NULL argument");
         return PEEK_ERR_INVALID_ARG;
     }
+    if ((uintptr_t)tokens & 15) {
+        set_error("peek_block_hash: tokens must be 16-byte aligned");
+        return PEEK_ERR_INVALID_ARG;
+    }
     if (!ws || ((uintptr_t)ws & 255) || ws_bytes < block_hash_ws_bytes(N)) {
         set_error("peek_block_hash: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;
@@ -212,26 +392,31 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
     Arena a(ws);
     i64 nchunks = (N + SCAN_CHUNK - 1) / SCAN_CHUNK;
     i64* partial = a.take<i64>(nchunks + 1);
+    unsigned long long* counter = a.take<unsigned long long>(1);
     {
         Prof pr(PROF_HASH_SCAN, st, 3);
         k_nb_partial<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial);
-        k_scan_partials<<<1, 1024, 0, st>>>(partial, nchunks);
+        k_scan_partials<<<1, 1024, 0, st>>>(partial, nchunks, counter);
         k_nb_apply<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial, blk_off);
     }
     if (hashes_capacity > 0) {
-        // NB is only known on the device; the grid is sized for the caller's capacity (>= NB).
-        i64 warps = (hashes_capacity + TILE_BLOCKS - 1) / TILE_BLOCKS;
-        i64 ctas = (warps * 32 + HB_THREADS - 1) / HB_THREADS;
-        {
-            Prof pr(PROF_HASH_CONTENT, st, 1);
-            k_block_content<<<(unsigned)ctas, HB_THREADS, 0, st>>>(tokens, tok_off, blk_off, N, hashes,
-                                                                  hashes_capacity);
+        static bool attr_set = false;
+        if (!attr_set) {
+            PEEK_CUDA(cudaFuncSetAttribute(k_block_hash_fused, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           HF_SMEM_BYTES));
+            attr_set = true;
         }
-        {
-            Prof pr(PROF_HASH_CHAIN, st, 1);
-            k_block_chain<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(blk_off, N, seed, hashes,
-                                                                      hashes_capacity);
+        int grid = sm_count();
+        i64 warps = (i64)grid * HF_WARPS;
+        if (N < warps) {  // fewer requests than warps: no point in idle CTAs
+            grid = (int)((N + HF_WARPS - 1) / HF_WARPS);
+            warps = (i64)grid * HF_WARPS;
         }
+        i64 per_warp = (N + warps - 1) / warps;
+        HashArgs A{tokens, tok_off, blk_off, N, seed, hashes, hashes_capacity, counter,
+                   (int)(per_warp < 1 ? 1 : (per_warp > 32 ? 32 : per_warp))};
+        Prof pr(PROF_HASH_CONTENT, st, 1);
+        k_block_hash_fused<<<grid, HF_THREADS, HF_SMEM_BYTES, st>>>(A);
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;
