@@ -100,9 +100,15 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_nb_apply(const i64* __restrict
 // and S_j = U_j + Q_{j+1} takes one shuffle.
 // Bank conflicts: rows are 64 bytes apart, so lane j reads its four 16-byte vectors in the rotated
 // order (c + (j>>1)) & 3 and keeps its multipliers pre-rotated the same way (M[c][e] below).
-static constexpr int HF_WARPS = 12;
+#ifndef PEEK_HF_WARPS
+#define PEEK_HF_WARPS 15
+#endif
+#ifndef PEEK_HF_STAGES
+#define PEEK_HF_STAGES 3
+#endif
+static constexpr int HF_WARPS = PEEK_HF_WARPS;
 static constexpr int HF_THREADS = HF_WARPS * 32;
-static constexpr int HF_STAGES = 4;
+static constexpr int HF_STAGES = PEEK_HF_STAGES;
 static constexpr int HF_STAGE_BYTES = 2176;          // 2048 + 16 rounded up to a multiple of 128
 static constexpr int HF_CROW = 33;                   // c-buffer row pitch in u64 (32 + 1: no conflicts)
 static constexpr int HF_WARP_BYTES = HF_STAGES * HF_STAGE_BYTES + 32 * HF_CROW * 8 + 64;
@@ -225,41 +231,57 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
     for (int c = 0; c < 4; ++c)
 #pragma unroll
         for (int e = 0; e < 4; ++e) M[c][e] = pos_mult(4 * ((c + x) & 3) + e);
-    const u32 rowoff = 64u * lane;
     u32 voff[4];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) voff[c] = rowoff + 16u * ((c + x) & 3);
+    for (int c = 0; c < 4; ++c) voff[c] = 64u * lane + 16u * ((c + x) & 3);
 
     const char* pool_end = (const char*)(A.tokens + A.tok_off[A.N]);
     const char* pool_end16 = (const char*)((uintptr_t)pool_end & ~(uintptr_t)15);
 
-    // lane state
-    bool own = false;
+    // request owned by this lane
+    bool own = false, exhausted = false;
     i32 pos = 0, nb = 0;
     const char* tptr = nullptr;  // first token of the request
     i64 obase = 0;
-    u64 k = 0;
-    bool exhausted = false;
-    u32 parity = 0;  // bit s = parity to wait for on stage s
+    u64 k = A.seed;
+    // this lane's chunk of the round being staged: 16-byte aligned source, clipped copy size,
+    // meta = n | a << 8 | (words past the last 16-byte boundary of the pool) << 16
+    const char* c_src = nullptr;
+    u32 c_bytes = 0, c_meta = 0;
+    unsigned im = 0, cm = 0;  // lanes whose chunk is still to be issued / consumed
+    u32 parity = 0;           // bit s = parity to wait for on stage s
     int sI = 0, sC = 0;
 
-    for (;;) {
-        // ---- refill: lanes without a request take the next ones from the global counter ----
+    auto issue = [&]() {  // next chunk of `im` -> stage sI
+        const int q = __ffs(im) - 1;
+        im &= im - 1;
+        const uintptr_t src = (uintptr_t)__shfl_sync(FULL, (unsigned long long)(uintptr_t)c_src, q);
+        const u32 bytes = __shfl_sync(FULL, c_bytes, q);
+        if (lane == 0) {
+            const u32 bar = bar0 + 8 * sI;
+            mbar_expect_tx(bar, bytes);
+            if (bytes) tma_load_1d(stage0 + sI * HF_STAGE_BYTES, (const void*)src, bytes, bar);
+        }
+        sI = sI + 1 == HF_STAGES ? 0 : sI + 1;
+    };
+    // Take requests for the lanes that have none, describe every owning lane's next chunk and put
+    // the first HF_STAGES - 1 copies of the round in flight.  Returns false when nothing is left.
+    auto next_round = [&]() -> bool {
         bool need = !own && lane < A.lanes_cap && !exhausted;
         for (;;) {
-            unsigned m = __ballot_sync(FULL, need);
+            const unsigned m = __ballot_sync(FULL, need);
             if (!m) break;
             unsigned long long base = 0;
             if (lane == 0) base = atomicAdd(A.counter, (unsigned long long)__popc(m));
             base = __shfl_sync(FULL, base, 0);
-            if ((i64)base >= A.N) { exhausted = true; need = false; break; }
+            if ((i64)base >= A.N) { exhausted = true; break; }
             if (need) {
-                i64 r = (i64)base + __popc(m & lt);
+                const i64 r = (i64)base + __popc(m & lt);
                 if (r < A.N) {
-                    i64 b0 = A.blk_off[r], b1 = A.blk_off[r + 1];
+                    const i64 b0 = A.blk_off[r], b1 = A.blk_off[r + 1];
                     if (b1 > b0) {
                         own = true; need = false;
-                        pos = 0; nb = (i32)(b1 - b0); obase = b0; k = A.seed;
+                        pos = 0; nb = (i32)(b1 - b0); obase = b0;
                         tptr = (const char*)(A.tokens + A.tok_off[r]);
                     }
                 } else {
@@ -268,52 +290,49 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
             }
         }
         const unsigned active = __ballot_sync(FULL, own);
-        if (!active) break;
-        const i32 n_l = own ? min(32, nb - pos) : 0;
-        const char* a_l = tptr + (size_t)pos * 64;  // first token byte of this lane's chunk
-
-        // ---- phase A: stage chunks by TMA (HF_STAGES deep), one thread per block ----
-        auto issue = [&](int q) {
-            const i32 n = __shfl_sync(FULL, n_l, q);
-            const uintptr_t ad = (uintptr_t)__shfl_sync(FULL, (unsigned long long)(uintptr_t)a_l, q);
-            if (lane == 0) {
-                const u32 a4 = (u32)(ad & 15);
-                const char* src = (const char*)(ad - a4);
-                u32 bytes = 64u * n + (a4 ? 16u : 0u);
-                if (src + bytes > pool_end16) bytes = src < pool_end16 ? (u32)(pool_end16 - src) : 0u;
-                const u32 bar = bar0 + 8 * sI;
-                mbar_expect_tx(bar, bytes);
-                if (bytes) tma_load_1d(stage0 + sI * HF_STAGE_BYTES, src, bytes, bar);
+        if (!active) return false;
+        c_meta = 0;
+        if (own) {
+            const u32 n = (u32)min(32, nb - pos);
+            const uintptr_t ad = (uintptr_t)tptr + (size_t)pos * 64;
+            const u32 a4 = (u32)(ad & 15);
+            const char* need_end = (const char*)ad + 64 * n;
+            c_src = (const char*)(ad - a4);
+            c_bytes = 64u * n + (a4 ? 16u : 0u);
+            u32 tail = 0;
+            if (c_src + c_bytes > pool_end16) {  // the copy stops at the last 16-byte boundary of the pool
+                c_bytes = (u32)(pool_end16 - c_src);
+                if (need_end > pool_end16) tail = (u32)(need_end - pool_end16) >> 2;
             }
-            sI = sI + 1 == HF_STAGES ? 0 : sI + 1;
-        };
-        unsigned im = active, cm = active;
-#pragma unroll
-        for (int s = 0; s < HF_STAGES - 1; ++s) {
-            if (im) { int q = __ffs(im) - 1; im &= im - 1; issue(q); }
+            c_meta = n | (a4 >> 2) << 8 | tail << 16;
         }
+        im = cm = active;
+#pragma unroll
+        for (int s = 0; s < HF_STAGES - 1; ++s)
+            if (im) issue();
+        return true;
+    };
+
+    bool more = next_round();
+    while (more) {
+        // ---- phase A: one thread per block of each staged chunk ----
         while (cm) {
-            if (im) { int q = __ffs(im) - 1; im &= im - 1; issue(q); }
+            if (im) issue();
             const int q = __ffs(cm) - 1;
             cm &= cm - 1;
-            const i32 n = __shfl_sync(FULL, n_l, q);
-            const uintptr_t ad = (uintptr_t)__shfl_sync(FULL, (unsigned long long)(uintptr_t)a_l, q);
-            const int a = (int)((ad & 15) >> 2);
+            const u32 meta = __shfl_sync(FULL, c_meta, q);
+            const int n = meta & 0xff, a = (meta >> 8) & 3;
             const u32 sbase = stage0 + sC * HF_STAGE_BYTES;
             mbar_wait(bar0 + 8 * sC, (parity >> sC) & 1u);
             parity ^= 1u << sC;
             sC = sC + 1 == HF_STAGES ? 0 : sC + 1;
-            {   // the copy stops at the last 16-byte boundary inside the pool: fetch the rest by hand
-                const char* need_end = (const char*)ad + (size_t)n * 64;
-                if (need_end > pool_end16) {
-                    const char* src = (const char*)(ad - (ad & 15));
-                    const int words = (int)((need_end - pool_end16) >> 2);  // 1..3
-                    if (lane < words) {
-                        u32 v = *(const u32*)(pool_end16 + 4 * lane);
-                        asm volatile("st.shared.u32 [%0], %1;" ::"r"(sbase + (u32)(pool_end16 - src) + 4u * lane), "r"(v) : "memory");
-                    }
-                    __syncwarp();
+            if (meta >> 16) {  // last words of the pool, past its last 16-byte boundary: by hand
+                const u32 src_lo = __shfl_sync(FULL, (u32)(uintptr_t)c_src, q);
+                if (lane < (int)(meta >> 16)) {
+                    const u32 v = *(const u32*)(pool_end16 + 4 * lane);
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(sbase + ((u32)(uintptr_t)pool_end16 - src_lo) + 4u * lane), "r"(v) : "memory");
                 }
+                __syncwarp();
             }
             uint4 V[4];
 #pragma unroll
@@ -326,35 +345,46 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
                 default: U = block_sum<3>(V, M, c0, sbase, lane, n); break;
             }
             if (lane < n) cbuf[q * HF_CROW + lane] = mix64(U + SUM_M);
-            __syncwarp();  // stage sC-1 fully read before it is refilled; cbuf row visible
+            __syncwarp();  // the stage is fully read before it is refilled; cbuf row visible
         }
 
+        // ---- advance, and put the next round's first copies in flight before the chain ----
+        const i32 nB = (i32)(c_meta & 0xff);  // this round: chain steps of this lane, output position
+        const i64 outp = obase + pos;
+        const unsigned done = __ballot_sync(FULL, own);
+        bool fresh = false;
+        if (own) {
+            pos += nB;
+            if (pos == nb) { own = false; fresh = true; }
+        }
+        more = next_round();
+
         // ---- phase B: serial chain, lane = request ----
-        const i32 nmax = __reduce_max_sync(FULL, n_l);
+        const i32 nmax = __reduce_max_sync(FULL, nB);
         u64* crow = cbuf + lane * HF_CROW;
         for (i32 s = 0; s < nmax; ++s) {
-            if (s < n_l) {
+            if (s < nB) {
                 k = mix64(k ^ crow[s]);
                 if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1;
                 crow[s] = k;
             }
         }
+        if (fresh) k = A.seed;
         __syncwarp();
 
-        // ---- phase C: coalesced stores of the chunk's hashes ----
-        unsigned om = active;
+        // ---- phase C: coalesced stores of the round's hashes ----
+        const i64 room = A.cap - outp;
+        const i32 ncl = room < (i64)nB ? (room < 0 ? 0 : (i32)room) : nB;
+        u64* const outq = A.hashes + outp;
+        unsigned om = done;
         while (om) {
             const int q = __ffs(om) - 1;
             om &= om - 1;
-            const i32 n = __shfl_sync(FULL, n_l, q);
-            const i64 ob = __shfl_sync(FULL, obase + pos, q);
-            if (lane < n && ob + lane < A.cap) A.hashes[ob + lane] = cbuf[q * HF_CROW + lane];
+            const i32 n = __shfl_sync(FULL, ncl, q);
+            u64* o = (u64*)__shfl_sync(FULL, (unsigned long long)(uintptr_t)outq, q);
+            if (lane < n) o[lane] = cbuf[q * HF_CROW + lane];
         }
         __syncwarp();
-        if (own) {
-            pos += n_l;
-            if (pos == nb) own = false;
-        }
     }
 }
 
