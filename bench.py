@@ -115,6 +115,25 @@ class Inputs:
     pass
 
 
+def rank_seed(seed: int, rank: int) -> int:
+    """Each rank owns an independent batch: its own generator seed."""
+    return seed + 1000 * rank
+
+
+def max_over_ranks(ms: float, device, world: int) -> float:
+    """Device time of a multi-GPU step is the max over ranks (all-reduce MAX; a no-op at world 1)."""
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(units_per_rank: int, world: int, steps: int, ms: float) -> float:
+    """Whole-job units/s: every rank processes its own batch in the same (max) time."""
+    return world * units_per_rank * steps / (ms * 1e-3)
+
+
 def gpu_hash_fn(dev):
     """hash_fn for workloads.build_cache: the CUDA call (the product path never touches oracle/)."""
     from paper_2607_02525_b200 import binding as B
@@ -320,7 +339,7 @@ def run_peek(args):
 
     # each rank owns an independent batch (its own queue and cache replica): weak scaling, no
     # data-path collective
-    inp = build_inputs(args.config, args.seed + 1000 * rank, args.small, dev)
+    inp = build_inputs(args.config, rank_seed(args.seed, rank), args.small, dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
     def barrier():
@@ -357,10 +376,7 @@ def run_peek(args):
         step(inp)
         torch.cuda.synchronize()
     clocks = sampler.stop()
-    tt = torch.tensor([t_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_ms = float(tt.item())
+    t_ms = max_over_ranks(t_ms, dev, world)
     sum_hit = int(out["hit"].long().sum().item())
 
     # end to end: host buffers in, results out, copies inside the timed region
@@ -389,13 +405,11 @@ def run_peek(args):
             e2e_step()
         e1.record()
         barrier()
-        te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * inp.N * args.e2e_steps / (float(te.item()) * 1e-3), "unit": UNIT,
+        te_ms = max_over_ranks(e0.elapsed_time(e1), dev, world)
+        e2e = {"value": job_throughput(inp.N, world, args.e2e_steps, te_ms), "unit": UNIT,
                "h2d_bytes_per_step": int(h_tok.numel() * 4 + h_off.numel() * 8),
                "d2h_bytes_per_step": int(inp.N * 8 + inp.S * 4), "steps": args.e2e_steps,
-               "ms_per_step": float(te.item()) / args.e2e_steps}
+               "ms_per_step": te_ms / args.e2e_steps}
         del h_tok, d_tok
 
     if rank != 0:
@@ -421,7 +435,7 @@ def run_peek(args):
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic(wname),
                 "alg_bytes_per_launch": balg.get(dom_call), "ms_per_launch": dom_ms}
-    line = {"metric": METRIC, "value": world * inp.N * args.steps / (t_ms * 1e-3), "unit": UNIT,
+    line = {"metric": METRIC, "value": job_throughput(inp.N, world, args.steps, t_ms), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64/int32",
             "data": "synthetic",

@@ -173,6 +173,20 @@ peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* blk_off, int
                              const int32_t* cluster_size, const int32_t* arrival, int32_t* demand,
                              int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream);
 
+/* ---- options: tuning and test hooks ------------------------------------------------------- */
+/* Process-wide, not thread-safe against concurrent calls; results never depend on them.
+ * PEEK_OPT_LPM_STRATEGY  how peek_lpm co-descends when a tree view is given:
+ *     PEEK_LPM_AUTO (default)  dual-walk for N >= 32768, speculative below
+ *     PEEK_LPM_DUAL_WALK       a warp walks a run of sorted positions in order, carrying the
+ *                              predecessor's hit and cache path (Alg. 1's co-descent)
+ *     PEEK_LPM_SPECULATIVE     every position walks in parallel from its shared depth, a scan
+ *                              resolves which walks were needed
+ * PEEK_OPT_LPM_WINDOW    sorted positions per dual-walk window (0 = automatic)
+ * Unknown key or bad value -> PEEK_ERR_INVALID_ARG. */
+enum { PEEK_OPT_LPM_STRATEGY = 1, PEEK_OPT_LPM_WINDOW = 2 };
+enum { PEEK_LPM_AUTO = 0, PEEK_LPM_DUAL_WALK = 1, PEEK_LPM_SPECULATIVE = 2 };
+peek_status peek_set_option(int32_t key, int64_t value);
+
 /* ---- tracing (CUDA events per kernel group) --------------------------- */
 /* Off by default.  When on, every kernel group a call enqueues is bracketed by a pair of CUDA
  * events on the caller's stream (up to 512 pairs per slot between reads; later ones are dropped).

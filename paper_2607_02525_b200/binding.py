@@ -20,7 +20,7 @@ _lib = None
 CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
-           "peek_launch_count",
+           "peek_launch_count", "peek_set_option",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank"]
 
 
@@ -59,6 +59,8 @@ def lib():
         L.peek_version.restype = i32
         L.peek_workspace_bytes.restype = i32
         L.peek_workspace_bytes.argtypes = [i32, i64, i64, i64, i64, i64, ctypes.POINTER(i64)]
+        L.peek_set_option.restype = i32
+        L.peek_set_option.argtypes = [i32, i64]
         L.peek_block_hash.restype = i32
         L.peek_block_hash.argtypes = [vp, vp, i64, i32, u64, vp, vp, i64, vp, i64, vp]
         L.peek_lpm.restype = i32
@@ -236,6 +238,15 @@ def peek_demand_rank(hashes=None, blk_off=None, tree: Optional[PendingTree] = No
                                 _ptr(arrival), _ptr(demand), _ptr(out), _ptr(ws), nbytes, _stream())
     _check(st, "peek_demand_rank")
     return demand, out
+
+
+OPT_LPM_STRATEGY, OPT_LPM_WINDOW = 1, 2
+LPM_AUTO, LPM_DUAL_WALK, LPM_SPECULATIVE = 0, 1, 2
+
+
+def set_option(key: int, value: int) -> None:
+    """include/peek.h "options": tuning and test hooks; results never depend on them."""
+    _check(lib().peek_set_option(key, value), "peek_set_option")
 
 
 # ---- tracing (include/peek.h "tracing") ---------------------------------------------------

@@ -65,6 +65,7 @@ i64 block_hash_ws_bytes(i64 N);
 i64 lpm_ws_bytes(i64 N);
 i64 pending_tree_ws_bytes(i64 N);
 i64 demand_rank_ws_bytes(i64 N, i64 S);
+void lpm_set_option(int key, i64 v);
 
 }  // namespace peek
 
@@ -103,6 +104,16 @@ extern "C" peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t 
     }
     if (*out_bytes < 256) *out_bytes = 256;
     return PEEK_OK;
+}
+
+extern "C" peek_status peek_set_option(int32_t key, int64_t value) {
+    if ((key == PEEK_OPT_LPM_STRATEGY && value >= 0 && value <= 2) ||
+        (key == PEEK_OPT_LPM_WINDOW && value >= 0 && value <= (1 << 20))) {
+        peek::lpm_set_option(key, value);
+        return PEEK_OK;
+    }
+    peek::set_error("peek_set_option: unknown key %d or bad value %lld", key, (long long)value);
+    return PEEK_ERR_INVALID_ARG;
 }
 
 extern "C" void peek_profile_enable(int32_t on) { peek::g_prof_on = on != 0; }

@@ -7,19 +7,17 @@
 // Hash mode ("per-request find_longest_cache_hit"): one warp per request, 32
 // consecutive blocks probed per step in the open-addressed table, first miss wins.
 //
-// Co-descent ("one cache walk per pending edge"): with a peek_tree_view the
-// request at sorted position j starts at depth s_j = B*lcp[j] (the prefix it shares with its sorted
-// predecessor) instead of 0: W_j = the walk resumed at s_j (radix mode re-descends to s_j by child
-// lookups only, no token compares).  A per-group pass then resolves
-//   H_j = (H_{j-1} >= s_j) ? W_j : H_{j-1}
-// (if the predecessor's hit ends inside the shared prefix, so does this request's, at the same
-// place; otherwise the shared prefix is fully cached and the resumed walk is exact).
+// Without a peek_tree_view every request walks on its own (k_lpm_radix / k_lpm_hash, one warp per
+// request).  With it the calls co-descend over the sorted order: k_lpm_radix_dual /
+// k_lpm_hash_dual below ("one cache walk per pending edge").
+#include <stdlib.h>
+
 #include "peek_common.cuh"
 
 namespace peek {
 
 static constexpr int LPM_THREADS = 256;
-static constexpr int CMP_UNROLL = 4;
+static constexpr int CMP_UNROLL = 8;
 
 struct RadixDev {
     const i32* c_tokens;
@@ -50,27 +48,38 @@ __device__ __forceinline__ i32 find_child(const i32* __restrict__ e_first_tok, i
     return m ? e0 + (__ffs(m) - 1) : -1;
 }
 
-// number of leading equal tokens of a[0..limit) and b[0..limit), warp-cooperative
-__device__ __forceinline__ i64 match_len(const i32* __restrict__ a, const i32* __restrict__ b, i64 limit,
-                                         int lane) {
-    for (i64 base = 0; base < limit; base += 32 * CMP_UNROLL) {
-        i32 x[CMP_UNROLL], y[CMP_UNROLL];
+// number of leading equal tokens of a[0..limit) and b[0..limit), warp-cooperative.  Most compares
+// end at once (a random token differs) or run the whole edge: the first step looks at 64 tokens,
+// later steps at 32 x CMP_UNROLL tokens per round trip.
+template <int U>
+__device__ __forceinline__ bool match_step(const i32* __restrict__ a, const i32* __restrict__ b, i64 base,
+                                           i64 limit, int lane, i64* m) {
+    i32 x[U], y[U];
 #pragma unroll
-        for (int u = 0; u < CMP_UNROLL; ++u) {
-            i64 i = base + u * 32 + lane;
-            bool in = i < limit;
-            x[u] = in ? __ldg(a + i) : 0;
-            y[u] = in ? __ldg(b + i) : 1;
-        }
+    for (int u = 0; u < U; ++u) {
+        const i64 i = base + u * 32 + lane;
+        const bool in = i < limit;
+        x[u] = in ? __ldg(a + i) : 0;
+        y[u] = in ? __ldg(b + i) : 1;
+    }
 #pragma unroll
-        for (int u = 0; u < CMP_UNROLL; ++u) {
-            unsigned neq = __ballot_sync(0xffffffffu, x[u] != y[u]);
-            if (neq) {
-                i64 m = base + u * 32 + (__ffs(neq) - 1);
-                return m < limit ? m : limit;
-            }
+    for (int u = 0; u < U; ++u) {
+        const unsigned neq = __ballot_sync(0xffffffffu, x[u] != y[u]);
+        if (neq) {
+            const i64 f = base + u * 32 + (__ffs(neq) - 1);
+            *m = f < limit ? f : limit;
+            return true;
         }
     }
+    return false;
+}
+__device__ __forceinline__ i64 match_len(const i32* __restrict__ a, const i32* __restrict__ b, i64 limit,
+                                         int lane) {
+    i64 m = limit;
+    if (limit <= 0) return 0;
+    if (match_step<2>(a, b, 0, limit, lane, &m)) return m;
+    for (i64 base = 64; base < limit; base += 32 * CMP_UNROLL)
+        if (match_step<CMP_UNROLL>(a, b, base, limit, lane, &m)) return m;
     return limit;
 }
 
@@ -105,6 +114,54 @@ __device__ __forceinline__ i32 radix_walk(const RadixDev& R, const i32* __restri
 
 __global__ void __launch_bounds__(LPM_THREADS) k_lpm_radix(const i32* __restrict__ tokens,
                                                           const i64* __restrict__ tok_off, i64 N,
+                                                          RadixDev R, i32* __restrict__ out) {
+    const int lane = threadIdx.x & 31;
+    i64 r = ((i64)blockIdx.x * LPM_THREADS + threadIdx.x) >> 5;
+    if (r >= N) return;
+    i64 o = tok_off[r];
+    i64 len = tok_off[r + 1] - o;
+    i32 h = radix_walk(R, tokens + o, len, 0, lane);
+    if (lane == 0) out[r] = h;
+}
+
+__device__ __forceinline__ bool table_has(const u64* __restrict__ t_keys, u64 mask, u64 key) {
+    u64 p = key & mask;
+    for (;;) {
+        u64 tk = __ldg(t_keys + p);
+        if (tk == key) return true;
+        if (tk == PEEK_EMPTY) return false;
+        p = (p + 1) & mask;
+    }
+}
+
+__global__ void __launch_bounds__(LPM_THREADS) k_lpm_hash(const u64* __restrict__ hashes,
+                                                         const i64* __restrict__ blk_off, i64 N,
+                                                         const u64* __restrict__ t_keys, u64 mask,
+                                                         i32* __restrict__ out) {
+    const int lane = threadIdx.x & 31;
+    i64 r = ((i64)blockIdx.x * LPM_THREADS + threadIdx.x) >> 5;
+    if (r >= N) return;
+    i64 b0 = blk_off[r];
+    i64 nb = blk_off[r + 1] - b0;
+    i64 i0 = 0;
+    i64 hit = nb;
+    for (; i0 < nb; i0 += 32) {
+        i64 i = i0 + lane;
+        bool miss = false;
+        if (i < nb) miss = !table_has(t_keys, mask, hashes[b0 + i]);
+        unsigned m = __ballot_sync(0xffffffffu, miss);
+        if (m) { hit = i0 + (__ffs(m) - 1); break; }
+    }
+    if (lane == 0) out[r] = (i32)(hit * 16);
+}
+
+// ---- speculative co-descent (small N, long requests) -----------------------------------------
+// Every sorted position j walks on its own, in parallel, but starts at depth s_j = B*lcp[j] (radix
+// mode re-descends to s_j by child lookups only): W_j.  W_j is the true hit whenever
+// hit(j-1) >= s_j; otherwise hit(j) = hit(j-1).  The recurrence is resolved by a scan (below).
+// Preferred when there are too few requests for the sequential dual-walk to fill the machine.
+__global__ void __launch_bounds__(LPM_THREADS) k_lpm_radix_spec(const i32* __restrict__ tokens,
+                                                          const i64* __restrict__ tok_off, i64 N,
                                                           RadixDev R, const i32* __restrict__ order,
                                                           const i32* __restrict__ lcp,
                                                           i32* __restrict__ out) {
@@ -119,17 +176,7 @@ __global__ void __launch_bounds__(LPM_THREADS) k_lpm_radix(const i32* __restrict
     if (lane == 0) out[j] = h;  // by sorted position when co-descending, by request otherwise
 }
 
-__device__ __forceinline__ bool table_has(const u64* __restrict__ t_keys, u64 mask, u64 key) {
-    u64 p = key & mask;
-    for (;;) {
-        u64 tk = __ldg(t_keys + p);
-        if (tk == key) return true;
-        if (tk == PEEK_EMPTY) return false;
-        p = (p + 1) & mask;
-    }
-}
-
-__global__ void __launch_bounds__(LPM_THREADS) k_lpm_hash(const u64* __restrict__ hashes,
+__global__ void __launch_bounds__(LPM_THREADS) k_lpm_hash_spec(const u64* __restrict__ hashes,
                                                          const i64* __restrict__ blk_off, i64 N,
                                                          const u64* __restrict__ t_keys, u64 mask,
                                                          const i32* __restrict__ order,
@@ -267,12 +314,209 @@ __global__ void __launch_bounds__(RS_THREADS) k_resolve_apply(const i32* __restr
     }
 }
 
-i64 lpm_ws_bytes(i64 N) {
+// one CTA does the whole scan (small N: one launch instead of three)
+__global__ void __launch_bounds__(1024) k_resolve_single(const i32* __restrict__ order,
+                                                         const i32* __restrict__ lcp,
+                                                         const i32* __restrict__ W, i64 N,
+                                                         i32* __restrict__ hit) {
+    __shared__ Fn sm[34];
+    Fn carry = fn_id();
+    for (i64 base = 0; base < N; base += 1024 * RS_ITEMS) {
+        const i64 j0 = base + (i64)threadIdx.x * RS_ITEMS;
+        Fn f[RS_ITEMS];
+        Fn acc = fn_id();
+#pragma unroll
+        for (int it = 0; it < RS_ITEMS; ++it) {
+            f[it] = fn_load(lcp, W, j0 + it, N);
+            acc = fn_comb(acc, f[it]);
+        }
+        Fn tot;
+        Fn ex = fn_comb(carry, block_exscan_fn(acc, sm, &tot));
+#pragma unroll
+        for (int it = 0; it < RS_ITEMS; ++it) {
+            ex = fn_comb(ex, f[it]);
+            if (j0 + it < N) hit[order[j0 + it]] = ex.c;
+        }
+        carry = fn_comb(carry, tot);
+    }
+}
+
+// ---- dual-walk over the sorted order (PAPER.md:65-90 Alg. 1, :96) ------------------------------
+// A warp owns a RUN of consecutive sorted positions and processes it in order, carrying the
+// predecessor's hit and - in radix mode - the predecessor's path through the cache (the nodes it
+// entered and the depth it entered them at, one entry per lane, in registers).  For position j
+// with s = B*lcp[j] tokens shared with j-1:
+//     hit(j-1) <  s : hit(j) = hit(j-1), nothing is read from the cache
+//     hit(j-1) >= s : pop the path back to depth s and resume the walk inside the node that covers
+//                     s - no re-descent from the root, no compares below s
+// which is the co-descent of the pending trie (order + lcp) against the radix cache: one cache
+// walk per pending edge.  Runs are cut at the position of minimal lcp inside fixed windows of
+// `win` positions (cheap heads: a run head has no predecessor and does a full walk from the root).
+static constexpr int DW_THREADS = 256;
+
+// first position of minimal lcp in [w0, w0 + win) (clipped to N); w0 = 0 gives 0 (lcp[0] = 0)
+__device__ __forceinline__ i64 window_head(const i32* __restrict__ lcp, i64 w0, int win, i64 N, int lane) {
+    if (w0 >= N) return N;
+    i32 best = 0x7fffffff, bidx = 0x7fffffff;
+    for (int t = 0; t < win; t += 32) {
+        i64 j = w0 + t + lane;
+        i32 v = (t + lane < win && j < N) ? __ldg(lcp + j) : 0x7fffffff;
+        i32 m = __reduce_min_sync(0xffffffffu, v);
+        i32 idx = __reduce_min_sync(0xffffffffu, v == m ? t + lane : 0x7fffffff);
+        if (m < best) { best = m; bidx = idx; }
+    }
+    return w0 + bidx;
+}
+
+struct PathEntry { i32 u, ds, L; i64 lab; };  // node entered at token depth ds; label length, offset
+
+__global__ void __launch_bounds__(DW_THREADS) k_lpm_radix_dual(const i32* __restrict__ tokens,
+                                                               const i64* __restrict__ tok_off, i64 N,
+                                                               RadixDev R, const i32* __restrict__ order,
+                                                               const i32* __restrict__ lcp, int win,
+                                                               i32* __restrict__ out) {
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const i64 w = ((i64)blockIdx.x * DW_THREADS + threadIdx.x) >> 5;
+    const i64 w0 = w * win;
+    if (w0 >= N) return;
+    const i64 head = window_head(lcp, w0, win, N, lane);
+    const i64 end = window_head(lcp, w0 + win, win, N, lane);
+    PathEntry pe{0, 0, 0, 0};  // this lane's stack entry (entry index = lane)
+    int top = 0;               // entries in use (<= 32; deeper nodes are not recorded)
+    i32 Hprev = 0;
+    for (i64 jb = head; jb < end; jb += 32) {
+        const i64 jl = jb + lane;
+        const bool valid = jl < end;
+        const i32 r_l = valid ? __ldg(order + jl) : 0;
+        const i32 s_l = valid ? 16 * __ldg(lcp + jl) : 0;
+        const i64 o_l = valid ? __ldg(tok_off + r_l) : 0;
+        const i32 len_l = valid ? (i32)(__ldg(tok_off + r_l + 1) - o_l) : 0;
+        i32 H_l = 0;
+        const int cnt = (int)min((i64)32, end - jb);
+        for (int i = 0; i < cnt; ++i) {
+            i32 s = __shfl_sync(FULL, s_l, i);
+            const bool first = (jb == head && i == 0);
+            if (first) s = 0;
+            i32 H;
+            if (!first && Hprev < s) {
+                H = Hprev;
+            } else {
+                const i64 o = __shfl_sync(FULL, o_l, i);
+                const i32 len = __shfl_sync(FULL, len_l, i);
+                const i32* __restrict__ q = tokens + o;
+                // deepest recorded entry entered strictly above depth s
+                const unsigned mk = __ballot_sync(FULL, lane < top && pe.ds < s);
+                i32 v = 0, d = 0;
+                bool stop = false;
+                if (mk) {
+                    const int k = 31 - __clz(mk);
+                    top = k + 1;
+                    const i32 u = __shfl_sync(FULL, pe.u, k), ds = __shfl_sync(FULL, pe.ds, k),
+                              L = __shfl_sync(FULL, pe.L, k);
+                    const i64 lab = __shfl_sync(FULL, pe.lab, k);
+                    const i32 off = s - ds;
+                    if (off >= L) {  // node fully inside the shared prefix: continue below it
+                        v = u; d = ds + L;
+                    } else {
+                        const i32 limit = min(L, len - ds);
+                        const i32 m = off + (i32)match_len(R.c_tokens + lab + off, q + ds + off, limit - off, lane);
+                        d = ds + m;
+                        if (m < L) stop = true; else v = u;
+                    }
+                } else {
+                    top = 0;
+                }
+                while (!stop && d < len) {
+                    const i32 t = __ldg(q + d);
+                    const i32 e = find_child(R.e_first_tok, __ldg(R.n_child_off + v), __ldg(R.n_child_off + v + 1), t, lane);
+                    if (e < 0) break;
+                    const i32 u = __ldg(R.e_child + e);
+                    const i32 L = __ldg(R.n_tok_len + u);
+                    const i64 lab = __ldg(R.n_tok_off + u);
+                    if (top < 32) {
+                        if (lane == top) { pe.u = u; pe.ds = d; pe.L = L; pe.lab = lab; }
+                        ++top;
+                    }
+                    if (d + L <= s) { d += L; v = u; continue; }  // still inside the shared prefix: no compares
+                    const i32 skip = s > d ? s - d : 0;
+                    const i32 limit = min(L, len - d);
+                    const i32 m = skip + (i32)match_len(R.c_tokens + lab + skip, q + d + skip, limit - skip, lane);
+                    d += m;
+                    if (m < L) break;
+                    v = u;
+                }
+                H = d;
+            }
+            Hprev = H;
+            if (lane == i) H_l = H;
+        }
+        if (valid) out[r_l] = H_l;
+    }
+}
+
+__global__ void __launch_bounds__(DW_THREADS) k_lpm_hash_dual(const u64* __restrict__ hashes,
+                                                              const i64* __restrict__ blk_off, i64 N,
+                                                              const u64* __restrict__ t_keys, u64 mask,
+                                                              const i32* __restrict__ order,
+                                                              const i32* __restrict__ lcp, int win,
+                                                              i32* __restrict__ out) {
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const i64 w = ((i64)blockIdx.x * DW_THREADS + threadIdx.x) >> 5;
+    const i64 w0 = w * win;
+    if (w0 >= N) return;
+    const i64 head = window_head(lcp, w0, win, N, lane);
+    const i64 end = window_head(lcp, w0 + win, win, N, lane);
+    i32 Hprev = 0;  // in blocks
+    for (i64 jb = head; jb < end; jb += 32) {
+        const i64 jl = jb + lane;
+        const bool valid = jl < end;
+        const i32 r_l = valid ? __ldg(order + jl) : 0;
+        const i32 s_l = valid ? __ldg(lcp + jl) : 0;
+        const i64 b_l = valid ? __ldg(blk_off + r_l) : 0;
+        const i32 nb_l = valid ? (i32)(__ldg(blk_off + r_l + 1) - b_l) : 0;
+        i32 H_l = 0;
+        const int cnt = (int)min((i64)32, end - jb);
+        for (int i = 0; i < cnt; ++i) {
+            i32 s = __shfl_sync(FULL, s_l, i);
+            const bool first = (jb == head && i == 0);
+            if (first) s = 0;
+            i32 H;
+            if (!first && Hprev < s) {
+                H = Hprev;
+            } else {
+                const i64 b0 = __shfl_sync(FULL, b_l, i);
+                const i32 nb = __shfl_sync(FULL, nb_l, i);
+                H = nb;
+                for (i32 i0 = s; i0 < nb; i0 += 32) {
+                    const i32 x = i0 + lane;
+                    bool miss = false;
+                    if (x < nb) miss = !table_has(t_keys, mask, __ldg(hashes + b0 + x));
+                    const unsigned m = __ballot_sync(FULL, miss);
+                    if (m) { H = i0 + (__ffs(m) - 1); break; }
+                }
+            }
+            Hprev = H;
+            if (lane == i) H_l = H;
+        }
+        if (valid) out[r_l] = H_l * 16;
+    }
+}
+
+i64 lpm_ws_bytes(i64 N) {  // speculative path: W per mode and the scan partials
     Arena a(nullptr);
     a.take<i32>(N);
     a.take<i32>(N);
     a.take<Fn>((N + RS_CHUNK - 1) / RS_CHUNK + 1);
     return a.used;
+}
+
+static int g_lpm_strategy = 0;  // PEEK_OPT_LPM_STRATEGY
+static int g_lpm_window = 0;    // PEEK_OPT_LPM_WINDOW
+void lpm_set_option(int key, i64 v) {
+    if (key == PEEK_OPT_LPM_STRATEGY) g_lpm_strategy = (int)v;
+    if (key == PEEK_OPT_LPM_WINDOW) g_lpm_window = (int)v;
 }
 
 }  // namespace peek
@@ -313,42 +557,54 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
         return PEEK_ERR_WORKSPACE;
     }
     cudaStream_t st = (cudaStream_t)stream;
+    const i32* order = tree ? tree->order : nullptr;
+    const i32* lcp = tree ? tree->lcp : nullptr;
+    const unsigned warps_grid = (unsigned)((N * 32 + LPM_THREADS - 1) / LPM_THREADS);
+    // co-descent strategy: sequential dual-walk needs many runs to fill the machine
+    const bool dual = tree && (g_lpm_strategy == PEEK_LPM_DUAL_WALK ||
+                               (g_lpm_strategy == PEEK_LPM_AUTO && N >= 32768));
+    const bool spec = tree && !dual;
+    // sorted positions per dual-walk window: enough windows to fill the machine (~8K warps), at
+    // most 32 positions (a run head pays a full walk from the root)
+    int win = 1;
+    while (win < 32 && N / win > 8192) win *= 2;
+    if (g_lpm_window > 0) win = g_lpm_window;
+    const unsigned dual_grid = (unsigned)((((N + win - 1) / win) * 32 + DW_THREADS - 1) / DW_THREADS);
     Arena a(ws);
     i32* Wr = a.take<i32>(N);
     i32* Wh = a.take<i32>(N);
-    const i32* order = tree ? tree->order : nullptr;
-    const i32* lcp = tree ? tree->lcp : nullptr;
-    unsigned warps_grid = (unsigned)((N * 32 + LPM_THREADS - 1) / LPM_THREADS);
-    i64 nchunks = (N + RS_CHUNK - 1) / RS_CHUNK;
+    const i64 nchunks = (N + RS_CHUNK - 1) / RS_CHUNK;
     Fn* partial = a.take<Fn>(nchunks + 1);
+    auto resolve = [&](const i32* W, i32* hit) {
+        if (N <= 65536) {
+            Prof pr(PROF_LPM_RESOLVE, st, 1);
+            k_resolve_single<<<1, 1024, 0, st>>>(order, lcp, W, N, hit);
+        } else {
+            Prof pr(PROF_LPM_RESOLVE, st, 3);
+            k_resolve_partial<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(lcp, W, N, partial);
+            k_resolve_scan<<<1, 1024, 0, st>>>(partial, nchunks);
+            k_resolve_apply<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(order, lcp, W, N, partial, hit);
+        }
+    };
     if (hit_radix) {
         RadixDev R{radix->c_tokens, radix->n_tok_off, radix->n_tok_len,
                    radix->n_child_off, radix->e_first_tok, radix->e_child};
         {
             Prof pr(PROF_LPM_RADIX, st, 1);
-            k_lpm_radix<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, order, lcp,
-                                                           tree ? Wr : hit_radix);
+            if (dual) k_lpm_radix_dual<<<dual_grid, DW_THREADS, 0, st>>>(tokens, tok_off, N, R, order, lcp, win, hit_radix);
+            else if (spec) k_lpm_radix_spec<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, order, lcp, Wr);
+            else k_lpm_radix<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, hit_radix);
         }
-        if (tree) {
-            Prof pr(PROF_LPM_RESOLVE, st, 3);
-            k_resolve_partial<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(lcp, Wr, N, partial);
-            k_resolve_scan<<<1, 1024, 0, st>>>(partial, nchunks);
-            k_resolve_apply<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(order, lcp, Wr, N, partial, hit_radix);
-        }
+        if (spec) resolve(Wr, hit_radix);
     }
     if (hit_hash) {
         {
             Prof pr(PROF_LPM_HASH, st, 1);
-            k_lpm_hash<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys,
-                                                          (u64)(table->S - 1), order, lcp,
-                                                          tree ? Wh : hit_hash);
+            if (dual) k_lpm_hash_dual<<<dual_grid, DW_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), order, lcp, win, hit_hash);
+            else if (spec) k_lpm_hash_spec<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), order, lcp, Wh);
+            else k_lpm_hash<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), hit_hash);
         }
-        if (tree) {
-            Prof pr(PROF_LPM_RESOLVE, st, 3);
-            k_resolve_partial<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(lcp, Wh, N, partial);
-            k_resolve_scan<<<1, 1024, 0, st>>>(partial, nchunks);
-            k_resolve_apply<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(order, lcp, Wh, N, partial, hit_hash);
-        }
+        if (spec) resolve(Wh, hit_hash);
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;

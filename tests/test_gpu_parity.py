@@ -69,13 +69,26 @@ def run_pipeline(toks, off, radix, t_keys, arrival, check_tree_free=True):
     d_radix = _radix_dev(radix) if radix is not None else None
     o_hr = oracle.lpm_radix(toks, off, _orc_radix(radix)) if radix is not None else None
     o_hh = oracle.lpm_hash(o_h, o_bo, t_keys) if t_keys is not None else None
-    # co-descent (tree view) and the naive per-request walk must both equal the oracle
-    for tree in ([gt, None] if check_tree_free else [gt]):
-        g_hr, g_hh = b.peek_lpm(d_tok, d_off, g_h, g_bo, radix=d_radix, t_keys=d_keys, tree=tree)
-        if radix is not None:
-            assert np.array_equal(_np(g_hr), o_hr), "hit_radix tree=%s" % (tree is not None)
-        if t_keys is not None:
-            assert np.array_equal(_np(g_hh), o_hh), "hit_hash tree=%s" % (tree is not None)
+    # every co-descent strategy (dual-walk at several window sizes, speculative + scan) and the
+    # naive per-request walk (no tree view) must all equal the oracle
+    variants = [(gt, b.LPM_DUAL_WALK, 0), (gt, b.LPM_DUAL_WALK, 1), (gt, b.LPM_DUAL_WALK, 5),
+                (gt, b.LPM_DUAL_WALK, 32), (gt, b.LPM_DUAL_WALK, 64), (gt, b.LPM_SPECULATIVE, 0),
+                (gt, b.LPM_AUTO, 0)]
+    if check_tree_free:
+        variants.append((None, b.LPM_AUTO, 0))
+    try:
+        for tree, strategy, window in variants:
+            b.set_option(b.OPT_LPM_STRATEGY, strategy)
+            b.set_option(b.OPT_LPM_WINDOW, window)
+            g_hr, g_hh = b.peek_lpm(d_tok, d_off, g_h, g_bo, radix=d_radix, t_keys=d_keys, tree=tree)
+            what = "tree=%s strategy=%d window=%d" % (tree is not None, strategy, window)
+            if radix is not None:
+                assert np.array_equal(_np(g_hr), o_hr), "hit_radix " + what
+            if t_keys is not None:
+                assert np.array_equal(_np(g_hh), o_hh), "hit_hash " + what
+    finally:
+        b.set_option(b.OPT_LPM_STRATEGY, b.LPM_AUTO)
+        b.set_option(b.OPT_LPM_WINDOW, 0)
 
     hit_np = o_hr if o_hr is not None else o_hh
     d_hit = _dev(hit_np)
