@@ -236,13 +236,19 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(workload: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+def ncu_traffic(workload: str, kernel_slot: str):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel
+    from the committed ncu capture (profiles/ncu_traffic.csv), or None."""
+    import csv
+    names = {"hash.content": "k_block_hash_fused"}
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     try:
-        return json.load(open(p)).get(workload)
+        for row in csv.DictReader(open(p)):
+            if row["workload"] == workload and row["kernel"] == names.get(kernel_slot, kernel_slot):
+                return int(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 # ------------------------------------------------------------------------------------------
@@ -433,7 +439,7 @@ def run_peek(args):
     achieved = balg.get(dom_call, 0) / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
     wname = CONFIG_NAMES[args.config] + (" (small)" if args.small else "")
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic(wname),
+                "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic(wname, dom),
                 "alg_bytes_per_launch": balg.get(dom_call), "ms_per_launch": dom_ms}
     line = {"metric": METRIC, "value": job_throughput(inp.N, world, args.steps, t_ms), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_ms / args.steps,
