@@ -140,3 +140,4 @@ extern "C" peek_status peek_profile_read(int32_t slot, double* total_ms, int64_t
     return PEEK_OK;
 }
 extern "C" int64_t peek_launch_count(void) { return peek::g_launches; }
+

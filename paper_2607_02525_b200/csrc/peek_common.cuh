@@ -100,6 +100,39 @@ __device__ __forceinline__ void grid_barrier(u32* ctr, u32& epoch) {
     __syncthreads();
 }
 
+// Phase timeline of the persistent kernels (development builds only: -DPEEK_TRACE; the product
+// build has none of this): CTA 0 stamps %globaltimer at PEEK_MARK(id); each translation unit keeps
+// its own buffer and exports a reader with PEEK_TRACE_EXPORT(name).
+#ifdef PEEK_TRACE
+static __device__ unsigned long long g_trace[1024];
+static __device__ int g_trace_n;
+#define PEEK_MARK(id)                                                                      \
+    do {                                                                                   \
+        if (blockIdx.x == 0 && threadIdx.x == 0) {                                         \
+            unsigned long long t__;                                                        \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));                        \
+            int n__ = g_trace_n++;                                                         \
+            if (n__ < 1024) g_trace[n__] = (t__ << 10) | (unsigned long long)((id) & 1023); \
+        }                                                                                  \
+    } while (0)
+static inline int32_t trace_read_tu(unsigned long long* out, int32_t cap) {
+    int n = 0;
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(&n, g_trace_n, sizeof(int));
+    if (n > 1024) n = 1024;
+    if (n > cap) n = cap;
+    if (n > 0) cudaMemcpyFromSymbol(out, g_trace, sizeof(unsigned long long) * n);
+    int z = 0;
+    cudaMemcpyToSymbol(g_trace_n, &z, sizeof(int));
+    return n;
+}
+#define PEEK_TRACE_EXPORT(name) \
+    extern "C" int32_t name(unsigned long long* out, int32_t cap) { return peek::trace_read_tu(out, cap); }
+#else
+#define PEEK_MARK(id) do { } while (0)
+#define PEEK_TRACE_EXPORT(name)
+#endif
+
 __device__ __forceinline__ int bits_for(u64 maxval) {  // bits needed to hold 0..maxval
     return maxval == 0 ? 1 : 64 - __clzll((long long)maxval);
 }

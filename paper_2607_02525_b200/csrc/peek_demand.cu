@@ -8,7 +8,7 @@
 //
 // cLPM order (sub-key of Eq. 1): stable LSD radix sort of request indices by
 // (-hit, -cluster_size, arrival), digits gathered from the three arrays; constant digits skipped.
-#include "peek_grid.cuh"
+#include "peek_sort.cuh"
 
 namespace peek {
 
@@ -19,114 +19,224 @@ __global__ void __launch_bounds__(256) k_mintree_level(MinTree mt, int k) {
     mintree_build_level(mt, k, gw, nw, threadIdx.x & 31);
 }
 
-__device__ __forceinline__ i64 table_slot(const u64* __restrict__ t_keys, u64 mask, u64 key) {
-    u64 p = key & mask;
+__device__ __forceinline__ i64 table_slot_from(const u64* __restrict__ t_keys, u64 mask, u64 key, u64 p,
+                                              u64 tk) {  // tk = t_keys[p] already loaded
     for (;;) {
-        u64 tk = __ldg(t_keys + p);
         if (tk == key) return (i64)p;
         if (tk == PEEK_EMPTY) return -1;
         p = (p + 1) & mask;
+        tk = __ldg(t_keys + p);
     }
 }
 
-__device__ __forceinline__ void demand_range(const u64* __restrict__ chain, i64 i_lo, i64 i_hi, i32 count,
-                                             const u64* __restrict__ t_keys, u64 mask, i32* demand,
-                                             int lane) {
-    for (i64 i = i_lo + lane; i <= i_hi; i += 32) {
-        i64 p = table_slot(t_keys, mask, __ldg(chain + i));
-        if (p >= 0) atomicAdd(demand + p, count);
-    }
-}
+// A warp owns 32 consecutive sorted positions.  Lane q describes position j0 + q: its chain, the
+// range [l0, nb) of blocks that first appear there, and the first step of the next-smaller-value
+// walk (blocks [lo1, l1) are shared with positions j+1 .. t1-1, pending_count cnt1 = t1 - j).  The
+// new blocks of the 32 positions are then flattened and handed out 32 x DM_UNROLL at a time, one
+// block per lane: hash load -> table probe -> atomicAdd(pending_count), coalesced along each chain.
+// Blocks below lo1 (tries nested deeper than one level under this position) take a per-lane search.
+static constexpr int DM_THREADS = 256, DM_WARPS = DM_THREADS / 32, DM_UNROLL = 2;
 
-__global__ void __launch_bounds__(256) k_demand(const u64* __restrict__ hashes, const i64* __restrict__ blk_off,
-                                               i64 N, const i32* __restrict__ order,
-                                               const i32* __restrict__ lcp, MinTree mt,
-                                               const u64* __restrict__ t_keys, u64 mask,
-                                               i32* __restrict__ demand) {
-    const int lane = threadIdx.x & 31;
-    i64 j = ((i64)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    if (j >= N) return;
-    i64 r = order[j];
-    i64 b0 = blk_off[r], nb = blk_off[r + 1] - b0;
-    i64 l0 = lcp[j], l1 = j + 1 < N ? lcp[j + 1] : 0;
-    const u64* chain = hashes + b0;
-    // blocks [l0, l1) are shared with later positions: runs of equal pending_count
-    i64 i_hi = l1 - 1, t = j + 1;
-    while (i_hi >= l0) {
-        t = nsv_next_less(mt, t, (i32)(i_hi + 1));  // first later position sharing <= i_hi blocks
-        i64 lt = mt.val(0, t);
-        i64 i_lo = lt > l0 ? lt : l0;
-        demand_range(chain, i_lo, i_hi, (i32)(t - j), t_keys, mask, demand, lane);
-        i_hi = i_lo - 1;
+struct DemandMeta {
+    i64 b0[32];
+    i32 l0[32], l1[32], lo1[32], cnt1[32], t1[32];
+};
+
+__global__ void __launch_bounds__(DM_THREADS) k_demand(const u64* __restrict__ hashes,
+                                                      const i64* __restrict__ blk_off, i64 N,
+                                                      const i32* __restrict__ order,
+                                                      const i32* __restrict__ lcp, MinTree mt,
+                                                      const u64* __restrict__ t_keys, u64 mask,
+                                                      i32* __restrict__ demand) {
+    __shared__ DemandMeta sm[DM_WARPS];
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const i64 j0 = (((i64)blockIdx.x * DM_THREADS + threadIdx.x) >> 5) * 32;
+    if (j0 >= N) return;
+    DemandMeta& M = sm[w];
+    const i64 j = j0 + lane;
+    i32 n_new = 0;
+    {
+        const bool valid = j < N;
+        i64 b0 = 0;
+        i32 nb = 0, l0 = 0, l1 = 0;
+        if (valid) {
+            const i64 r = __ldg(order + j);
+            b0 = __ldg(blk_off + r);
+            nb = (i32)(__ldg(blk_off + r + 1) - b0);
+            l0 = __ldg(lcp + j);
+            l1 = j + 1 < N ? __ldg(lcp + j + 1) : 0;
+            n_new = nb - l0;
+        }
+        i32 lo1 = l1, cnt1 = 1, t1 = (i32)(j + 1);
+        if (valid && l1 > l0) {
+            const i64 t = nsv_next_less(mt, j + 1, l1);  // first later position sharing < l1 blocks
+            const i32 lt = mt.val(0, t);
+            lo1 = lt > l0 ? lt : l0;
+            cnt1 = (i32)(t - j);
+            t1 = (i32)t;
+        }
+        M.b0[lane] = b0; M.l0[lane] = l0; M.l1[lane] = l1; M.lo1[lane] = lo1; M.cnt1[lane] = cnt1; M.t1[lane] = t1;
     }
-    // blocks only this request has
-    demand_range(chain, l0 > l1 ? l0 : l1, nb - 1, 1, t_keys, mask, demand, lane);
+    i32 pre = n_new;  // inclusive prefix of the new-block counts over the warp's positions
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const i32 t = __shfl_up_sync(FULL, pre, o);
+        if (lane >= o) pre += t;
+    }
+    const i32 total = __shfl_sync(FULL, pre, 31);
+    const i32 excl = pre - n_new;
+    __syncwarp();
+    for (i32 base = 0; base < total; base += 32 * DM_UNROLL) {
+        u64 key[DM_UNROLL], slot0[DM_UNROLL], tk[DM_UNROLL];
+        i32 cnt[DM_UNROLL];
+        bool act[DM_UNROLL];
+#pragma unroll
+        for (int u = 0; u < DM_UNROLL; ++u) {
+            const i32 it = base + u * 32 + lane;
+            act[u] = it < total;
+            const i32 itc = act[u] ? it : total - 1;
+            int lo = 0, hi = 31;  // first position q with pre[q] > itc
+#pragma unroll
+            for (int s = 0; s < 5; ++s) {
+                const int mid = (lo + hi) >> 1;
+                const i32 v = __shfl_sync(FULL, pre, mid);
+                if (v > itc) hi = mid; else lo = mid + 1;
+            }
+            const int q = lo;
+            const i32 i = M.l0[q] + (itc - __shfl_sync(FULL, excl, q));
+            key[u] = __ldg(hashes + M.b0[q] + i);
+            i32 c = 1;
+            if (i < M.l1[q]) {
+                if (i >= M.lo1[q]) c = M.cnt1[q];
+                else c = (i32)(nsv_next_less(mt, (i64)M.t1[q], i + 1) - (j0 + q));
+            }
+            cnt[u] = c;
+        }
+#pragma unroll
+        for (int u = 0; u < DM_UNROLL; ++u) {
+            slot0[u] = key[u] & mask;
+            tk[u] = __ldg(t_keys + slot0[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < DM_UNROLL; ++u) {
+            if (act[u]) {
+                const i64 p = table_slot_from(t_keys, mask, key[u], slot0[u], tk[u]);
+                if (p >= 0) atomicAdd(demand + p, cnt[u]);
+            }
+        }
+    }
 }
 
 // ---- cLPM order ---------------------------------------------------------------------------
-struct RankCtl { u32 bar; u32 pad[3]; };
+// Order-preserving u32 images of the three key parts: th, tc descending (signed), ta ascending.
+// One pass finds their ranges; the parts are packed, range-compressed, into one u64 key when they
+// fit (they do for every BASELINE config: e.g. 15 + 5 + 20 bits in config 5) and the pairs
+// (key, request index) go through ONE stable LSD sort whose passes cover only the varying bits.
+// If they do not fit: a first sort by arrival, then a stable sort by (hit, cluster size).
+struct RankCtl {
+    u32 bar;
+    u32 mx[3];  // max of th, tc, ta
+    u32 mn[3];  // max of ~th, ~tc, ~ta  (i.e. ~min)
+    u32 pad;
+    unsigned long long vary[2];
+};
 
 struct RankArgs {
     const i32 *hit, *csize, *arrival;
     i64 N;
     i32* out;
     RankCtl* ctl;
-    u32* ord2;
-    u32* tile_hist;
-    u32* digit_total;
+    GsBufs bufs;
 };
 
-__global__ void __launch_bounds__(PK_THREADS) k_clpm_sort(RankArgs A) {
-    __shared__ SortSmem ssm;
+__device__ __forceinline__ u32 img_desc(i32 v) { return ~((u32)v ^ 0x80000000u); }
+__device__ __forceinline__ u32 img_asc(i32 v) { return (u32)v ^ 0x80000000u; }
+
+__global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
+    __shared__ GsSmem ssm;
     const i64 N = A.N;
-    const i64 gtid = (i64)blockIdx.x * PK_THREADS + threadIdx.x, gsize = (i64)gridDim.x * PK_THREADS;
+    const i64 gtid = (i64)blockIdx.x * GS_THREADS + threadIdx.x, gsize = (i64)gridDim.x * GS_THREADS;
     Grid g{&A.ctl->bar, 0};
-    u32* cur = (u32*)A.out;
-    u32* nxt = A.ord2;
-    for (i64 r = gtid; r < N; r += gsize) cur[r] = (u32)r;
-    g.sync();
-    SortScratch sc{A.tile_hist, A.digit_total};
-    const i32* hit = A.hit;
-    const i32* cs = A.csize;
-    const i32* arr = A.arrival;
-    for (int p = 0; p < 12; ++p) {
-        const int sh = 8 * (p & 3);
-        bool moved;
-        if (p < 4) {  // arrival ascending (signed: flip the sign bit); NULL => the index itself
-            moved = radix_pass(cur, nxt, N, [=](u32 idx) {
-                u32 v = arr ? ((u32)__ldg(arr + idx) ^ 0x80000000u) : idx;
-                return (v >> sh) & 255u;
-            }, sc, ssm, g);
-        } else if (p < 8) {  // cluster size descending
-            moved = radix_pass(cur, nxt, N, [=](u32 idx) {
-                u32 v = ~(u32)__ldg(cs + idx);
-                return (v >> sh) & 255u;
-            }, sc, ssm, g);
-        } else {  // hit descending
-            moved = radix_pass(cur, nxt, N, [=](u32 idx) {
-                u32 v = ~(u32)__ldg(hit + idx);
-                return (v >> sh) & 255u;
-            }, sc, ssm, g);
+    PEEK_MARK(1);
+    const i32* __restrict__ hit = A.hit;
+    const i32* __restrict__ cs = A.csize;
+    const i32* __restrict__ arr = A.arrival;
+    {
+        u32 mx[3] = {0, 0, 0}, mn[3] = {0, 0, 0};
+        for (i64 r = gtid; r < N; r += gsize) {
+            const u32 v[3] = {img_desc(__ldg(hit + r)), img_desc(__ldg(cs + r)),
+                              arr ? img_asc(__ldg(arr + r)) : (u32)r};
+#pragma unroll
+            for (int q = 0; q < 3; ++q) { mx[q] = max(mx[q], v[q]); mn[q] = max(mn[q], ~v[q]); }
         }
-        if (moved) { u32* t = cur; cur = nxt; nxt = t; }
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            const u32 a = __reduce_max_sync(0xffffffffu, mx[q]), b = __reduce_max_sync(0xffffffffu, mn[q]);
+            if ((threadIdx.x & 31) == 0) { atomicMax(&A.ctl->mx[q], a); atomicMax(&A.ctl->mn[q], b); }
+        }
     }
-    if (cur != (u32*)A.out) {
-        for (i64 r = gtid; r < N; r += gsize) A.out[r] = (i32)cur[r];
+    g.sync();
+    PEEK_MARK(2);
+    u32 lo[3];
+    int bits[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        lo[q] = ~__ldcg(&A.ctl->mn[q]);
+        bits[q] = bits_for((u64)(__ldcg(&A.ctl->mx[q]) - lo[q]));
     }
+    const bool one = bits[0] + bits[1] + bits[2] <= 64;
+    const int nphase = one ? 1 : 2;
+    auto make_key = [&](u32 r, int ph) -> u64 {
+        const u64 kh = img_desc(__ldg(hit + r)) - lo[0], kc = img_desc(__ldg(cs + r)) - lo[1];
+        const u64 ka = (arr ? img_asc(__ldg(arr + r)) : r) - lo[2];
+        if (one) return (bits[1] + bits[2] >= 64 ? 0 : kh << (bits[1] + bits[2])) | (kc << bits[2]) | ka;
+        return ph == 0 ? ka : ((kh << bits[1]) | kc);
+    };
+    int src = 0;  // buffer whose val[] holds the current order (after phase 0)
+    for (int ph = 0; ph < nphase; ++ph) {
+        // keys of this phase in the current order (phase 0: the identity) -> buffer 0
+        const u32* vcur = A.bufs.val[src];
+        const u64 kref = make_key(ph == 0 ? 0u : __ldcg(vcur), ph);
+        u64 diff = 0;
+        for (i64 j = gtid; j < N; j += gsize) {
+            const u32 r = ph == 0 ? (u32)j : __ldcg(vcur + j);
+            const u64 key = make_key(r, ph);
+            A.bufs.key[0][j] = key;
+            A.bufs.val[0][j] = r;
+            diff |= key ^ kref;
+        }
+        gs_vary_accumulate(diff, &A.ctl->vary[ph]);
+        g.sync();
+        PEEK_MARK(3);
+        src = grid_sort_pairs(A.bufs, N, __ldcg(&A.ctl->vary[ph]), g, ssm);
+        if (ph + 1 < nphase && src == 0) {  // move the order out of buffer 0 before it is overwritten
+            for (i64 j = gtid; j < N; j += gsize) A.bufs.val[1][j] = __ldcg(&A.bufs.val[0][j]);
+            g.sync();
+            src = 1;
+        }
+    }
+    const u32* res = A.bufs.val[src];
+    for (i64 j = gtid; j < N; j += gsize) A.out[j] = (i32)__ldcg(res + j);
+    PEEK_MARK(4);
 }
 
-static void rank_layout(Arena& a, i64 N, RankArgs& A) {
+static void rank_layout(Arena& a, i64 N, int grid, RankArgs& A) {
     A.ctl = a.take<RankCtl>(1);
-    A.ord2 = a.take<u32>(N);
-    A.tile_hist = a.take<u32>(256 * sort_tiles(N));
-    A.digit_total = a.take<u32>(256);
+    A.bufs.key[0] = a.take<u64>(N);
+    A.bufs.key[1] = a.take<u64>(N);
+    A.bufs.val[0] = a.take<u32>(N);
+    A.bufs.val[1] = a.take<u32>(N);
+    A.bufs.hist = a.take<u32>((i64)grid * 256);
 }
+
+static constexpr int RANK_MAX_GRID = 1024;  // workspace sizing bound on the cooperative grid
 
 i64 demand_rank_ws_bytes(i64 N, i64 S) {
     (void)S;
     Arena a(nullptr);
     RankArgs A;
-    rank_layout(a, N, A);
+    rank_layout(a, N, RANK_MAX_GRID, A);
     a.take<i32>(mintree_words(N));
     return a.used;
 }
@@ -164,7 +274,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
     }
     Arena a(ws);
     RankArgs A;
-    rank_layout(a, N, A);
+    rank_layout(a, N, RANK_MAX_GRID, A);
     i32* mt_buf = a.take<i32>(mintree_words(N));
     if (demand) {
         MinTree mt;
@@ -176,20 +286,23 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
             if (grid > 148u * 8u) grid = 148u * 8u;
             k_mintree_level<<<grid, 256, 0, st>>>(mt, k);
         }
-        unsigned grid = (unsigned)((N * 32 + 255) / 256);
-        k_demand<<<grid, 256, 0, st>>>(hashes, blk_off, N, order, lcp, mt, table->t_keys,
+        unsigned grid = (unsigned)(((N + 31) / 32 * 32 + DM_THREADS - 1) / DM_THREADS);
+        k_demand<<<grid, DM_THREADS, 0, st>>>(hashes, blk_off, N, order, lcp, mt, table->t_keys,
                                       (u64)(table->S - 1), demand);
     }
     if (clpm_order) {
         A.hit = hit; A.csize = cluster_size; A.arrival = arrival; A.N = N; A.out = clpm_order;
-        int grid = persistent_grid((const void*)k_clpm_sort);
-        i64 want = (N + PK_THREADS - 1) / PK_THREADS;
+        int grid = sm_count();  // one CTA of GS_THREADS per SM (co-resident: cooperative launch)
+        if (grid > RANK_MAX_GRID) grid = RANK_MAX_GRID;
+        i64 want = (N + GS_THREADS - 1) / GS_THREADS;
         if (want < grid) grid = (int)(want < 1 ? 1 : want);
         PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, sizeof(RankCtl), st));
         void* params[] = {&A};
         Prof pr(PROF_RANK, st, 1);
-        PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort, dim3(grid), dim3(PK_THREADS), params, 0, st));
+        PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort, dim3(grid), dim3(GS_THREADS), params, 0, st));
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;
 }
+
+PEEK_TRACE_EXPORT(peek_trace_read_rank)

@@ -351,3 +351,5 @@ extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* 
     PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(PK_THREADS), params, 0, st));
     return PEEK_OK;
 }
+
+PEEK_TRACE_EXPORT(peek_trace_read_tree)
