@@ -162,13 +162,26 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
     const i32* __restrict__ hit = A.hit;
     const i32* __restrict__ cs = A.csize;
     const i32* __restrict__ arr = A.arrival;
-    {
+    {   // ranges of the three key images; RK_U x 3 loads in flight per thread
+        constexpr int RK_U = 8;
         u32 mx[3] = {0, 0, 0}, mn[3] = {0, 0, 0};
-        for (i64 r = gtid; r < N; r += gsize) {
-            const u32 v[3] = {img_desc(__ldg(hit + r)), img_desc(__ldg(cs + r)),
-                              arr ? img_asc(__ldg(arr + r)) : (u32)r};
+        for (i64 r0 = gtid; r0 < N; r0 += gsize * RK_U) {
+            u32 v[RK_U][3];
 #pragma unroll
-            for (int q = 0; q < 3; ++q) { mx[q] = max(mx[q], v[q]); mn[q] = max(mn[q], ~v[q]); }
+            for (int u = 0; u < RK_U; ++u) {
+                const i64 r = r0 + u * gsize;
+                const bool in = r < N;
+                v[u][0] = in ? img_desc(__ldg(hit + r)) : 0;
+                v[u][1] = in ? img_desc(__ldg(cs + r)) : 0;
+                v[u][2] = in ? (arr ? img_asc(__ldg(arr + r)) : (u32)r) : 0;
+            }
+#pragma unroll
+            for (int u = 0; u < RK_U; ++u) {
+                if (r0 + u * gsize < N) {
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) { mx[q] = max(mx[q], v[u][q]); mn[q] = max(mn[q], ~v[u][q]); }
+                }
+            }
         }
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
@@ -185,37 +198,29 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
         lo[q] = ~__ldcg(&A.ctl->mn[q]);
         bits[q] = bits_for((u64)(__ldcg(&A.ctl->mx[q]) - lo[q]));
     }
-    const bool one = bits[0] + bits[1] + bits[2] <= 64;
-    const int nphase = one ? 1 : 2;
-    auto make_key = [&](u32 r, int ph) -> u64 {
-        const u64 kh = img_desc(__ldg(hit + r)) - lo[0], kc = img_desc(__ldg(cs + r)) - lo[1];
-        const u64 ka = (arr ? img_asc(__ldg(arr + r)) : r) - lo[2];
-        if (one) return (bits[1] + bits[2] >= 64 ? 0 : kh << (bits[1] + bits[2])) | (kc << bits[2]) | ka;
-        return ph == 0 ? ka : ((kh << bits[1]) | kc);
+    const int bca = bits[1] + bits[2], ball = bits[0] + bca;
+    const bool one = ball <= 64;
+    auto key_a = [&](u32 r) -> u64 { return (u64)((arr ? img_asc(__ldg(arr + r)) : r) - lo[2]); };
+    auto key_hc = [&](u32 r) -> u64 {
+        return ((u64)(img_desc(__ldg(hit + r)) - lo[0]) << bits[1]) | (u64)(img_desc(__ldg(cs + r)) - lo[1]);
     };
-    int src = 0;  // buffer whose val[] holds the current order (after phase 0)
-    for (int ph = 0; ph < nphase; ++ph) {
-        // keys of this phase in the current order (phase 0: the identity) -> buffer 0
-        const u32* vcur = A.bufs.val[src];
-        const u64 kref = make_key(ph == 0 ? 0u : __ldcg(vcur), ph);
-        u64 diff = 0;
-        for (i64 j = gtid; j < N; j += gsize) {
-            const u32 r = ph == 0 ? (u32)j : __ldcg(vcur + j);
-            const u64 key = make_key(r, ph);
-            A.bufs.key[0][j] = key;
-            A.bufs.val[0][j] = r;
-            diff |= key ^ kref;
-        }
-        gs_vary_accumulate(diff, &A.ctl->vary[ph]);
+    auto mask_of = [](int nb) -> u64 { return nb >= 64 ? ~0ull : ((1ull << nb) - 1ull); };
+    int src;
+    if (one) {  // one packed key: [hit | cluster size | arrival], request index breaks ties (stable)
+        src = grid_sort_pairs_gen(A.bufs, N, mask_of(ball), g, ssm, [&](i64 i, u64& k, u32& v) {
+            v = (u32)i;
+            k = (key_hc((u32)i) << bits[2]) | key_a((u32)i);  // bits[2] <= 32 here: no shift overflow
+        });
+    } else {    // arrival first, then a stable sort by (hit, cluster size)
+        src = grid_sort_pairs_gen(A.bufs, N, mask_of(bits[2]), g, ssm, [&](i64 i, u64& k, u32& v) {
+            v = (u32)i;
+            k = key_a((u32)i);
+        });
+        for (i64 j = gtid; j < N; j += gsize) A.bufs.key[src][j] = key_hc(__ldcg(&A.bufs.val[src][j]));
         g.sync();
-        PEEK_MARK(3);
-        src = grid_sort_pairs(A.bufs, N, __ldcg(&A.ctl->vary[ph]), g, ssm);
-        if (ph + 1 < nphase && src == 0) {  // move the order out of buffer 0 before it is overwritten
-            for (i64 j = gtid; j < N; j += gsize) A.bufs.val[1][j] = __ldcg(&A.bufs.val[0][j]);
-            g.sync();
-            src = 1;
-        }
+        src = grid_sort_pairs(A.bufs, N, mask_of(bits[0] + bits[1]), g, ssm, src);
     }
+    PEEK_MARK(3);
     const u32* res = A.bufs.val[src];
     for (i64 j = gtid; j < N; j += gsize) A.out[j] = (i32)__ldcg(res + j);
     PEEK_MARK(4);
@@ -241,7 +246,6 @@ i64 demand_rank_ws_bytes(i64 N, i64 S) {
     return a.used;
 }
 
-int persistent_grid(const void* kernel);
 
 }  // namespace peek
 

@@ -14,13 +14,21 @@
 // taken only where `vary` (the OR of key ^ key' over all pairs, or any superset) has bits set:
 // constant bit ranges cost nothing.
 #pragma once
+#include <type_traits>
+
 #include "peek_grid.cuh"
 
 namespace peek {
 
-static constexpr int GS_THREADS = 1024;
+#ifndef PEEK_GS_THREADS
+#define PEEK_GS_THREADS 1024
+#endif
+#ifndef PEEK_GS_KPT
+#define PEEK_GS_KPT 8
+#endif
+static constexpr int GS_THREADS = PEEK_GS_THREADS;
 static constexpr int GS_WARPS = GS_THREADS / 32;
-static constexpr int GS_KPT = 8;
+static constexpr int GS_KPT = PEEK_GS_KPT;
 static constexpr int GS_TILE = GS_THREADS * GS_KPT;
 
 struct GsSmem {
@@ -36,32 +44,52 @@ struct GsBufs {
     u32* hist;  // 256 * gridDim.x, digit-major
 };
 
-// rank the tile's elements: pre[k] = elements with the same digit earlier in this warp's rows;
-// afterwards sm.wcnt[w][d] = elements with digit d in warps < w, sm.tot[d] = tile count of d
+// lanes of the warp whose 8-bit digit equals this lane's (ballot per bit: cheaper than MATCH.ANY
+// on near-distinct digits); a lane with dg >= 256 (padding) must not take part in any group
+__device__ __forceinline__ unsigned gs_peers(u32 dg) {
+    unsigned m = __ballot_sync(0xffffffffu, dg < 256u);
+#pragma unroll
+    for (int bit = 0; bit < 8; ++bit) {
+        const bool one = (dg >> bit) & 1u;
+        const unsigned bal = __ballot_sync(0xffffffffu, one);
+        m &= one ? bal : ~bal;
+    }
+    return m;
+}
+
+// rank the tile's elements: meta[k] = digit | (elements with the same digit earlier in this warp's
+// rows) << 16; afterwards sm.wcnt[w][d] = elements with digit d in warps < w, sm.tot[d] = tile count
 template <int K>
-__device__ __forceinline__ void gs_rank_tile(const u32 (&dg)[K], u32 (&pre)[K], GsSmem& sm) {
+__device__ __forceinline__ void gs_rank_tile(u32 (&meta)[K], GsSmem& sm) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const unsigned lt = (1u << lane) - 1u;
     for (int d = threadIdx.x; d < GS_WARPS * 256 / 2; d += GS_THREADS) ((u32*)&sm.wcnt[0][0])[d] = 0;
+    unsigned peers[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) peers[k] = gs_peers(meta[k]);
     __syncthreads();
 #pragma unroll
     for (int k = 0; k < K; ++k) {
-        const bool valid = dg[k] < 256u;
-        const unsigned peers = __match_any_sync(0xffffffffu, dg[k]);
-        const u32 old = valid ? sm.wcnt[w][dg[k]] : 0;
-        pre[k] = old + __popc(peers & lt);
+        const u32 dg = meta[k];
+        const bool valid = dg < 256u;
+        const u32 old = valid ? sm.wcnt[w][dg] : 0;
+        meta[k] = dg | ((old + __popc(peers[k] & lt)) << 16);
         __syncwarp();
-        if (valid && (peers & lt) == 0) sm.wcnt[w][dg[k]] = (unsigned short)(old + __popc(peers));
+        if (valid && (peers[k] & lt) == 0) sm.wcnt[w][dg] = (unsigned short)(old + __popc(peers[k]));
         __syncwarp();
     }
     __syncthreads();
     if (threadIdx.x < 256) {
         u32 run = 0;
-#pragma unroll 8
-        for (int ww = 0; ww < GS_WARPS; ++ww) {
-            const u32 c = sm.wcnt[ww][threadIdx.x];
-            sm.wcnt[ww][threadIdx.x] = (unsigned short)run;
-            run += c;
+        for (int w0 = 0; w0 < GS_WARPS; w0 += 8) {
+            u32 c[8];
+#pragma unroll
+            for (int ww = 0; ww < 8; ++ww) c[ww] = sm.wcnt[w0 + ww][threadIdx.x];
+#pragma unroll
+            for (int ww = 0; ww < 8; ++ww) {
+                sm.wcnt[w0 + ww][threadIdx.x] = (unsigned short)run;
+                run += c[ww];
+            }
         }
         sm.tot[threadIdx.x] = run;
     }
@@ -69,23 +97,34 @@ __device__ __forceinline__ void gs_rank_tile(const u32 (&dg)[K], u32 (&pre)[K], 
 }
 
 // sm.base[d] from the published histograms, digit-major hist[d * G + c] (call after the grid
-// barrier): warp w sums digits 8w .. 8w+7 over the G chunks with coalesced loads
+// barrier): warp w sums digits 8w .. 8w+7 over the G chunks; all loads are issued before any use
 __device__ __forceinline__ void gs_bases(const u32* __restrict__ hist, GsSmem& sm) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int G = gridDim.x, me = blockIdx.x;
-    constexpr int DPW = 256 / GS_WARPS;
+    constexpr int DPW = 256 / GS_WARPS, DH = DPW / 2, CPL = 5;  // CPL * 32 = 160 chunks per sweep
     u32 tot[DPW], bel[DPW];
 #pragma unroll
-    for (int q = 0; q < DPW; ++q) {
-        const u32* row = hist + (size_t)(w * DPW + q) * G;
-        u32 t = 0, bl = 0;
-        for (int c = lane; c < G; c += 32) {
-            const u32 v = __ldcg(row + c);
-            t += v;
-            if (c < me) bl += v;
+    for (int q = 0; q < DPW; ++q) tot[q] = bel[q] = 0;
+    for (int cb = 0; cb < G; cb += 32 * CPL) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {  // two batches of DH x CPL loads (register budget)
+            u32 v[DH][CPL];
+#pragma unroll
+            for (int q = 0; q < DH; ++q)
+#pragma unroll
+                for (int x = 0; x < CPL; ++x) {
+                    const int c = cb + x * 32 + lane;
+                    v[q][x] = c < G ? __ldcg(hist + (size_t)(w * DPW + h * DH + q) * G + c) : 0;
+                }
+#pragma unroll
+            for (int q = 0; q < DH; ++q)
+#pragma unroll
+                for (int x = 0; x < CPL; ++x) {
+                    const int c = cb + x * 32 + lane;
+                    tot[h * DH + q] += v[q][x];
+                    if (c < me) bel[h * DH + q] += v[q][x];
+                }
         }
-        tot[q] = t;
-        bel[q] = bl;
     }
 #pragma unroll
     for (int q = 0; q < DPW; ++q) {
@@ -104,36 +143,55 @@ __device__ __forceinline__ void gs_bases(const u32* __restrict__ hist, GsSmem& s
     __syncthreads();
 }
 
-// Sorts n pairs held in buffer 0 of `b`; returns the buffer (0 or 1) that holds the result.
+struct GsNoGen {};  // tag: pass 0 reads buffer 0
+
+// Stable sort of n (key, value) pairs.  With a generator `gen(i, key&, val&)` the pairs of pass 0
+// are produced on the fly (position i of the input order) instead of being read from buffer 0, and
+// pass 0 writes buffer 0; without one the input is buffer 0.  Returns the buffer (0 or 1) that
+// holds the result; with a generator and vary == 0 the pairs are materialised into buffer 0.
 // Must be called by all threads of all CTAs of a cooperative launch with blockDim.x == GS_THREADS.
-__device__ inline int grid_sort_pairs(const GsBufs& b, i64 n, u64 vary, Grid& g, GsSmem& sm) {
+template <typename Gen>
+__device__ __forceinline__ int grid_sort_pairs_gen(const GsBufs& b, i64 n, u64 vary, Grid& g, GsSmem& sm,
+                                                   Gen gen, int start_buf = 0) {
+    constexpr bool HAS_GEN = !std::is_same<Gen, GsNoGen>::value;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const i64 C = (n + gridDim.x - 1) / gridDim.x;
     const i64 c0 = min((i64)blockIdx.x * C, n), c1 = min(c0 + C, n);
     const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
-    int cur = 0;
+    int cur = HAS_GEN ? -1 : start_buf;  // -1: the generator is the source
+    if (HAS_GEN && vary == 0) vary = 1;  // one (trivial) pass materialises the pairs
     while (vary) {
         const int sh = __ffsll((long long)vary) - 1;
         vary &= ~(0xffull << sh);
-        const u64* __restrict__ ks = b.key[cur];
-        const u32* __restrict__ vs = b.val[cur];
-        u64* __restrict__ kd = b.key[cur ^ 1];
-        u32* __restrict__ vd = b.val[cur ^ 1];
+        const int dstb = cur < 0 ? 0 : cur ^ 1;
+        const u64* __restrict__ ks = b.key[cur < 0 ? 0 : cur];
+        const u32* __restrict__ vs = b.val[cur < 0 ? 0 : cur];
+        u64* __restrict__ kd = b.key[dstb];
+        u32* __restrict__ vd = b.val[dstb];
         u64 key[GS_KPT];
-        u32 dg[GS_KPT], pre[GS_KPT];
+        u32 val[GS_KPT], meta[GS_KPT];
         auto load_tile = [&](int t) {
 #pragma unroll
             for (int k = 0; k < GS_KPT; ++k) {
                 const i64 i = c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane;
                 const bool valid = i < c1;
-                key[k] = valid ? __ldcg(ks + i) : 0;
-                dg[k] = valid ? (u32)(key[k] >> sh) & 255u : (0x100u | lane);
+                key[k] = 0;
+                val[k] = 0;
+                if (valid) {
+                    if constexpr (HAS_GEN) {
+                        if (cur < 0) gen(i, key[k], val[k]);
+                        else { key[k] = __ldcg(ks + i); val[k] = __ldcg(vs + i); }
+                    } else {
+                        key[k] = __ldcg(ks + i);
+                        val[k] = __ldcg(vs + i);
+                    }
+                }
+                meta[k] = valid ? (u32)(key[k] >> sh) & 255u : (0x100u | lane);
             }
         };
         if (ntiles == 1) {
             load_tile(0);
-            gs_rank_tile<GS_KPT>(dg, pre, sm);
-            if (threadIdx.x < 256) b.hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = sm.tot[threadIdx.x];
+            gs_rank_tile<GS_KPT>(meta, sm);
         } else {
             if (threadIdx.x < 256) sm.tot[threadIdx.x] = 0;
             __syncthreads();
@@ -141,11 +199,11 @@ __device__ inline int grid_sort_pairs(const GsBufs& b, i64 n, u64 vary, Grid& g,
                 load_tile(t);
 #pragma unroll
                 for (int k = 0; k < GS_KPT; ++k)
-                    if (dg[k] < 256u) atomicAdd(&sm.tot[dg[k]], 1u);
+                    if (meta[k] < 256u) atomicAdd(&sm.tot[meta[k]], 1u);
             }
             __syncthreads();
-            if (threadIdx.x < 256) b.hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = sm.tot[threadIdx.x];
         }
+        if (threadIdx.x < 256) b.hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = sm.tot[threadIdx.x];
         PEEK_MARK(101);
         g.sync();
         PEEK_MARK(102);
@@ -154,16 +212,16 @@ __device__ inline int grid_sort_pairs(const GsBufs& b, i64 n, u64 vary, Grid& g,
         for (int t = 0; t < ntiles; ++t) {
             if (ntiles > 1) {
                 load_tile(t);
-                gs_rank_tile<GS_KPT>(dg, pre, sm);
+                gs_rank_tile<GS_KPT>(meta, sm);
             }
 #pragma unroll
             for (int k = 0; k < GS_KPT; ++k) {
                 const i64 i = c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane;
                 if (i < c1) {
-                    const u32 d = dg[k];
-                    const u32 pos = sm.base[d] + sm.wcnt[w][d] + pre[k];
+                    const u32 d = meta[k] & 0xffffu;
+                    const u32 pos = sm.base[d] + sm.wcnt[w][d] + (meta[k] >> 16);
                     kd[pos] = key[k];
-                    vd[pos] = __ldcg(vs + i);
+                    vd[pos] = val[k];
                 }
             }
             if (ntiles > 1) {
@@ -175,9 +233,15 @@ __device__ inline int grid_sort_pairs(const GsBufs& b, i64 n, u64 vary, Grid& g,
         PEEK_MARK(104);
         g.sync();
         PEEK_MARK(105);
-        cur ^= 1;
+        cur = dstb;
     }
-    return cur;
+    return cur < 0 ? 0 : cur;
+}
+
+// input in buffer `start_buf`
+__device__ __forceinline__ int grid_sort_pairs(const GsBufs& b, i64 n, u64 vary, Grid& g, GsSmem& sm,
+                                               int start_buf = 0) {
+    return grid_sort_pairs_gen(b, n, vary, g, sm, GsNoGen{}, start_buf);
 }
 
 // OR-accumulate (x ^ ref) of a grid-stride loop into a 64-bit device word: call once per thread

@@ -16,7 +16,7 @@
 // the whole root-to-leaf path of h at once, so rounds ~ 3 on the paper's workloads (shared
 // prompt / conversation / turn) instead of one per trie level.  LCPs use the chain property
 // (k_i equal => all earlier words equal, R15) to binary-search the first differing word.
-#include "peek_grid.cuh"
+#include "peek_sort.cuh"
 
 namespace peek {
 
@@ -25,6 +25,7 @@ struct TreeCtl {      // device control block (zeroed by the host before launch)
     u32 unres[3];     // unresolved-position counters, rotating
     u32 maxnb;        // max chain length in blocks
     u32 pad[3];
+    unsigned long long kor[2], kand[2];  // OR / AND of the round's keys (rotating): varying bits
 };
 
 struct TreeArgs {
@@ -36,13 +37,10 @@ struct TreeArgs {
     i32* n_groups;
     // workspace
     TreeCtl* ctl;
-    u32* ord2;        // N   ping-pong partner of `order`
-    u64* key;         // N   sort key by request
+    GsBufs bufs;      // (sort key, request) by position, ping-pong
     u32* seg;         // N   by position: segment start | unresolved << 31
     u64* seghead;     // N   by segment start: (nb << 32) | ~position of the longest chain
     i32* segdepth;    // N   by segment start: blocks all members are known to share
-    u32* tile_hist;   // 256 * tiles
-    u32* digit_total; // 256
     i64* agg;         // gridDim scratch for grid scans
     i32* gsz;         // N   group size by group id
     i32* mt_buf;      // min hierarchy
@@ -95,16 +93,17 @@ __device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb) {
     return kl;
 }
 
-__global__ void __launch_bounds__(PK_THREADS) k_pending_tree(TreeArgs A) {
-    __shared__ SortSmem ssm;
-    __shared__ i64 s64[PK_WARPS + 2];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+__global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
+    __shared__ GsSmem ssm;
+    __shared__ i64 s64[GS_WARPS + 2];
+    const int lane = threadIdx.x & 31;
     const i64 N = A.N;
-    const i64 gtid = (i64)blockIdx.x * PK_THREADS + threadIdx.x, gsize = (i64)gridDim.x * PK_THREADS;
+    const i64 gtid = (i64)blockIdx.x * GS_THREADS + threadIdx.x, gsize = (i64)gridDim.x * GS_THREADS;
     const i64 gwarp = gtid >> 5, nwarps = gsize >> 5;
     Grid g{&A.ctl->bar, 0};
     const u64* __restrict__ H = A.hashes;
     const i64* __restrict__ BO = A.blk_off;
+    PEEK_MARK(1);
 
     // ---- phase 0: max chain length, initial state (one segment, everything "branch at 0") ----
     {
@@ -112,27 +111,32 @@ __global__ void __launch_bounds__(PK_THREADS) k_pending_tree(TreeArgs A) {
         for (i64 r = gtid; r < N; r += gsize) {
             i64 nb = BO[r + 1] - BO[r];
             mx = max(mx, (u32)nb);
-            A.order[r] = (i32)r;
+            A.bufs.val[0][r] = (u32)r;
         }
         mx = __reduce_max_sync(0xffffffffu, mx);
         if (lane == 0 && mx) atomicMax(&A.ctl->maxnb, mx);
+        if (gtid == 0) { A.ctl->kand[0] = ~0ull; A.ctl->kand[1] = ~0ull; }
     }
     g.sync();
     const KeyLayout kl = make_layout(N, __ldcg(&A.ctl->maxnb));
-    for (i64 r = gtid; r < N; r += gsize) A.key[r] = kl.pack(0, kl.f_before(0, false), 0);
-    u32* cur = (u32*)A.order;
-    u32* nxt = A.ord2;
-    SortScratch sc{A.tile_hist, A.digit_total};
-    const int npass = (kl.total + 7) / 8;
+    for (i64 r = gtid; r < N; r += gsize) A.bufs.key[0][r] = kl.pack(0, kl.f_before(0, false), 0);
+    int cb = 0;  // buffer that holds the current (key, request) pairs by position
 
     for (int round = 0;; ++round) {
-        // ---- R4/R1: segment boundaries from equal keys, max-scan of segment starts, heads ----
+        // ---- R1: segment boundaries from equal keys, max-scan of segment starts, heads ----
         g.sync();  // keys / order of the previous phase visible
+        PEEK_MARK(10);
+        const u64* K = A.bufs.key[cb];
+        const u32* cur = A.bufs.val[cb];
         u32* cnt = &A.ctl->unres[round % 3];
-        if (gtid == 0) A.ctl->unres[(round + 1) % 3] = 0;
+        if (gtid == 0) {
+            A.ctl->unres[(round + 1) % 3] = 0;
+            A.ctl->kor[(round + 1) & 1] = 0;
+            A.ctl->kand[(round + 1) & 1] = ~0ull;
+        }
         for (i64 j = gtid; j < N; j += gsize) {
-            u64 kj = __ldcg(A.key + cur[j]);
-            bool start = j == 0 || __ldcg(A.key + cur[j - 1]) != kj;
+            u64 kj = __ldcg(K + j);
+            bool start = j == 0 || __ldcg(K + j - 1) != kj;
             if (start) {
                 A.seghead[j] = 0;
                 u64 F = kl.F_of(kj);
@@ -141,14 +145,13 @@ __global__ void __launch_bounds__(PK_THREADS) k_pending_tree(TreeArgs A) {
         }
         {
             auto load = [&](i64 j) -> i64 {
-                u64 kj = __ldcg(A.key + cur[j]);
-                bool start = j == 0 || __ldcg(A.key + cur[j - 1]) != kj;
+                bool start = j == 0 || __ldcg(K + j - 1) != __ldcg(K + j);
                 return start ? j : 0;
             };
             auto store = [&](i64 j, i64 s) {
-                u64 kj = __ldcg(A.key + cur[j]);
-                bool start = j == 0 || __ldcg(A.key + cur[j - 1]) != kj;
-                bool last = j == N - 1 || __ldcg(A.key + cur[j + 1]) != kj;
+                u64 kj = __ldcg(K + j);
+                bool start = j == 0 || __ldcg(K + j - 1) != kj;
+                bool last = j == N - 1 || __ldcg(K + j + 1) != kj;
                 bool unres = kl.is_branch(kl.F_of(kj)) && !(start && last);
                 A.seg[j] = (u32)s | (unres ? 0x80000000u : 0u);
                 // head = longest chain of the segment (lowest position on ties); one atomic per
@@ -157,7 +160,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pending_tree(TreeArgs A) {
                 unsigned any = __ballot_sync(act, unres);
                 u32 nb = 0;
                 if (unres) {
-                    u32 r = cur[j];
+                    u32 r = __ldcg(cur + j);
                     nb = (u32)(BO[r + 1] - BO[r]);
                 }
                 int same = 0;
@@ -176,51 +179,65 @@ __global__ void __launch_bounds__(PK_THREADS) k_pending_tree(TreeArgs A) {
             };
             grid_inscan<i64>(N, load, store, [](i64 a, i64 b) { return a > b ? a : b; }, (i64)0, A.agg, s64, g);
         }
+        PEEK_MARK(11);
         if (__ldcg(cnt) == 0) break;  // grid-uniform: read after the scan's final barrier
 
-        // ---- R2: classify every unresolved position against its segment head ----
-        for (i64 j = gtid; j < N; j += gsize) {
-            u32 sg = A.seg[j];
-            u32 s = sg & 0x7fffffffu;
-            u32 r = cur[j];
-            if (!(sg >> 31)) { A.key[r] = kl.pack(s, 0, 0); continue; }
-            u64 hv = __ldcg(A.seghead + s);
-            u32 hp = 0xffffffffu - (u32)hv;
-            i64 nbh = (i64)(hv >> 32);
-            u32 h = cur[hp];
-            i64 nbr = BO[r + 1] - BO[r];
-            const u64* cr = H + BO[r];
-            const u64* ch = H + BO[h];
-            i64 l = (r == h) ? nbr : chain_lcp(cr, nbr, ch, nbh, A.segdepth[s]);
-            u64 F, dig = 0;
-            if (l == nbr && l == nbh) F = kl.f_head();
-            else if (l == nbr) F = kl.f_before((u64)kl.D * l, true);
-            else {  // l < nbr <= nbh: the words at l differ
-                u64 a = __ldg(cr + l), b = __ldg(ch + l);
-                int jd = __clzll((long long)(a ^ b)) / kl.w;
-                u64 ld = (u64)kl.D * l + jd;
-                u64 da = (a << (jd * kl.w)) >> (64 - kl.w), db = (b << (jd * kl.w)) >> (64 - kl.w);
-                dig = da;
-                F = da < db ? kl.f_before(ld, false) : kl.f_after(ld);
+        // ---- R2: classify every unresolved position against its segment head (keys in place) ----
+        {
+            u64* Kw = A.bufs.key[cb];
+            u64 orv = 0, andv = ~0ull;
+            for (i64 j = gtid; j < N; j += gsize) {
+                u32 sg = A.seg[j];
+                u32 s = sg & 0x7fffffffu;
+                u64 nk;
+                if (!(sg >> 31)) {
+                    nk = kl.pack(s, 0, 0);
+                } else {
+                    u32 r = __ldcg(cur + j);
+                    u64 hv = __ldcg(A.seghead + s);
+                    u32 hp = 0xffffffffu - (u32)hv;
+                    i64 nbh = (i64)(hv >> 32);
+                    u32 h = __ldcg(cur + hp);
+                    i64 nbr = BO[r + 1] - BO[r];
+                    const u64* cr = H + BO[r];
+                    const u64* ch = H + BO[h];
+                    i64 l = (r == h) ? nbr : chain_lcp(cr, nbr, ch, nbh, A.segdepth[s]);
+                    u64 F, dig = 0;
+                    if (l == nbr && l == nbh) F = kl.f_head();
+                    else if (l == nbr) F = kl.f_before((u64)kl.D * l, true);
+                    else {  // l < nbr <= nbh: the words at l differ
+                        u64 a = __ldg(cr + l), b = __ldg(ch + l);
+                        int jd = __clzll((long long)(a ^ b)) / kl.w;
+                        u64 ld = (u64)kl.D * l + jd;
+                        u64 da = (a << (jd * kl.w)) >> (64 - kl.w), db = (b << (jd * kl.w)) >> (64 - kl.w);
+                        dig = da;
+                        F = da < db ? kl.f_before(ld, false) : kl.f_after(ld);
+                    }
+                    nk = kl.pack(s, F, dig);
+                }
+                Kw[j] = nk;
+                orv |= nk;
+                andv &= nk;
             }
-            A.key[r] = kl.pack(s, F, dig);
+            const u32 olo = __reduce_or_sync(0xffffffffu, (u32)orv), ohi = __reduce_or_sync(0xffffffffu, (u32)(orv >> 32));
+            const u32 alo = __reduce_and_sync(0xffffffffu, (u32)andv), ahi = __reduce_and_sync(0xffffffffu, (u32)(andv >> 32));
+            if (lane == 0) {
+                atomicOr(&A.ctl->kor[round & 1], ((unsigned long long)ohi << 32) | olo);
+                atomicAnd(&A.ctl->kand[round & 1], ((unsigned long long)ahi << 32) | alo);
+            }
         }
         g.sync();
+        PEEK_MARK(12);
 
-        // ---- R3: stable LSD radix sort of positions by key ----
-        for (int p = 0; p < npass; ++p) {
-            const u64* key = A.key;
-            const int sh = 8 * p;
-            bool moved = radix_pass(cur, nxt, N, [=](u32 idx) { return (u32)(__ldcg(key + idx) >> sh) & 255u; },
-                                    sc, ssm, g);
-            if (moved) { u32* t = cur; cur = nxt; nxt = t; }
-        }
+        // ---- R3: stable LSD radix sort of the pairs over the bits that vary ----
+        const u64 vary = __ldcg(&A.ctl->kor[round & 1]) & ~__ldcg(&A.ctl->kand[round & 1]);
+        cb = grid_sort_pairs(A.bufs, N, vary, g, ssm, cb);
+        PEEK_MARK(13);
     }
+    const u32* cur = A.bufs.val[cb];
 
     // ---- F1: final order into `order`, adjacent LCP ----
-    if (cur != (u32*)A.order) {
-        for (i64 j = gtid; j < N; j += gsize) A.order[j] = (i32)cur[j];
-    }
+    for (i64 j = gtid; j < N; j += gsize) A.order[j] = (i32)cur[j];
     for (i64 j = gtid; j < N; j += gsize) {
         i32 l = 0;
         if (j > 0) {
@@ -229,6 +246,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pending_tree(TreeArgs A) {
         }
         A.lcp[j] = l;
     }
+    PEEK_MARK(20);
     const bool want_groups = A.group_id || A.group_size || A.n_groups;
     const bool want_clusters = A.cluster_depth || A.cluster_size || A.cluster_id;
     if (!want_groups && !want_clusters) return;
@@ -260,6 +278,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pending_tree(TreeArgs A) {
             if (A.group_size) A.group_size[r] = __ldcg(A.gsz + gid);
         }
     }
+    PEEK_MARK(21);
     if (!want_clusters) return;
 
     // ---- F4: clusters by nearest-smaller-value searches on the LCP array ----
@@ -285,37 +304,32 @@ __global__ void __launch_bounds__(PK_THREADS) k_pending_tree(TreeArgs A) {
         if (A.cluster_size) A.cluster_size[r] = cs;
         if (A.cluster_id) A.cluster_id[r] = cid;
     }
+    PEEK_MARK(22);
 }
+
 
 static void tree_layout(Arena& a, i64 N, int grid, TreeArgs& A) {
     A.ctl = a.take<TreeCtl>(1);
-    A.ord2 = a.take<u32>(N);
-    A.key = a.take<u64>(N);
+    A.bufs.key[0] = a.take<u64>(N);
+    A.bufs.key[1] = a.take<u64>(N);
+    A.bufs.val[0] = a.take<u32>(N);
+    A.bufs.val[1] = a.take<u32>(N);
+    A.bufs.hist = a.take<u32>(256 * (i64)grid);
     A.seg = a.take<u32>(N);
     A.seghead = a.take<u64>(N);
     A.segdepth = a.take<i32>(N);
-    A.tile_hist = a.take<u32>(256 * sort_tiles(N));
-    A.digit_total = a.take<u32>(256);
     A.agg = a.take<i64>(grid);
     A.gsz = a.take<i32>(N);
     A.mt_buf = a.take<i32>(mintree_words(N));
 }
 
-static constexpr int MAX_GRID = 148 * 4 * 4;  // upper bound used for workspace sizing
+static constexpr int MAX_GRID = 1024;  // upper bound on the cooperative grid (workspace sizing)
 
 i64 pending_tree_ws_bytes(i64 N) {
     Arena a(nullptr);
     TreeArgs A;
     tree_layout(a, N, MAX_GRID, A);
     return a.used;
-}
-
-int persistent_grid(const void* kernel) {
-    int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, PK_THREADS, 0) != cudaSuccess || occ < 1) occ = 1;
-    if (occ > 4) occ = 4;
-    int g = sm_count() * occ;
-    return g > MAX_GRID ? MAX_GRID : g;
 }
 
 }  // namespace peek
@@ -335,8 +349,9 @@ extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* 
         return PEEK_ERR_WORKSPACE;
     }
     cudaStream_t st = (cudaStream_t)stream;
-    int grid = persistent_grid((const void*)k_pending_tree);
-    i64 want = (N + PK_THREADS - 1) / PK_THREADS;  // no point in more CTAs than work
+    int grid = sm_count();  // one CTA of GS_THREADS per SM, all co-resident (cooperative launch)
+    if (grid > MAX_GRID) grid = MAX_GRID;
+    i64 want = (N + GS_THREADS - 1) / GS_THREADS;  // no point in more CTAs than work
     if (want < grid) grid = (int)(want < 1 ? 1 : want);
     Arena a(ws);
     TreeArgs A;
@@ -348,7 +363,7 @@ extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* 
     PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, sizeof(TreeCtl), st));
     void* params[] = {&A};
     Prof pr(PROF_TREE, st, 1);
-    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(PK_THREADS), params, 0, st));
+    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(GS_THREADS), params, 0, st));
     return PEEK_OK;
 }
 
