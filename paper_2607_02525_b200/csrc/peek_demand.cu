@@ -154,7 +154,9 @@ __device__ __forceinline__ u32 img_desc(i32 v) { return ~((u32)v ^ 0x80000000u);
 __device__ __forceinline__ u32 img_asc(i32 v) { return (u32)v ^ 0x80000000u; }
 
 __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
     __shared__ GsSmem ssm;
+    const GsStage stg = gs_stage(dyn_smem);
     const i64 N = A.N;
     const i64 gtid = (i64)blockIdx.x * GS_THREADS + threadIdx.x, gsize = (i64)gridDim.x * GS_THREADS;
     Grid g{&A.ctl->bar, 0};
@@ -183,11 +185,18 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
                 }
             }
         }
+        // CTA-level max through shared memory, then six atomics per CTA
+        __shared__ u32 s_mm[6];
+        if (threadIdx.x < 6) s_mm[threadIdx.x] = 0;
+        __syncthreads();
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
             const u32 a = __reduce_max_sync(0xffffffffu, mx[q]), b = __reduce_max_sync(0xffffffffu, mn[q]);
-            if ((threadIdx.x & 31) == 0) { atomicMax(&A.ctl->mx[q], a); atomicMax(&A.ctl->mn[q], b); }
+            if ((threadIdx.x & 31) == 0) { atomicMax(&s_mm[q], a); atomicMax(&s_mm[3 + q], b); }
         }
+        __syncthreads();
+        if (threadIdx.x < 3) atomicMax(&A.ctl->mx[threadIdx.x], s_mm[threadIdx.x]);
+        else if (threadIdx.x < 6) atomicMax(&A.ctl->mn[threadIdx.x - 3], s_mm[threadIdx.x]);
     }
     g.sync();
     PEEK_MARK(2);
@@ -207,18 +216,18 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
     auto mask_of = [](int nb) -> u64 { return nb >= 64 ? ~0ull : ((1ull << nb) - 1ull); };
     int src;
     if (one) {  // one packed key: [hit | cluster size | arrival], request index breaks ties (stable)
-        src = grid_sort_pairs_gen(A.bufs, N, mask_of(ball), g, ssm, [&](i64 i, u64& k, u32& v) {
+        src = grid_sort_pairs_gen(A.bufs, N, mask_of(ball), g, ssm, stg, [&](i64 i, u64& k, u32& v) {
             v = (u32)i;
             k = (key_hc((u32)i) << bits[2]) | key_a((u32)i);  // bits[2] <= 32 here: no shift overflow
         });
     } else {    // arrival first, then a stable sort by (hit, cluster size)
-        src = grid_sort_pairs_gen(A.bufs, N, mask_of(bits[2]), g, ssm, [&](i64 i, u64& k, u32& v) {
+        src = grid_sort_pairs_gen(A.bufs, N, mask_of(bits[2]), g, ssm, stg, [&](i64 i, u64& k, u32& v) {
             v = (u32)i;
             k = key_a((u32)i);
         });
         for (i64 j = gtid; j < N; j += gsize) A.bufs.key[src][j] = key_hc(__ldcg(&A.bufs.val[src][j]));
         g.sync();
-        src = grid_sort_pairs(A.bufs, N, mask_of(bits[0] + bits[1]), g, ssm, src);
+        src = grid_sort_pairs(A.bufs, N, mask_of(bits[0] + bits[1]), g, ssm, stg, src);
     }
     PEEK_MARK(3);
     const u32* res = A.bufs.val[src];
@@ -228,11 +237,11 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
 
 static void rank_layout(Arena& a, i64 N, int grid, RankArgs& A) {
     A.ctl = a.take<RankCtl>(1);
+    A.bufs.hist = a.take<u32>(gs_hist_words(grid));  // directly after ctl: one memset clears both
     A.bufs.key[0] = a.take<u64>(N);
     A.bufs.key[1] = a.take<u64>(N);
     A.bufs.val[0] = a.take<u32>(N);
     A.bufs.val[1] = a.take<u32>(N);
-    A.bufs.hist = a.take<u32>((i64)grid * 256);
 }
 
 static constexpr int RANK_MAX_GRID = 1024;  // workspace sizing bound on the cooperative grid
@@ -300,10 +309,16 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
         if (grid > RANK_MAX_GRID) grid = RANK_MAX_GRID;
         i64 want = (N + GS_THREADS - 1) / GS_THREADS;
         if (want < grid) grid = (int)(want < 1 ? 1 : want);
-        PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, sizeof(RankCtl), st));
+        PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(RANK_MAX_GRID)) - (char*)A.ctl), st));
         void* params[] = {&A};
         Prof pr(PROF_RANK, st, 1);
-        PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort, dim3(grid), dim3(GS_THREADS), params, 0, st));
+        static bool attr_set = false;
+        if (!attr_set) {
+            PEEK_CUDA(cudaFuncSetAttribute(k_clpm_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
+            attr_set = true;
+        }
+        PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort, dim3(grid), dim3(GS_THREADS), params,
+                                              GS_STAGE_BYTES, st));
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;

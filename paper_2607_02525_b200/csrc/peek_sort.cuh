@@ -35,13 +35,25 @@ struct GsSmem {
     unsigned short wcnt[GS_WARPS][256];  // per-warp digit counts, then exclusive prefix over warps
     u32 base[256];                       // where this CTA's next element with digit d goes
     u32 tot[256];                        // digit counts of the tile / chunk
+    u32 dstart[256];                     // exclusive prefix of the tile's digit counts
     u32 scan[GS_WARPS + 2];
 };
+
+// dynamic shared memory of a kernel that sorts: one tile of pairs, staged in digit order so that
+// the scatter writes runs of consecutive addresses (full sectors instead of one sector per pair)
+static constexpr int GS_STAGE_BYTES = GS_TILE * (int)(sizeof(u64) + sizeof(u32));
+struct GsStage {
+    u64* key;
+    u32* val;
+};
+__device__ __forceinline__ GsStage gs_stage(void* dyn_smem) {
+    return GsStage{(u64*)dyn_smem, (u32*)((char*)dyn_smem + (size_t)GS_TILE * sizeof(u64))};
+}
 
 struct GsBufs {
     u64* key[2];
     u32* val[2];
-    u32* hist;  // 256 * gridDim.x, digit-major
+    u32* hist;  // gs_hist_words(gridDim.x) words; the accumulator part must be zero on entry
 };
 
 // lanes of the warp whose 8-bit digit equals this lane's (ballot per bit: cheaper than MATCH.ANY
@@ -68,6 +80,7 @@ __device__ __forceinline__ void gs_rank_tile(u32 (&meta)[K], GsSmem& sm) {
 #pragma unroll
     for (int k = 0; k < K; ++k) peers[k] = gs_peers(meta[k]);
     __syncthreads();
+    PEEK_MARK(110);
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const u32 dg = meta[k];
@@ -79,6 +92,7 @@ __device__ __forceinline__ void gs_rank_tile(u32 (&meta)[K], GsSmem& sm) {
         __syncwarp();
     }
     __syncthreads();
+    PEEK_MARK(111);
     if (threadIdx.x < 256) {
         u32 run = 0;
         for (int w0 = 0; w0 < GS_WARPS; w0 += 8) {
@@ -94,52 +108,89 @@ __device__ __forceinline__ void gs_rank_tile(u32 (&meta)[K], GsSmem& sm) {
         sm.tot[threadIdx.x] = run;
     }
     __syncthreads();
+    PEEK_MARK(112);
+    {
+        const u32 t = threadIdx.x < 256 ? sm.tot[threadIdx.x] : 0;
+        u32 all;
+        const u32 inc = block_inscan(t, [](u32 a, u32 b) { return a + b; }, 0u, sm.scan, &all);
+        if (threadIdx.x < 256) sm.dstart[threadIdx.x] = inc - t;
+        __syncthreads();
+    }
 }
 
-// sm.base[d] from the published histograms, digit-major hist[d * G + c] (call after the grid
-// barrier): warp w sums digits 8w .. 8w+7 over the G chunks; all loads are issued before any use
-__device__ __forceinline__ void gs_bases(const u32* __restrict__ hist, GsSmem& sm) {
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int G = gridDim.x, me = blockIdx.x;
-    constexpr int DPW = 256 / GS_WARPS, DH = DPW / 2, CPL = 5;  // CPL * 32 = 160 chunks per sweep
-    u32 tot[DPW], bel[DPW];
-#pragma unroll
-    for (int q = 0; q < DPW; ++q) tot[q] = bel[q] = 0;
-    for (int cb = 0; cb < G; cb += 32 * CPL) {
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {  // two batches of DH x CPL loads (register budget)
-            u32 v[DH][CPL];
-#pragma unroll
-            for (int q = 0; q < DH; ++q)
-#pragma unroll
-                for (int x = 0; x < CPL; ++x) {
-                    const int c = cb + x * 32 + lane;
-                    v[q][x] = c < G ? __ldcg(hist + (size_t)(w * DPW + h * DH + q) * G + c) : 0;
-                }
-#pragma unroll
-            for (int q = 0; q < DH; ++q)
-#pragma unroll
-                for (int x = 0; x < CPL; ++x) {
-                    const int c = cb + x * 32 + lane;
-                    tot[h * DH + q] += v[q][x];
-                    if (c < me) bel[h * DH + q] += v[q][x];
-                }
+// ---- digit bases without an all-to-all read ------------------------------------------------------
+// Every CTA needs, per digit, the elements with a smaller digit anywhere plus those with the same
+// digit in earlier chunks.  Reading all G histograms in all G CTAs is G*G KB of L2 traffic on the
+// same lines (measured 8 us per pass at G = 148).  Instead a CTA publishes its histogram row AND adds
+// it (fire-and-forget reductions) to the digit totals and to the row of its group of GS_GROUP
+// chunks; after the barrier it reads the totals, the rows of the groups before its own and the rows
+// of the chunks before it inside its group: <= 1 + G/GS_GROUP + GS_GROUP rows instead of G.
+// The accumulators come in two sets (passes alternate); the set a pass does not use is zeroed
+// during that pass, and both must be zero when a sort starts (host memset, and restored on exit).
+static constexpr int GS_GROUP = 16;
+__host__ __device__ inline i64 gs_hist_words(int grid) {
+    return 256 * ((i64)grid + 2 * ((grid + GS_GROUP - 1) / GS_GROUP + 1));
+}
+struct GsHist {
+    u32* rows;    // [G][256] per-chunk histograms
+    u32* acc[2];  // [1 + NG][256]: row 0 digit totals, row 1 + g the sum over group g
+    int ng;
+};
+__device__ __forceinline__ GsHist gs_hist(u32* hist) {
+    const int G = gridDim.x, ng = (G + GS_GROUP - 1) / GS_GROUP;
+    GsHist h;
+    h.rows = hist;
+    h.acc[0] = hist + (size_t)256 * G;
+    h.acc[1] = h.acc[0] + (size_t)256 * (ng + 1);
+    h.ng = ng;
+    return h;
+}
+
+// before the barrier: publish sm.tot (this chunk's digit counts); `set` = pass parity
+__device__ __forceinline__ void gs_publish(const GsHist& h, int set, const GsSmem& sm) {
+    if (threadIdx.x < 256) {
+        const u32 v = sm.tot[threadIdx.x];
+        h.rows[(size_t)blockIdx.x * 256 + threadIdx.x] = v;
+        if (v) {
+            atomicAdd(h.acc[set] + threadIdx.x, v);
+            atomicAdd(h.acc[set] + (size_t)256 * (1 + blockIdx.x / GS_GROUP) + threadIdx.x, v);
         }
     }
+}
+
+// after the barrier: sm.base[d]; also zeroes the other accumulator set for the next pass
+__device__ __forceinline__ void gs_bases(const GsHist& h, int set, GsSmem& sm) {
+    const int me = blockIdx.x, grp = me / GS_GROUP, d = threadIdx.x & 255, part = threadIdx.x >> 8;
+    constexpr int PARTS = GS_THREADS / 256;  // thread groups that split the rows between them
+    // rows to add up for "same digit, earlier chunks": groups < grp, then chunks grp*GS_GROUP .. me-1
+    const int nrows = grp + (me - grp * GS_GROUP);
+    u32 below = 0;
+    for (int r0 = part; r0 < nrows; r0 += PARTS * 8) {
+        u32 v[8];
 #pragma unroll
-    for (int q = 0; q < DPW; ++q) {
-        tot[q] = __reduce_add_sync(0xffffffffu, tot[q]);
-        bel[q] = __reduce_add_sync(0xffffffffu, bel[q]);
-    }
-    if (lane == 0) {
+        for (int x = 0; x < 8; ++x) {
+            const int r = r0 + x * PARTS;
+            const u32* row = r < grp ? h.acc[set] + (size_t)256 * (1 + r)
+                                     : h.rows + (size_t)256 * (grp * GS_GROUP + (r - grp));
+            v[x] = r < nrows ? __ldcg(row + d) : 0u;
+        }
 #pragma unroll
-        for (int q = 0; q < DPW; ++q) { sm.tot[w * DPW + q] = tot[q]; sm.base[w * DPW + q] = bel[q]; }
+        for (int x = 0; x < 8; ++x) below += v[x];
     }
-    __syncthreads();
-    const u32 total = threadIdx.x < 256 ? sm.tot[threadIdx.x] : 0;
+    const u32 total = part == 0 ? __ldcg(h.acc[set] + d) : 0u;
+    if (PARTS > 1) {
+        if (part == 0) sm.base[d] = 0;
+        __syncthreads();
+        if (below) atomicAdd(&sm.base[d], below);
+        __syncthreads();
+        below = part == 0 ? sm.base[d] : 0u;
+    }
     u32 all;
     const u32 inc = block_inscan(total, [](u32 a, u32 b) { return a + b; }, 0u, sm.scan, &all);
-    if (threadIdx.x < 256) sm.base[threadIdx.x] += inc - total;
+    if (part == 0) sm.base[d] = below + inc - total;
+    // the other set was last read before the previous pass's closing barrier
+    const int words = 256 * (h.ng + 1);
+    for (int i = blockIdx.x * GS_THREADS + threadIdx.x; i < words; i += gridDim.x * GS_THREADS) h.acc[set ^ 1][i] = 0;
     __syncthreads();
 }
 
@@ -152,13 +203,15 @@ struct GsNoGen {};  // tag: pass 0 reads buffer 0
 // Must be called by all threads of all CTAs of a cooperative launch with blockDim.x == GS_THREADS.
 template <typename Gen>
 __device__ __forceinline__ int grid_sort_pairs_gen(const GsBufs& b, i64 n, u64 vary, Grid& g, GsSmem& sm,
-                                                   Gen gen, int start_buf = 0) {
+                                                   GsStage stg, Gen gen, int start_buf = 0) {
     constexpr bool HAS_GEN = !std::is_same<Gen, GsNoGen>::value;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const i64 C = (n + gridDim.x - 1) / gridDim.x;
     const i64 c0 = min((i64)blockIdx.x * C, n), c1 = min(c0 + C, n);
     const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
     int cur = HAS_GEN ? -1 : start_buf;  // -1: the generator is the source
+    const GsHist gh = gs_hist(b.hist);
+    int pass = 0;
     if (HAS_GEN && vary == 0) vary = 1;  // one (trivial) pass materialises the pairs
     while (vary) {
         const int sh = __ffsll((long long)vary) - 1;
@@ -191,6 +244,7 @@ __device__ __forceinline__ int grid_sort_pairs_gen(const GsBufs& b, i64 n, u64 v
         };
         if (ntiles == 1) {
             load_tile(0);
+            PEEK_MARK(100);
             gs_rank_tile<GS_KPT>(meta, sm);
         } else {
             if (threadIdx.x < 256) sm.tot[threadIdx.x] = 0;
@@ -203,11 +257,11 @@ __device__ __forceinline__ int grid_sort_pairs_gen(const GsBufs& b, i64 n, u64 v
             }
             __syncthreads();
         }
-        if (threadIdx.x < 256) b.hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = sm.tot[threadIdx.x];
+        gs_publish(gh, pass & 1, sm);
         PEEK_MARK(101);
         g.sync();
         PEEK_MARK(102);
-        gs_bases(b.hist, sm);
+        gs_bases(gh, pass & 1, sm);
         PEEK_MARK(103);
         for (int t = 0; t < ntiles; ++t) {
             if (ntiles > 1) {
@@ -215,17 +269,33 @@ __device__ __forceinline__ int grid_sort_pairs_gen(const GsBufs& b, i64 n, u64 v
                 gs_rank_tile<GS_KPT>(meta, sm);
             }
 #pragma unroll
-            for (int k = 0; k < GS_KPT; ++k) {
+            for (int k = 0; k < GS_KPT; ++k) {  // stage the tile in digit order
                 const i64 i = c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane;
                 if (i < c1) {
                     const u32 d = meta[k] & 0xffffu;
-                    const u32 pos = sm.base[d] + sm.wcnt[w][d] + (meta[k] >> 16);
-                    kd[pos] = key[k];
-                    vd[pos] = val[k];
+                    const u32 lp = sm.dstart[d] + sm.wcnt[w][d] + (meta[k] >> 16);
+                    stg.key[lp] = key[k];
+                    stg.val[lp] = val[k];
                 }
             }
+            __syncthreads();
+            {
+                const i64 tbase = c0 + (i64)t * GS_TILE;
+                const int tcount = (int)min((i64)GS_TILE, c1 - tbase);
+#pragma unroll
+                for (int k = 0; k < GS_KPT; ++k) {  // runs of equal digits go to consecutive addresses
+                    const int q = k * GS_THREADS + threadIdx.x;
+                    if (q < tcount) {
+                        const u64 kk = stg.key[q];
+                        const u32 d = (u32)(kk >> sh) & 255u;
+                        const u32 pos = sm.base[d] + ((u32)q - sm.dstart[d]);
+                        kd[pos] = kk;
+                        vd[pos] = stg.val[q];
+                    }
+                }
+            }
+            __syncthreads();  // the stage is reused by the next tile / pass
             if (ntiles > 1) {
-                __syncthreads();
                 if (threadIdx.x < 256) sm.base[threadIdx.x] += sm.tot[threadIdx.x];
                 __syncthreads();
             }
@@ -234,14 +304,21 @@ __device__ __forceinline__ int grid_sort_pairs_gen(const GsBufs& b, i64 n, u64 v
         g.sync();
         PEEK_MARK(105);
         cur = dstb;
+        ++pass;
+    }
+    // leave both accumulator sets zero: the last pass's set is dirty, nobody reads it any more
+    if (pass > 0) {
+        const int words = 256 * (gh.ng + 1);
+        for (int i = blockIdx.x * GS_THREADS + threadIdx.x; i < words; i += gridDim.x * GS_THREADS)
+            gh.acc[(pass - 1) & 1][i] = 0;
     }
     return cur < 0 ? 0 : cur;
 }
 
 // input in buffer `start_buf`
 __device__ __forceinline__ int grid_sort_pairs(const GsBufs& b, i64 n, u64 vary, Grid& g, GsSmem& sm,
-                                               int start_buf = 0) {
-    return grid_sort_pairs_gen(b, n, vary, g, sm, GsNoGen{}, start_buf);
+                                               GsStage stg, int start_buf = 0) {
+    return grid_sort_pairs_gen(b, n, vary, g, sm, stg, GsNoGen{}, start_buf);
 }
 
 // OR-accumulate (x ^ ref) of a grid-stride loop into a 64-bit device word: call once per thread

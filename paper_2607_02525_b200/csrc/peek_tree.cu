@@ -39,6 +39,7 @@ struct TreeArgs {
     TreeCtl* ctl;
     GsBufs bufs;      // (sort key, request) by position, ping-pong
     u32* seg;         // N   by position: segment start | unresolved << 31
+    u32* srank;       // N   by position: dense rank of the segment (the sort key's leading field)
     u64* seghead;     // N   by segment start: (nb << 32) | ~position of the longest chain
     i32* segdepth;    // N   by segment start: blocks all members are known to share
     i64* agg;         // gridDim scratch for grid scans
@@ -77,6 +78,11 @@ struct KeyLayout {
         return (seg << (lbits + w)) | (F << w) | dig;
     }
     __device__ __forceinline__ u64 F_of(u64 key) const { return (key >> w) & ((1ull << lbits) - 1); }
+    __device__ __forceinline__ u64 seg_of(u64 key) const { return key >> (lbits + w); }
+    // digits a member of class F shares with its segment head (the head itself: everything)
+    __device__ __forceinline__ u64 ldv(u64 F) const {
+        return (F <= 2 * LDmax + 1) ? (F >> 1) : (F == 2 * LDmax + 2 ? 2 * LDmax : LDmax - (F - (2 * LDmax + 3)));
+    }
 };
 
 __device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb) {
@@ -93,37 +99,178 @@ __device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb) {
     return kl;
 }
 
-__global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
-    __shared__ GsSmem ssm;
-    __shared__ i64 s64[GS_WARPS + 2];
+// ---- staged tile processing ---------------------------------------------------------------------
+// Every phase walks the CTA's chunk of positions (the sort engine's ownership: CTA c owns
+// [c0, c1), element (t, k) of thread (w, lane) is c0 + t*GS_TILE + w*32*GS_KPT + k*32 + lane) with
+// GS_KPT elements per thread held in registers, and is written stage by stage: all loads of a
+// stage are issued for the GS_KPT elements before any is used, so a phase costs (dependent stages)
+// x (one memory round trip) instead of (elements per thread) x (stages) round trips.
+#define ELEMS(k) _Pragma("unroll") for (int k = 0; k < GS_KPT; ++k)
+// the register-hungry phases (lock-step searches) take the tile in sub-batches of SB elements
+#ifndef PEEK_SB
+#define PEEK_SB 1
+#endif
+static constexpr int SB = PEEK_SB;
+#define SUBS(k) _Pragma("unroll") for (int k = 0; k < SB; ++k)
+
+struct TreeSmem {
+    i32 wv[GS_WARPS + 1];   // per-warp values of the carry chains
+    i64 wv64[GS_WARPS + 1];
+    i64 carry64;
+    i32 carry;
+    i32 lvl_hi[2048 + 64 + 8];  // per-CTA copy of the min-hierarchy levels >= 3
+};
+
+// LCP of K pairs of chains in lock step: chains H[ao..ao+na), H[bo..bo+nb), first lo words known
+// equal (chain property R15: equal at a depth => equal above it, so the first difference is found
+// by bisection).  act[k] selects the pairs to do; others keep res[k].
+// Probes are random 32-byte sectors of a multi-GB array (the phase is bound by HBM transactions,
+// not latency), so the search is organised to need few of them: (1) the last common word (one chain
+// prefixes the other: done); (2) per warp row, ONE lane bisects and its answer g is the guess of
+// the others (neighbours in sorted order mostly branch off their head at the same depth), who
+// probe words g-1 and g - usually one sector - and (3) bisect on only if that did not settle it.
+// HINT = false skips (2).  Must be called by full warps (uses warp collectives).
+template <int K, bool HINT>
+__device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i64 (&ao)[K], const i32 (&na)[K],
+                                             const i64 (&bo)[K], const i32 (&nb)[K], const i32 (&lo)[K],
+                                             const bool (&act)[K], i32 (&res)[K], bool probe_lo) {
+    const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
+    i32 L[K], R[K];  // while go: equal below/at L (L = lo - 1: nothing known), differ at R
+    bool go[K];
+    u64 x[K], y[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const i32 m = na[k] < nb[k] ? na[k] : nb[k];
+        go[k] = act[k] && m > lo[k];
+        if (act[k] && !go[k]) res[k] = m;
+        L[k] = lo[k] - 1;
+        R[k] = m - 1;
+    }
+    {   // first round trip: the last common word and - if the caller expects branches right at
+        // lo (first round) - the first unknown word with it
+        u64 x2[K], y2[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            if (go[k]) {
+                x[k] = __ldg(H + ao[k] + R[k]); y[k] = __ldg(H + bo[k] + R[k]);
+                if (probe_lo) { x2[k] = __ldg(H + ao[k] + lo[k]); y2[k] = __ldg(H + bo[k] + lo[k]); }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            if (go[k]) {
+                if (x[k] == y[k]) { res[k] = R[k] + 1; go[k] = false; }
+                else if (probe_lo) {
+                    if (x2[k] != y2[k]) { res[k] = lo[k]; go[k] = false; }
+                    else L[k] = lo[k];
+                }
+                if (go[k] && R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
+            }
+        }
+    }
+    // one bisection step for the elements selected by sel[k]; returns whether any is still going
+    auto step = [&](const bool (&sel)[K]) -> bool {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            if (go[k] && sel[k]) {
+                const i32 p = (L[k] + R[k]) >> 1;
+                x[k] = __ldg(H + ao[k] + p); y[k] = __ldg(H + bo[k] + p);
+            }
+        }
+        bool any = false;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            if (go[k] && sel[k]) {
+                const i32 p = (L[k] + R[k]) >> 1;
+                if (x[k] == y[k]) L[k] = p; else R[k] = p;
+                if (R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
+                any |= go[k];
+            }
+        }
+        return any;
+    };
+    bool all_sel[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) all_sel[k] = true;
+    bool pending = false;
+#pragma unroll
+    for (int k = 0; k < K; ++k) pending |= go[k];
+    if (HINT && __any_sync(FULL, pending)) {
+        bool lead[K];
+        int leader[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const unsigned bal = __ballot_sync(FULL, go[k]);
+            leader[k] = bal ? __ffs(bal) - 1 : -1;
+            lead[k] = lane == leader[k];
+        }
+        bool any = true;
+        while (__any_sync(FULL, any)) any = step(lead);
+        // the others probe around the leader's answer
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const i32 gk = __shfl_sync(FULL, res[k], leader[k] < 0 ? 0 : leader[k]);
+            const bool pr = go[k] && leader[k] >= 0;
+            const bool p1 = pr && gk - 1 > L[k] && gk - 1 < R[k], p2 = pr && gk > L[k] && gk < R[k];
+            if (p1) { x[k] = __ldg(H + ao[k] + gk - 1); y[k] = __ldg(H + bo[k] + gk - 1); }
+            u64 x2 = 0, y2 = 0;
+            if (p2) { x2 = __ldg(H + ao[k] + gk); y2 = __ldg(H + bo[k] + gk); }
+            if (p1) { if (x[k] == y[k]) L[k] = gk - 1; else R[k] = gk - 1; }
+            if (p2 && gk < R[k]) { if (x2 == y2) L[k] = gk; else R[k] = gk; }
+            if (go[k] && R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
+        }
+    }
+    bool any = true;
+    while (any) any = step(all_sel);
+}
+
+__global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    __shared__ GsSmem ssm;
+    __shared__ TreeSmem tsm;
+    const GsStage stg = gs_stage(dyn_smem);
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
     const i64 N = A.N;
-    const i64 gtid = (i64)blockIdx.x * GS_THREADS + threadIdx.x, gsize = (i64)gridDim.x * GS_THREADS;
-    const i64 gwarp = gtid >> 5, nwarps = gsize >> 5;
+    const int G = gridDim.x, me = blockIdx.x;
+    const i64 gtid = (i64)me * GS_THREADS + threadIdx.x;
     Grid g{&A.ctl->bar, 0};
     const u64* __restrict__ H = A.hashes;
     const i64* __restrict__ BO = A.blk_off;
+    const i64 C = (N + G - 1) / G;
+    const i64 c0 = min((i64)me * C, N), c1 = min(c0 + C, N);
+    const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
+    auto IDX = [&](int t, int k) -> i64 { return c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane; };
     PEEK_MARK(1);
 
-    // ---- phase 0: max chain length, initial state (one segment, everything "branch at 0") ----
+    // ---- phase 0: max chain length, identity order ----
     {
         u32 mx = 0;
-        for (i64 r = gtid; r < N; r += gsize) {
-            i64 nb = BO[r + 1] - BO[r];
-            mx = max(mx, (u32)nb);
-            A.bufs.val[0][r] = (u32)r;
+        for (int t = 0; t < ntiles; ++t) {
+            i64 b0[GS_KPT], b1[GS_KPT];
+            ELEMS(k) {
+                const i64 i = IDX(t, k);
+                b0[k] = b1[k] = 0;
+                if (i < c1) { b0[k] = __ldg(BO + i); b1[k] = __ldg(BO + i + 1); A.bufs.val[0][i] = (u32)i; }
+            }
+            ELEMS(k) mx = max(mx, (u32)(b1[k] - b0[k]));
         }
-        mx = __reduce_max_sync(0xffffffffu, mx);
+        mx = __reduce_max_sync(FULL, mx);
         if (lane == 0 && mx) atomicMax(&A.ctl->maxnb, mx);
         if (gtid == 0) { A.ctl->kand[0] = ~0ull; A.ctl->kand[1] = ~0ull; }
     }
     g.sync();
     const KeyLayout kl = make_layout(N, __ldcg(&A.ctl->maxnb));
-    for (i64 r = gtid; r < N; r += gsize) A.bufs.key[0][r] = kl.pack(0, kl.f_before(0, false), 0);
+    {
+        const u64 k_init = kl.pack(0, kl.f_before(0, false), 0);
+        for (int t = 0; t < ntiles; ++t)
+            ELEMS(k) { const i64 i = IDX(t, k); if (i < c1) A.bufs.key[0][i] = k_init; }
+    }
     int cb = 0;  // buffer that holds the current (key, request) pairs by position
 
     for (int round = 0;; ++round) {
-        // ---- R1: segment boundaries from equal keys, max-scan of segment starts, heads ----
         g.sync();  // keys / order of the previous phase visible
         PEEK_MARK(10);
         const u64* K = A.bufs.key[cb];
@@ -134,93 +281,227 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
             A.ctl->kor[(round + 1) & 1] = 0;
             A.ctl->kand[(round + 1) & 1] = ~0ull;
         }
-        for (i64 j = gtid; j < N; j += gsize) {
-            u64 kj = __ldcg(K + j);
-            bool start = j == 0 || __ldcg(K + j - 1) != kj;
-            if (start) {
-                A.seghead[j] = 0;
-                u64 F = kl.F_of(kj);
-                A.segdepth[j] = kl.is_branch(F) ? (i32)(kl.ld_of(F) / kl.D) : 0;
+        // ---- R1a: segment starts (key differs from the left neighbour); last start per CTA ----
+        {
+            i32 cta_last = -1;
+            u32 cta_cnt = 0;  // segment starts seen by this warp
+            for (int t = 0; t < ntiles; ++t)
+            for (int hb = 0; hb < GS_KPT / SB; ++hb) {
+                u64 k0[SB], km[SB];
+                SUBS(k) {
+                    const i64 i = IDX(t, hb * SB + k);
+                    k0[k] = km[k] = 0;
+                    if (i < c1) { k0[k] = __ldcg(K + i); if (i > 0) km[k] = __ldcg(K + i - 1); }
+                }
+                SUBS(k) {
+                    const i64 i = IDX(t, hb * SB + k);
+                    const bool start = i < c1 && (i == 0 || km[k] != k0[k]);
+                    const unsigned bal = __ballot_sync(FULL, start);
+                    if (bal) cta_last = (i32)(i - lane) + 31 - __clz(bal);
+                    cta_cnt += __popc(bal);
+                    if (start) {
+                        A.seghead[i] = 0;
+                        const u64 F = kl.F_of(k0[k]);
+                        A.segdepth[i] = kl.is_branch(F) ? (i32)(kl.ld_of(F) / kl.D) : 0;
+                        // a boundary made by the last sort (both sides come from one segment): the
+                        // two chains leave their old head's path at ldv digits, so they share
+                        // exactly min(ldv) digits - the final adjacent LCP, no chain reads needed
+                        if (i == 0) A.lcp[0] = 0;
+                        else if (round > 0 && kl.seg_of(km[k]) == kl.seg_of(k0[k])) {
+                            const u64 la = kl.ldv(kl.F_of(km[k])), lb = kl.ldv(F);
+                            A.lcp[i] = (i32)((la < lb ? la : lb) / kl.D);
+                        }
+                    }
+                }
+            }
+            if (lane == 0) tsm.wv64[w] = ((i64)cta_cnt << 32) | (u32)(cta_last + 1);
+            __syncthreads();
+            if (w == 0) {
+                const i64 v = lane < GS_WARPS ? tsm.wv64[lane] : 0;
+                const u32 cs = __reduce_add_sync(FULL, (u32)(v >> 32)), ls = __reduce_max_sync(FULL, (u32)v);
+                if (lane == 0) A.agg[me] = ((i64)cs << 32) | ls;
             }
         }
+        g.sync();
+        // ---- R1b: segment start of every position, unresolved flag, head = longest chain ----
         {
-            auto load = [&](i64 j) -> i64 {
-                bool start = j == 0 || __ldcg(K + j - 1) != __ldcg(K + j);
-                return start ? j : 0;
-            };
-            auto store = [&](i64 j, i64 s) {
-                u64 kj = __ldcg(K + j);
-                bool start = j == 0 || __ldcg(K + j - 1) != kj;
-                bool last = j == N - 1 || __ldcg(K + j + 1) != kj;
-                bool unres = kl.is_branch(kl.F_of(kj)) && !(start && last);
-                A.seg[j] = (u32)s | (unres ? 0x80000000u : 0u);
-                // head = longest chain of the segment (lowest position on ties); one atomic per
-                // warp when the whole warp sits in one unresolved segment (the common case)
-                const unsigned act = __activemask();
-                unsigned any = __ballot_sync(act, unres);
-                u32 nb = 0;
-                if (unres) {
-                    u32 r = __ldcg(cur + j);
-                    nb = (u32)(BO[r + 1] - BO[r]);
+            if (w == 0) {  // segment starts in the chunks before mine: how many, and the last one
+                u32 cs = 0, ls = 0;
+                for (int cbase = 0; cbase < me; cbase += 32 * 5) {
+                    i64 x[5];
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) { const int c = cbase + q * 32 + lane; x[q] = c < me ? __ldcg(A.agg + c) : 0; }
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) { cs += (u32)(x[q] >> 32); ls = max(ls, (u32)x[q]); }
                 }
-                int same = 0;
-                __match_all_sync(act, (u32)s, &same);
-                if (same && any == act) {
-                    u32 mnb = __reduce_max_sync(act, nb);
-                    u32 mj = __reduce_max_sync(act, nb == mnb ? 0xffffffffu - (u32)j : 0u);
-                    if (lane == (__ffs(act) - 1)) {
-                        atomicAdd(cnt, (u32)__popc(any));
-                        atomicMax((unsigned long long*)&A.seghead[s], ((u64)mnb << 32) | (u64)mj);
+                cs = __reduce_add_sync(FULL, cs);
+                ls = __reduce_max_sync(FULL, ls);
+                if (lane == 0) tsm.carry64 = ((i64)cs << 32) | ls;
+            }
+            __syncthreads();
+            u32 n_unres = 0;
+            for (int t = 0; t < ntiles; ++t) {
+                unsigned bal[GS_KPT];
+                u32 fl[GS_KPT];  // bit 0 start, bit 1 last, bit 2 branch class
+                u32 wl = 0, wc = 0;  // this warp's last segment start + 1, and how many it has
+#pragma unroll
+                for (int hb = 0; hb < GS_KPT / SB; ++hb) {
+                    u64 k0[SB], km[SB], kp[SB];
+                    SUBS(k) {
+                        const i64 i = IDX(t, hb * SB + k);
+                        k0[k] = km[k] = kp[k] = 0;
+                        if (i < c1) {
+                            k0[k] = __ldcg(K + i);
+                            if (i > 0) km[k] = __ldcg(K + i - 1);
+                            if (i + 1 < N) kp[k] = __ldcg(K + i + 1);
+                        }
                     }
-                } else if (unres) {
-                    if (lane == (__ffs(any) - 1)) atomicAdd(cnt, (u32)__popc(any));
-                    atomicMax((unsigned long long*)&A.seghead[s], ((u64)nb << 32) | (u64)(0xffffffffu - (u32)j));
+                    SUBS(k) {
+                        const i64 i = IDX(t, hb * SB + k);
+                        const bool valid = i < c1;
+                        const bool start = valid && (i == 0 || km[k] != k0[k]);
+                        const bool last = valid && (i == N - 1 || kp[k] != k0[k]);
+                        const bool br = valid && kl.is_branch(kl.F_of(k0[k]));
+                        const unsigned bl = __ballot_sync(FULL, start);
+                        if (bl) wl = (u32)((i - lane) + 31 - __clz(bl)) + 1u;
+                        wc += __popc(bl);
+                        bal[hb * SB + k] = bl;
+                        fl[hb * SB + k] = (start ? 1u : 0u) | (last ? 2u : 0u) | (br ? 4u : 0u);
+                    }
                 }
-            };
-            grid_inscan<i64>(N, load, store, [](i64 a, i64 b) { return a > b ? a : b; }, (i64)0, A.agg, s64, g);
+                if (lane == 0) tsm.wv64[w] = ((i64)wc << 32) | wl;
+                __syncthreads();
+                if (w == 0) {  // exclusive (sum, max) scan over the warps, seeded with the carry
+                    const i64 own = lane < GS_WARPS ? tsm.wv64[lane] : 0;
+                    u32 ic = (u32)(own >> 32), il = (u32)own;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const u32 xc = __shfl_up_sync(FULL, ic, o), xl = __shfl_up_sync(FULL, il, o);
+                        if (lane >= o) { ic += xc; il = max(il, xl); }
+                    }
+                    u32 ec = __shfl_up_sync(FULL, ic, 1), el = __shfl_up_sync(FULL, il, 1);
+                    if (lane == 0) { ec = 0; el = 0; }
+                    const i64 cin = tsm.carry64;
+                    if (lane < GS_WARPS) tsm.wv64[lane] = ((i64)(ec + (u32)(cin >> 32)) << 32) | max(el, (u32)cin);
+                    if (lane == 31) tsm.carry64 = ((i64)(ic + (u32)(cin >> 32)) << 32) | max(il, (u32)cin);
+                }
+                __syncthreads();
+                i32 c = (i32)(u32)tsm.wv64[w] - 1;     // last segment start before this warp's rows
+                u32 cc = (u32)(tsm.wv64[w] >> 32);     // segment starts before this warp's rows
+#pragma unroll
+                for (int hb = 0; hb < GS_KPT / SB; ++hb) {
+                    i32 sarr[SB];
+                    bool un[SB];
+                    u32 r[SB];
+                    SUBS(k) {
+                        const int kk = hb * SB + k;
+                        const i64 i = IDX(t, kk);
+                        const bool valid = i < c1;
+                        const unsigned m = bal[kk] & le_mask;
+                        const i32 s = m ? (i32)(i - lane) + 31 - __clz(m) : c;
+                        if (bal[kk]) c = (i32)(i - lane) + 31 - __clz(bal[kk]);
+                        const u32 rank = cc + __popc(m) - 1u;
+                        cc += __popc(bal[kk]);
+                        un[k] = valid && (fl[kk] & 4u) && (fl[kk] & 3u) != 3u;
+                        sarr[k] = s;
+                        if (valid) { A.seg[i] = (u32)s | (un[k] ? 0x80000000u : 0u); A.srank[i] = rank; }
+                        r[k] = un[k] ? __ldcg(cur + i) : 0u;
+                    }
+                    i64 b0[SB], b1[SB];
+                    SUBS(k) { b0[k] = b1[k] = 0; if (un[k]) { b0[k] = __ldg(BO + r[k]); b1[k] = __ldg(BO + r[k] + 1); } }
+                    SUBS(k) {
+                        // head = longest chain of the segment, lowest position on ties: segmented
+                        // max over the row's runs of equal s, one atomic per run
+                        const i64 i = IDX(t, hb * SB + k);
+                        u64 v = un[k] ? (((u64)(u32)(b1[k] - b0[k]) << 32) | (u64)(0xffffffffu - (u32)i)) : 0ull;
+                        const i32 s = sarr[k];
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const u64 x = __shfl_up_sync(FULL, v, o);
+                            const i32 sx = __shfl_up_sync(FULL, s, o);
+                            if (lane >= o && sx == s && x > v) v = x;
+                        }
+                        const i32 sn = __shfl_down_sync(FULL, s, 1);
+                        if (v && (lane == 31 || sn != s)) atomicMax((unsigned long long*)&A.seghead[s], v);
+                        n_unres += __popc(__ballot_sync(FULL, un[k]));
+                    }
+                }
+                __syncthreads();  // tsm.wv is reused by the next tile
+            }
+            if (lane == 0 && n_unres) atomicAdd(cnt, n_unres);
         }
+        g.sync();
         PEEK_MARK(11);
-        if (__ldcg(cnt) == 0) break;  // grid-uniform: read after the scan's final barrier
+        if (__ldcg(cnt) == 0) break;  // grid-uniform: read after the barrier
 
         // ---- R2: classify every unresolved position against its segment head (keys in place) ----
         {
             u64* Kw = A.bufs.key[cb];
             u64 orv = 0, andv = ~0ull;
-            for (i64 j = gtid; j < N; j += gsize) {
-                u32 sg = A.seg[j];
-                u32 s = sg & 0x7fffffffu;
-                u64 nk;
-                if (!(sg >> 31)) {
-                    nk = kl.pack(s, 0, 0);
-                } else {
-                    u32 r = __ldcg(cur + j);
-                    u64 hv = __ldcg(A.seghead + s);
-                    u32 hp = 0xffffffffu - (u32)hv;
-                    i64 nbh = (i64)(hv >> 32);
-                    u32 h = __ldcg(cur + hp);
-                    i64 nbr = BO[r + 1] - BO[r];
-                    const u64* cr = H + BO[r];
-                    const u64* ch = H + BO[h];
-                    i64 l = (r == h) ? nbr : chain_lcp(cr, nbr, ch, nbh, A.segdepth[s]);
-                    u64 F, dig = 0;
-                    if (l == nbr && l == nbh) F = kl.f_head();
-                    else if (l == nbr) F = kl.f_before((u64)kl.D * l, true);
-                    else {  // l < nbr <= nbh: the words at l differ
-                        u64 a = __ldg(cr + l), b = __ldg(ch + l);
-                        int jd = __clzll((long long)(a ^ b)) / kl.w;
-                        u64 ld = (u64)kl.D * l + jd;
-                        u64 da = (a << (jd * kl.w)) >> (64 - kl.w), db = (b << (jd * kl.w)) >> (64 - kl.w);
-                        dig = da;
-                        F = da < db ? kl.f_before(ld, false) : kl.f_after(ld);
-                    }
-                    nk = kl.pack(s, F, dig);
+            for (int t = 0; t < ntiles; ++t)
+            for (int hb = 0; hb < GS_KPT / SB; ++hb) {
+                u32 sg[SB], r[SB], h[SB], rk[SB];
+                bool un[SB], cmp[SB];
+                SUBS(k) {
+                    const i64 i = IDX(t, hb * SB + k);
+                    sg[k] = 0; r[k] = 0; rk[k] = 0;
+                    if (i < c1) { sg[k] = A.seg[i]; r[k] = __ldcg(cur + i); rk[k] = A.srank[i]; }
+                    un[k] = (sg[k] >> 31) != 0;
                 }
-                Kw[j] = nk;
-                orv |= nk;
-                andv &= nk;
+                u64 hv[SB];
+                i64 ao[SB], bo[SB];
+                i32 na[SB], nb[SB], lo[SB], l[SB];
+                SUBS(k) {
+                    hv[k] = 0; ao[k] = 0; na[k] = 0; lo[k] = 0;
+                    if (un[k]) {
+                        const u32 s = sg[k] & 0x7fffffffu;
+                        hv[k] = __ldcg(A.seghead + s);
+                        lo[k] = __ldcg(A.segdepth + s);
+                        ao[k] = __ldg(BO + r[k]);
+                        na[k] = (i32)(__ldg(BO + r[k] + 1) - ao[k]);
+                    }
+                }
+                SUBS(k) { h[k] = un[k] ? __ldcg(cur + (0xffffffffu - (u32)hv[k])) : 0u; nb[k] = (i32)(hv[k] >> 32); }
+                SUBS(k) {
+                    bo[k] = un[k] ? __ldg(BO + h[k]) : 0;
+                    cmp[k] = un[k] && r[k] != h[k];
+                    l[k] = na[k];  // r == h: the head itself
+                }
+                lcp_lockstep<SB, true>(H, ao, na, bo, nb, lo, cmp, l, round == 0);
+                u64 wa[SB], wb[SB];
+                SUBS(k) {
+                    wa[k] = wb[k] = 0;
+                    if (un[k] && l[k] < na[k]) { wa[k] = __ldg(H + ao[k] + l[k]); wb[k] = __ldg(H + bo[k] + l[k]); }
+                }
+                SUBS(k) {
+                    const i64 i = IDX(t, hb * SB + k);
+                    if (i < c1) {
+                        const u32 s = rk[k];  // dense segment rank: few leading key bits vary
+                        u64 nk;
+                        if (!un[k]) {
+                            nk = kl.pack(s, 0, 0);
+                        } else {
+                            u64 F, dig = 0;
+                            if (l[k] == na[k] && l[k] == nb[k]) F = kl.f_head();
+                            else if (l[k] == na[k]) F = kl.f_before((u64)kl.D * l[k], true);
+                            else {  // l < na <= nb: the words at l differ
+                                const u64 a = wa[k], b = wb[k];
+                                const int jd = __clzll((long long)(a ^ b)) / kl.w;
+                                const u64 ld = (u64)kl.D * l[k] + jd;
+                                const u64 da = (a << (jd * kl.w)) >> (64 - kl.w), db = (b << (jd * kl.w)) >> (64 - kl.w);
+                                dig = da;
+                                F = da < db ? kl.f_before(ld, false) : kl.f_after(ld);
+                            }
+                            nk = kl.pack(s, F, dig);
+                        }
+                        Kw[i] = nk;
+                        orv |= nk;
+                        andv &= nk;
+                    }
+                }
             }
-            const u32 olo = __reduce_or_sync(0xffffffffu, (u32)orv), ohi = __reduce_or_sync(0xffffffffu, (u32)(orv >> 32));
-            const u32 alo = __reduce_and_sync(0xffffffffu, (u32)andv), ahi = __reduce_and_sync(0xffffffffu, (u32)(andv >> 32));
+            const u32 olo = __reduce_or_sync(FULL, (u32)orv), ohi = __reduce_or_sync(FULL, (u32)(orv >> 32));
+            const u32 alo = __reduce_and_sync(FULL, (u32)andv), ahi = __reduce_and_sync(FULL, (u32)(andv >> 32));
             if (lane == 0) {
                 atomicOr(&A.ctl->kor[round & 1], ((unsigned long long)ohi << 32) | olo);
                 atomicAnd(&A.ctl->kand[round & 1], ((unsigned long long)ahi << 32) | alo);
@@ -231,91 +512,268 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
 
         // ---- R3: stable LSD radix sort of the pairs over the bits that vary ----
         const u64 vary = __ldcg(&A.ctl->kor[round & 1]) & ~__ldcg(&A.ctl->kand[round & 1]);
-        cb = grid_sort_pairs(A.bufs, N, vary, g, ssm, cb);
+        cb = grid_sort_pairs(A.bufs, N, vary, g, ssm, stg, cb);
         PEEK_MARK(13);
     }
     const u32* cur = A.bufs.val[cb];
 
-    // ---- F1: final order into `order`, adjacent LCP ----
-    for (i64 j = gtid; j < N; j += gsize) A.order[j] = (i32)cur[j];
-    for (i64 j = gtid; j < N; j += gsize) {
-        i32 l = 0;
-        if (j > 0) {
-            u32 a = cur[j - 1], b = cur[j];
-            l = (i32)chain_lcp(H + BO[a], BO[a + 1] - BO[a], H + BO[b], BO[b + 1] - BO[b], 0);
+    // ---- F1: final order.  The adjacent LCP of every segment boundary was written when the
+    // boundary appeared (R1a); positions inside a final segment repeat their neighbour's chain ----
+    {
+        const u64* K = A.bufs.key[cb];
+        for (int t = 0; t < ntiles; ++t) {
+            u32 r[GS_KPT];
+            bool same[GS_KPT];
+            ELEMS(k) {
+                const i64 i = IDX(t, k);
+                r[k] = 0; same[k] = false;
+                if (i < c1) {
+                    r[k] = __ldcg(cur + i);
+                    if (i > 0) same[k] = __ldcg(K + i) == __ldcg(K + i - 1);
+                }
+            }
+            ELEMS(k) {
+                const i64 i = IDX(t, k);
+                if (i < c1) {
+                    A.order[i] = (i32)r[k];
+                    if (same[k]) A.lcp[i] = (i32)(__ldg(BO + r[k] + 1) - __ldg(BO + r[k]));
+                }
+            }
         }
-        A.lcp[j] = l;
     }
     PEEK_MARK(20);
     const bool want_groups = A.group_id || A.group_size || A.n_groups;
     const bool want_clusters = A.cluster_depth || A.cluster_size || A.cluster_id;
     if (!want_groups && !want_clusters) return;
     g.sync();
+    MinTree mt;
+    mintree_layout(mt, A.lcp, N, A.mt_buf);
+    const i64 gwarp = gtid >> 5, nwarps = ((i64)G * GS_THREADS) >> 5;
 
-    // ---- F3: groups: sum-scan of (lcp == 0) flags and max-scan of their positions, packed ----
-    if (want_groups) {
-        auto op = [](i64 a, i64 b) -> i64 {
-            i64 hs = (a >> 32) + (b >> 32);
-            u32 la = (u32)a, lb = (u32)b;
-            return (hs << 32) | (i64)(la > lb ? la : lb);
-        };
-        auto load = [&](i64 j) -> i64 { return __ldcg(A.lcp + j) == 0 ? (((i64)1 << 32) | j) : 0; };
-        auto store = [&](i64 j, i64 v) {
-            i32 gid = (i32)(v >> 32) - 1;
-            i64 gstart = (u32)v;
-            A.seg[j] = (u32)gid;
-            bool last = j == N - 1 || __ldcg(A.lcp + j + 1) == 0;
-            if (last) {
-                A.gsz[gid] = (i32)(j - gstart + 1);
-                if (j == N - 1 && A.n_groups) *A.n_groups = gid + 1;
+    // ---- G1: per-CTA count of group starts (lcp == 0) and the last one; min-hierarchy level 1 ----
+    {
+        u32 cntw = 0;
+        i32 lastw = -1;
+        for (int t = 0; t < ntiles; ++t) {
+            i32 lv[GS_KPT];
+            ELEMS(k) { const i64 i = IDX(t, k); lv[k] = i < c1 ? __ldcg(A.lcp + i) : 1; }
+            ELEMS(k) {
+                const i64 i = IDX(t, k);
+                const unsigned bal = __ballot_sync(FULL, lv[k] == 0);
+                cntw += __popc(bal);
+                if (bal) lastw = (i32)(i - lane) + 31 - __clz(bal);
             }
-        };
-        grid_inscan<i64>(N, load, store, op, (i64)0, A.agg, s64, g);
-        for (i64 j = gtid; j < N; j += gsize) {
-            u32 r = (u32)A.order[j];
-            i32 gid = (i32)A.seg[j];
-            if (A.group_id) A.group_id[r] = gid;
-            if (A.group_size) A.group_size[r] = __ldcg(A.gsz + gid);
+        }
+        if (lane == 0) tsm.wv64[w] = ((i64)cntw << 32) | (u32)(lastw + 1);
+        __syncthreads();
+        if (w == 0) {
+            const i64 v = lane < GS_WARPS ? tsm.wv64[lane] : 0;
+            const u32 cs = __reduce_add_sync(FULL, (u32)(v >> 32)), ls = __reduce_max_sync(FULL, (u32)v);
+            if (lane == 0) A.agg[me] = ((i64)cs << 32) | ls;
+        }
+        if (want_clusters && mt.levels > 1) mintree_build_level(mt, 1, gwarp, nwarps, lane);
+    }
+    g.sync();
+    // ---- G2: group id / start of every position, group sizes; min-hierarchy level 2 ----
+    {
+        if (w == 0) {
+            u32 cs = 0, ls = 0;
+            for (int cbase = 0; cbase < me; cbase += 32 * 5) {
+                i64 x[5];
+#pragma unroll
+                for (int q = 0; q < 5; ++q) { const int c = cbase + q * 32 + lane; x[q] = c < me ? __ldcg(A.agg + c) : 0; }
+#pragma unroll
+                for (int q = 0; q < 5; ++q) { cs += (u32)(x[q] >> 32); ls = max(ls, (u32)x[q]); }
+            }
+            cs = __reduce_add_sync(FULL, cs);
+            ls = __reduce_max_sync(FULL, ls);
+            if (lane == 0) tsm.carry64 = ((i64)cs << 32) | ls;
+        }
+        __syncthreads();
+        for (int t = 0; t < ntiles; ++t) {
+            i32 lv[GS_KPT], ln[GS_KPT];
+            unsigned bal[GS_KPT];
+            ELEMS(k) {
+                const i64 i = IDX(t, k);
+                lv[k] = 1; ln[k] = 0;
+                if (i < c1) { lv[k] = __ldcg(A.lcp + i); if (i + 1 < N) ln[k] = __ldcg(A.lcp + i + 1); }
+            }
+            u32 cntw = 0, lastw = 0;
+            ELEMS(k) {
+                const i64 i = IDX(t, k);
+                bal[k] = __ballot_sync(FULL, lv[k] == 0);
+                cntw += __popc(bal[k]);
+                if (bal[k]) lastw = (u32)((i - lane) + 31 - __clz(bal[k])) + 1u;
+            }
+            if (lane == 0) tsm.wv64[w] = ((i64)cntw << 32) | lastw;
+            __syncthreads();
+            if (w == 0) {  // exclusive (sum, max) scan over the warps, seeded with the carry
+                const i64 own = lane < GS_WARPS ? tsm.wv64[lane] : 0;
+                u32 ic = (u32)(own >> 32), il = (u32)own;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const u32 xc = __shfl_up_sync(FULL, ic, o), xl = __shfl_up_sync(FULL, il, o);
+                    if (lane >= o) { ic += xc; il = max(il, xl); }
+                }
+                u32 ec = __shfl_up_sync(FULL, ic, 1), el = __shfl_up_sync(FULL, il, 1);
+                if (lane == 0) { ec = 0; el = 0; }
+                const i64 cin = tsm.carry64;
+                if (lane < GS_WARPS) tsm.wv64[lane] = ((i64)(ec + (u32)(cin >> 32)) << 32) | max(el, (u32)cin);
+                if (lane == 31) tsm.carry64 = ((i64)(ic + (u32)(cin >> 32)) << 32) | max(il, (u32)cin);
+            }
+            __syncthreads();
+            u32 cc = (u32)(tsm.wv64[w] >> 32), cl = (u32)tsm.wv64[w];
+            ELEMS(k) {
+                const i64 i = IDX(t, k);
+                const unsigned m = bal[k] & le_mask;
+                const i32 gid = (i32)(cc + __popc(m)) - 1;
+                const i64 gstart = m ? (i - lane) + 31 - __clz(m) : (i64)cl - 1;
+                cc += __popc(bal[k]);
+                if (bal[k]) cl = (u32)((i - lane) + 31 - __clz(bal[k])) + 1u;
+                if (i < c1) {
+                    A.seg[i] = (u32)gid;
+                    if (i == N - 1 || ln[k] == 0) {
+                        A.gsz[gid] = (i32)(i - gstart + 1);
+                        if (i == N - 1 && A.n_groups) *A.n_groups = gid + 1;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        if (want_clusters && mt.levels > 2) mintree_build_level(mt, 2, gwarp, nwarps, lane);
+    }
+    g.sync();
+    // ---- min-hierarchy levels >= 3: a private copy per CTA in shared memory when they fit ----
+    if (want_clusters && mt.levels > 3) {
+        if (mt.n[3] <= 2048) {
+            int off = 0;
+            for (int k = 3; k < mt.levels; ++k) {
+                mt.lvl[k] = tsm.lvl_hi + off;
+                off += k == 3 ? 2048 : (k == 4 ? 64 : 2);
+            }
+            for (int k = 3; k < mt.levels; ++k) {
+                mintree_build_level(mt, k, (i64)w, (i64)GS_WARPS, lane);
+                __syncthreads();
+            }
+        } else {
+            for (int k = 3; k < mt.levels; ++k) {
+                mintree_build_level(mt, k, gwarp, nwarps, lane);
+                g.sync();
+            }
         }
     }
     PEEK_MARK(21);
-    if (!want_clusters) return;
-
-    // ---- F4: clusters by nearest-smaller-value searches on the LCP array ----
-    MinTree mt;
-    mintree_layout(mt, A.lcp, N, A.mt_buf);
-    for (int k = 1; k < mt.levels; ++k) {
-        mintree_build_level(mt, k, gwarp, nwarps, lane);
-        g.sync();
-    }
-    for (i64 j = gtid; j < N; j += gsize) {
-        u32 r = (u32)A.order[j];
-        i32 l0 = A.lcp[j], l1 = j + 1 < N ? A.lcp[j + 1] : 0;
-        i32 cd = l0 > l1 ? l0 : l1;
-        i32 cs = 1;
-        i64 cid = (i64)((u64)j << 32);
-        if (cd > 0) {
-            i64 a = nsv_prev_less(mt, j, cd);
-            i64 b = nsv_next_less(mt, j + 1, cd) - 1;
-            cs = (i32)(b - a + 1);
-            cid = (i64)(((u64)a << 32) | (u64)(u32)cd);
+    // ---- G3: group outputs; clusters by nearest-smaller-value walks on the LCP array, in lock step ----
+    for (int t = 0; t < ntiles; ++t)
+    for (int hb = 0; hb < GS_KPT / SB; ++hb) {
+        u32 r[SB];
+        i32 gid[SB], l0[SB], l1[SB];
+        SUBS(k) {
+            const i64 i = IDX(t, hb * SB + k);
+            r[k] = 0; gid[k] = 0; l0[k] = 0; l1[k] = 0;
+            if (i < c1) {
+                r[k] = (u32)A.order[i];
+                if (want_groups) gid[k] = (i32)A.seg[i];
+                l0[k] = __ldcg(A.lcp + i);
+                if (i + 1 < N) l1[k] = __ldcg(A.lcp + i + 1);
+            }
         }
-        if (A.cluster_depth) A.cluster_depth[r] = cd;
-        if (A.cluster_size) A.cluster_size[r] = cs;
-        if (A.cluster_id) A.cluster_id[r] = cid;
+        if (want_groups) {
+            i32 gs[SB];
+            SUBS(k) { const i64 i = IDX(t, hb * SB + k); gs[k] = i < c1 ? __ldcg(A.gsz + gid[k]) : 0; }
+            SUBS(k) {
+                const i64 i = IDX(t, hb * SB + k);
+                if (i < c1) {
+                    if (A.group_id) A.group_id[r[k]] = gid[k];
+                    if (A.group_size) A.group_size[r[k]] = gs[k];
+                }
+            }
+        }
+        if (!want_clusters) continue;
+        i32 cd[SB];
+        i64 pa[SB], pb[SB];
+        int lv[SB];
+        bool go[SB];
+        // a = largest p <= i with L0x[p] < cd
+        bool any = false;
+        SUBS(k) {
+            const i64 i = IDX(t, hb * SB + k);
+            cd[k] = l0[k] > l1[k] ? l0[k] : l1[k];
+            go[k] = i < c1 && cd[k] > 0;
+            pa[k] = i; lv[k] = 0;
+            if (go[k] && l0[k] < cd[k]) go[k] = false;  // the position itself (value already at hand)
+            else if (go[k]) { if ((i & 31) == 0) { pa[k] = (i >> 5) - 1; lv[k] = 1; } else pa[k] = i - 1; }
+            any |= go[k];
+        }
+        while (any) {
+            i32 v[SB];
+            SUBS(k) v[k] = go[k] ? mt.val(lv[k], pa[k]) : 0;
+            any = false;
+            SUBS(k) {
+                if (go[k]) {
+                    if (v[k] < cd[k]) {
+                        if (lv[k] == 0) go[k] = false;
+                        else { --lv[k]; pa[k] = min(pa[k] * 32 + 31, mt.n[lv[k]] - 1); }
+                    } else if ((pa[k] & 31) == 0) { pa[k] = (pa[k] >> 5) - 1; ++lv[k]; }
+                    else --pa[k];
+                }
+                any |= go[k];
+            }
+        }
+        // b + 1 = smallest q >= i + 1 with L0x[q] < cd
+        any = false;
+        SUBS(k) {
+            const i64 i = IDX(t, hb * SB + k);
+            go[k] = i < c1 && cd[k] > 0;
+            pb[k] = i + 1; lv[k] = 0;
+            if (go[k] && l1[k] < cd[k]) go[k] = false;  // position i + 1 itself
+            else if (go[k]) {
+                if (((i + 1) & 31) == 31 || i + 1 == mt.n[0] - 1) { pb[k] = ((i + 1) >> 5) + 1; lv[k] = 1; } else pb[k] = i + 2;
+            }
+            any |= go[k];
+        }
+        while (any) {
+            i32 v[SB];
+            SUBS(k) v[k] = go[k] ? mt.val(lv[k], pb[k]) : 0;
+            any = false;
+            SUBS(k) {
+                if (go[k]) {
+                    if (v[k] < cd[k]) {
+                        if (lv[k] == 0) go[k] = false;
+                        else { --lv[k]; pb[k] = pb[k] * 32; }
+                    } else if ((pb[k] & 31) == 31 || pb[k] == mt.n[lv[k]] - 1) { pb[k] = (pb[k] >> 5) + 1; ++lv[k]; }
+                    else ++pb[k];
+                }
+                any |= go[k];
+            }
+        }
+        SUBS(k) {
+            const i64 i = IDX(t, hb * SB + k);
+            if (i < c1) {
+                i32 cs = 1;
+                i64 cid = (i64)((u64)i << 32);
+                if (cd[k] > 0) {
+                    cs = (i32)(pb[k] - pa[k]);
+                    cid = (i64)(((u64)pa[k] << 32) | (u64)(u32)cd[k]);
+                }
+                if (A.cluster_depth) A.cluster_depth[r[k]] = cd[k];
+                if (A.cluster_size) A.cluster_size[r[k]] = cs;
+                if (A.cluster_id) A.cluster_id[r[k]] = cid;
+            }
+        }
     }
     PEEK_MARK(22);
 }
 
-
 static void tree_layout(Arena& a, i64 N, int grid, TreeArgs& A) {
     A.ctl = a.take<TreeCtl>(1);
+    A.bufs.hist = a.take<u32>(gs_hist_words(grid));  // directly after ctl: one memset clears both
     A.bufs.key[0] = a.take<u64>(N);
     A.bufs.key[1] = a.take<u64>(N);
     A.bufs.val[0] = a.take<u32>(N);
     A.bufs.val[1] = a.take<u32>(N);
-    A.bufs.hist = a.take<u32>(256 * (i64)grid);
     A.seg = a.take<u32>(N);
+    A.srank = a.take<u32>(N);
     A.seghead = a.take<u64>(N);
     A.segdepth = a.take<i32>(N);
     A.agg = a.take<i64>(grid);
@@ -360,10 +818,16 @@ extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* 
     A.cluster_depth = cluster_depth; A.cluster_size = cluster_size; A.cluster_id = cluster_id;
     A.n_groups = n_groups;
     tree_layout(a, N, MAX_GRID, A);
-    PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, sizeof(TreeCtl), st));
+    PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(MAX_GRID)) - (char*)A.ctl), st));
     void* params[] = {&A};
     Prof pr(PROF_TREE, st, 1);
-    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(GS_THREADS), params, 0, st));
+    static bool attr_set = false;
+    if (!attr_set) {
+        PEEK_CUDA(cudaFuncSetAttribute(k_pending_tree, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
+        attr_set = true;
+    }
+    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(GS_THREADS), params,
+                                          GS_STAGE_BYTES, st));
     return PEEK_OK;
 }
 
