@@ -182,8 +182,11 @@ peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* blk_off, int
  *     PEEK_LPM_SPECULATIVE     every position walks in parallel from its shared depth, a scan
  *                              resolves which walks were needed
  * PEEK_OPT_LPM_WINDOW    sorted positions per dual-walk window (0 = automatic)
+ * PEEK_OPT_GRID_LIMIT    cap on the CTAs of the persistent (cooperative) kernels of
+ *                        peek_pending_tree and peek_demand_rank; 0 = one per SM (default).  A test
+ *                        hook: a small cap makes every CTA loop over several tiles at small N.
  * Unknown key or bad value -> PEEK_ERR_INVALID_ARG. */
-enum { PEEK_OPT_LPM_STRATEGY = 1, PEEK_OPT_LPM_WINDOW = 2 };
+enum { PEEK_OPT_LPM_STRATEGY = 1, PEEK_OPT_LPM_WINDOW = 2, PEEK_OPT_GRID_LIMIT = 3 };
 enum { PEEK_LPM_AUTO = 0, PEEK_LPM_DUAL_WALK = 1, PEEK_LPM_SPECULATIVE = 2 };
 peek_status peek_set_option(int32_t key, int64_t value);
 

@@ -240,7 +240,7 @@ def peek_demand_rank(hashes=None, blk_off=None, tree: Optional[PendingTree] = No
     return demand, out
 
 
-OPT_LPM_STRATEGY, OPT_LPM_WINDOW = 1, 2
+OPT_LPM_STRATEGY, OPT_LPM_WINDOW, OPT_GRID_LIMIT = 1, 2, 3
 LPM_AUTO, LPM_DUAL_WALK, LPM_SPECULATIVE = 0, 1, 2
 
 

@@ -20,6 +20,12 @@ peek_status cuda_fail(cudaError_t e, const char* what) {
     return PEEK_ERR_CUDA;
 }
 
+static int g_grid_limit = 0;  // PEEK_OPT_GRID_LIMIT
+int persistent_ctas() {       // CTAs of a persistent cooperative kernel: one per SM unless capped
+    int n = sm_count();
+    return (g_grid_limit > 0 && g_grid_limit < n) ? g_grid_limit : n;
+}
+
 int sm_count() {
     int dev = 0, n = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 148;
@@ -110,6 +116,10 @@ extern "C" peek_status peek_set_option(int32_t key, int64_t value) {
     if ((key == PEEK_OPT_LPM_STRATEGY && value >= 0 && value <= 2) ||
         (key == PEEK_OPT_LPM_WINDOW && value >= 0 && value <= (1 << 20))) {
         peek::lpm_set_option(key, value);
+        return PEEK_OK;
+    }
+    if (key == PEEK_OPT_GRID_LIMIT && value >= 0 && value <= 65536) {
+        peek::g_grid_limit = (int)value;
         return PEEK_OK;
     }
     peek::set_error("peek_set_option: unknown key %d or bad value %lld", key, (long long)value);

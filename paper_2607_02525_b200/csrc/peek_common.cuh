@@ -19,6 +19,7 @@ namespace peek {
 void set_error(const char* fmt, ...);
 peek_status cuda_fail(cudaError_t e, const char* what);
 int sm_count();  // SMs of the current device (148 on B200)
+int persistent_ctas();  // grid of the persistent cooperative kernels (PEEK_OPT_GRID_LIMIT)
 
 // tracing slots (peek_profile_*)
 enum ProfSlot {

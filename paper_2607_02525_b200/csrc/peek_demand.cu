@@ -305,7 +305,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
     }
     if (clpm_order) {
         A.hit = hit; A.csize = cluster_size; A.arrival = arrival; A.N = N; A.out = clpm_order;
-        int grid = sm_count();  // one CTA of GS_THREADS per SM (co-resident: cooperative launch)
+        int grid = persistent_ctas();  // one CTA of GS_THREADS per SM (co-resident: cooperative launch)
         if (grid > RANK_MAX_GRID) grid = RANK_MAX_GRID;
         i64 want = (N + GS_THREADS - 1) / GS_THREADS;
         if (want < grid) grid = (int)(want < 1 ? 1 : want);

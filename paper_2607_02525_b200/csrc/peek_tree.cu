@@ -807,7 +807,7 @@ extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* 
         return PEEK_ERR_WORKSPACE;
     }
     cudaStream_t st = (cudaStream_t)stream;
-    int grid = sm_count();  // one CTA of GS_THREADS per SM, all co-resident (cooperative launch)
+    int grid = persistent_ctas();  // one CTA of GS_THREADS per SM, all co-resident (cooperative launch)
     if (grid > MAX_GRID) grid = MAX_GRID;
     i64 want = (N + GS_THREADS - 1) / GS_THREADS;  // no point in more CTAs than work
     if (want < grid) grid = (int)(want < 1 ? 1 : want);

@@ -192,3 +192,94 @@ def test_arg_errors():
     off = torch.zeros(5, dtype=torch.int64, device=DEV)
     with pytest.raises(b.PeekError):
         b.peek_lpm(None, off, None, off, radix=None, t_keys=torch.zeros(6, dtype=torch.uint64, device=DEV))
+
+
+def _nested_queue(rng, n, vocab=4):
+    """Short requests over a tiny vocabulary: deep nesting, duplicates, prefix-of relations."""
+    stems = [rng.integers(0, vocab, size=int(rng.integers(16, 400))).astype(np.int32) for _ in range(40)]
+    reqs = []
+    for _ in range(n):
+        s = stems[int(rng.integers(0, len(stems)))]
+        cut = int(rng.integers(0, len(s) + 1))
+        tail = rng.integers(0, vocab, size=int(rng.integers(0, 48))).astype(np.int32)
+        reqs.append(np.concatenate([s[:cut], tail]))
+    return reqs, stems
+
+
+@pytest.mark.parametrize("grid_limit", [1, 3, 0])
+def test_persistent_kernels_multi_tile(grid_limit):
+    """peek_pending_tree / peek_demand_rank with the cooperative grid capped (PEEK_OPT_GRID_LIMIT):
+    with 1 or 3 CTAs every CTA owns several 8192-position tiles, so the tile loops, the carries
+    across tiles and CTAs and the multi-tile sort passes all run; results never depend on it."""
+    b = _b()
+    rng = np.random.default_rng(77)
+    reqs, stems = _nested_queue(rng, 30011)
+    toks, off = _csr(reqs)
+    radix, t_keys = _cache_from(stems[:20], 1 << 13)
+    b.set_option(b.OPT_GRID_LIMIT, grid_limit)
+    try:
+        run_pipeline(toks, off, radix, t_keys, rng.permutation(len(reqs)).astype(np.int32),
+                     check_tree_free=False)
+    finally:
+        b.set_option(b.OPT_GRID_LIMIT, 0)
+
+
+def test_rank_two_phase_wide_keys():
+    """cLPM keys too wide for one 64-bit packed key (full-range hit, cluster size and arrival):
+    the arrival sort followed by the stable (hit, cluster size) sort."""
+    b = _b()
+    rng = np.random.default_rng(3)
+    n = 20000
+    hit = rng.integers(-2**31, 2**31 - 1, size=n, dtype=np.int64).astype(np.int32)
+    hit[::3] = hit[0]  # ties on the leading key
+    cs = rng.integers(-2**31, 2**31 - 1, size=n, dtype=np.int64).astype(np.int32)
+    cs[::2] = 7
+    arr = rng.integers(-2**31, 2**31 - 1, size=n, dtype=np.int64).astype(np.int32)
+    arr[::5] = arr[1]  # duplicate arrivals: the request index decides
+    for a in (arr, None):
+        _, g_ord = b.peek_demand_rank(None, None, tree=None, t_keys=None, hit=_dev(hit),
+                                      cluster_size=_dev(cs), arrival=_dev(a) if a is not None else None)
+        assert np.array_equal(_np(g_ord), oracle.clpm_order(hit, cs, a))
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_size_configs(cfg):
+    """BASELINE.json configs[1..4] at FULL size in the launch configuration bench.py times (config 5:
+    N = 1 048 576, 4.28e9 tokens, one CTA per SM): every output of every call against the oracle,
+    element by element.  For config 5 the oracle needs the 17 GB of tokens on the host and about
+    half a minute."""
+    b = _b()
+    wl = W.make(cfg, seed=42)
+    d_tok, d_off = wl.queue.materialize(DEV)
+    toks = d_tok.cpu().numpy()
+    off = d_off.cpu().numpy()
+    cache = W.build_cache(wl, lambda t, o: oracle.block_hash(t, o, 16, 0))
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    NB = int(o_bo[-1])
+    g_bo, g_h = b.peek_block_hash(d_tok, d_off, NB)
+    assert np.array_equal(_np(g_bo), o_bo)
+    assert np.array_equal(_np(g_h), o_h)
+
+    gt = b.peek_pending_tree(g_h, g_bo)
+    ot = oracle.pending_tree(o_h, o_bo)
+    for name in ("order", "lcp", "group_id", "group_size", "cluster_depth", "cluster_size", "cluster_id"):
+        assert np.array_equal(_np(getattr(gt, name)), getattr(ot, name)), name
+    assert int(gt.n_groups.item()) == ot.n_groups
+
+    d_keys = _dev(cache.t_keys.view(np.int64), torch.uint64)
+    d_radix = _radix_dev(cache.radix) if cache.radix is not None else None
+    g_hr, g_hh = b.peek_lpm(d_tok, d_off, g_h, g_bo, radix=d_radix, t_keys=d_keys, tree=gt)
+    o_hh = oracle.lpm_hash(o_h, o_bo, cache.t_keys)
+    assert np.array_equal(_np(g_hh), o_hh)
+    o_hit = o_hh
+    if cache.radix is not None:
+        o_hr = oracle.lpm_radix(toks, off, _orc_radix(cache.radix))
+        assert np.array_equal(_np(g_hr), o_hr)
+        # mirrored, prefix-closed table: the two modes agree up to block rounding (SURVEY 8(c)-P5)
+        assert np.array_equal(o_hh, 16 * (o_hr // 16))
+        o_hit = o_hr
+
+    g_dem, g_ord = b.peek_demand_rank(g_h, g_bo, tree=gt, t_keys=d_keys, hit=_dev(o_hit),
+                                      cluster_size=_dev(ot.cluster_size), arrival=_dev(wl.arrival))
+    assert np.array_equal(_np(g_dem), oracle.demand(o_h, o_bo, cache.t_keys))
+    assert np.array_equal(_np(g_ord), oracle.clpm_order(o_hit, ot.cluster_size, wl.arrival))
