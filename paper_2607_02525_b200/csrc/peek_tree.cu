@@ -2,8 +2,10 @@
 // a batch: lexicographic order of the requests' hash chains (= DFS order of the compressed trie),
 // adjacent LCP (= its branching depths), flat groups and per-request clusters.
 //
-// ONE persistent cooperative kernel (a CTA per SM slot, grid barriers between phases), because
-// the number of refinement rounds is data dependent and the call may not synchronise with the host.
+// ONE persistent cooperative kernel (one CTA of GS_THREADS per SM, grid barriers between phases),
+// because the number of refinement rounds is data dependent and the call may not synchronise with
+// the host.  The pairs (sort key, request) are kept BY POSITION and go through peek_sort.cuh's
+// key/value sort; every phase walks the CTA's own chunk of positions in register tiles.
 //
 // Sort = path-peeling refinement.  Every unresolved segment (a run of sorted positions whose
 // chains share a prefix) picks its LONGEST chain as head h.  A member r is classified by its
@@ -12,10 +14,16 @@
 //     r's digit < h's at the LCP      -> before h, by ascending LCP, then digit
 //     r identical to h                -> with h
 //     r's digit > h's at the LCP      -> after h, by DESCENDING LCP, then digit
-// One stable LSD radix sort by key = [segment start | class+LCP | digit] splits the segment along
+// One stable LSD radix sort by key = [segment rank | class+LCP | digit] splits the segment along
 // the whole root-to-leaf path of h at once, so rounds ~ 3 on the paper's workloads (shared
-// prompt / conversation / turn) instead of one per trie level.  LCPs use the chain property
-// (k_i equal => all earlier words equal, R15) to binary-search the first differing word.
+// prompt / conversation / turn) instead of one per trie level; only the key bits that vary are
+// sorted on.  LCPs with the head use the chain property (k_i equal => all earlier words equal,
+// DESIGN.md R15) to bisect for the first differing word; the probes are random 32-byte sectors of
+// the hash array (the phase is HBM-transaction bound), so a warp row lets one lane bisect and the
+// others verify its answer with one probe pair (lcp_lockstep).
+// The ADJACENT LCP (output `lcp`) costs no chain reads at all: when a sort splits two neighbours
+// that came from one segment, they leave the old head's path at known digit depths, and
+// min(depths) / D is exactly their LCP (R1a); neighbours never split have identical chains.
 #include "peek_sort.cuh"
 
 namespace peek {
