@@ -228,6 +228,36 @@ SLOT_TO_CALL = {"hash.nb_scan": "hash", "hash.content": "hash.content", "hash.ch
                 "lpm.resolve_scan": None, "demand.count": "demand", "rank.clpm_sort": "rank"}
 
 
+def gather_ceiling(inp, dev):
+    """Random 32-byte-sector gather ceilings: the honest roofline of the probe /
+    child-lookup kernels.  Over a buffer far larger than L2 (the token array, capped at 4 GiB) and
+    over the table itself (8 S bytes: partly L2 resident)."""
+    from paper_2607_02525_b200 import binding as B
+    out = {}
+    tok_bytes = inp.tok.numel() * 4
+    big = inp.tok[: min(inp.tok.numel(), 1 << 30)] if tok_bytes >= (1 << 28) else None
+    for name, buf in (("hbm", big), ("table", inp.keys)):
+        if buf is None or buf.numel() * buf.element_size() < 64:
+            continue
+        if buf.data_ptr() % 32:
+            continue
+        reads = 1 << 26
+        B.bench_random_gather(buf, reads, 1)
+        torch.cuda.synchronize()
+        best = None
+        for it in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            B.bench_random_gather(buf, reads, 2 + it)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None or ms < best else best
+        out[name] = {"buffer_bytes": int(buf.numel() * buf.element_size()), "reads": reads,
+                     "Gsectors_per_s": reads / (best * 1e-3) / 1e9, "GBps": 32 * reads / (best * 1e-3) / 1e9}
+    return out
+
+
 def measured_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -433,6 +463,11 @@ def run_peek(args):
         if call and call in balg and per > 0:
             calls[slot]["alg_bytes"] = balg[call]
             calls[slot]["alg_GBps"] = balg[call] / (per * 1e-3) / 1e9
+    ceil = gather_ceiling(inp, dev)
+    if "hbm" in ceil:
+        for slot in ("lpm.radix_walk", "lpm.hash_probe", "demand.count"):
+            if slot in calls and "alg_GBps" in calls[slot]:
+                calls[slot]["frac_of_random_sector_ceiling"] = calls[slot]["alg_GBps"] / ceil["hbm"]["GBps"]
     dom = max(prof, key=lambda s: prof[s][0])
     dom_call = SLOT_TO_CALL.get(dom)
     dom_ms = prof[dom][0] / max(prof[dom][1], 1)
@@ -450,7 +485,8 @@ def run_peek(args):
                        "block_size": 16, "parallelism": "independent batches per GPU, no collective",
                        "l2": "256 MB buffer written between timed steps; inputs %.1f GB" % (inp.T * 4 / 1e9)},
             "tokens_matched_per_s": world * sum_hit * args.steps / (t_ms * 1e-3),
-            "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roofline, "calls": calls}
+            "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roofline, "calls": calls,
+            "random_sector_gather_ceiling": ceil}
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(inp.wl, inp.cache, args.cpu_seconds)
     print(json.dumps(line), flush=True)

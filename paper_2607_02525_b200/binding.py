@@ -20,7 +20,7 @@ _lib = None
 CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
-           "peek_launch_count", "peek_set_option",
+           "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank"]
 
 
@@ -71,6 +71,8 @@ def lib():
         L.peek_demand_rank.restype = i32
         L.peek_demand_rank.argtypes = [vp, vp, i64, vp, vp, ctypes.POINTER(_Table), vp, vp, vp, vp, vp,
                                        vp, i64, vp]
+        L.peek_bench_random_gather.restype = i32
+        L.peek_bench_random_gather.argtypes = [vp, i64, i64, u64, vp, vp]
         _lib = L
     return _lib
 
@@ -276,3 +278,13 @@ def launch_count() -> int:
     L = lib()
     L.peek_launch_count.restype = ctypes.c_int64
     return int(L.peek_launch_count())
+
+
+def bench_random_gather(buf: torch.Tensor, reads: int, seed: int = 1) -> torch.Tensor:
+    """Measurement utility (include/peek.h): `reads` random 32-byte-sector loads over `buf`;
+    returns the device sink word.  Time it with CUDA events."""
+    sink = torch.zeros(1, dtype=torch.int64, device=buf.device)
+    st = lib().peek_bench_random_gather(_ptr(buf), buf.numel() * buf.element_size(), int(reads), int(seed),
+                                        _ptr(sink), _stream())
+    _check(st, "peek_bench_random_gather")
+    return sink

@@ -48,6 +48,7 @@ struct TreeArgs {
     GsBufs bufs;      // (sort key, request) by position, ping-pong
     u32* seg;         // N   by position: segment start | unresolved << 31
     u32* srank;       // N   by position: dense rank of the segment (the sort key's leading field)
+    u64* lasth;       // N   by request: last word of its chain (read once; every round's first probe)
     u64* seghead;     // N   by segment start: (nb << 32) | ~position of the longest chain
     i32* segdepth;    // N   by segment start: blocks all members are known to share
     i64* agg;         // gridDim scratch for grid scans
@@ -141,7 +142,8 @@ struct TreeSmem {
 template <int K, bool HINT>
 __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i64 (&ao)[K], const i32 (&na)[K],
                                              const i64 (&bo)[K], const i32 (&nb)[K], const i32 (&lo)[K],
-                                             const bool (&act)[K], i32 (&res)[K], bool probe_lo) {
+                                             const bool (&act)[K], i32 (&res)[K], bool probe_lo,
+                                             const u64 (&alast)[K]) {  // alast[k] = H[ao[k] + na[k] - 1]
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     i32 L[K], R[K];  // while go: equal below/at L (L = lo - 1: nothing known), differ at R
@@ -161,7 +163,8 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             if (go[k]) {
-                x[k] = __ldg(H + ao[k] + R[k]); y[k] = __ldg(H + bo[k] + R[k]);
+                x[k] = R[k] == na[k] - 1 ? alast[k] : __ldg(H + ao[k] + R[k]);
+                y[k] = __ldg(H + bo[k] + R[k]);
                 if (probe_lo) { x2[k] = __ldg(H + ao[k] + lo[k]); y2[k] = __ldg(H + bo[k] + lo[k]); }
             }
         }
@@ -264,6 +267,11 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                 if (i < c1) { b0[k] = __ldg(BO + i); b1[k] = __ldg(BO + i + 1); A.bufs.val[0][i] = (u32)i; }
             }
             ELEMS(k) mx = max(mx, (u32)(b1[k] - b0[k]));
+            // the last word of every chain, gathered once: a member's chain is never longer than
+            // its head's, so the "does one chain prefix the other" probe of every round reads it
+            u64 lw[GS_KPT];
+            ELEMS(k) lw[k] = b1[k] > b0[k] ? __ldg(H + b1[k] - 1) : 0ull;
+            ELEMS(k) { const i64 i = IDX(t, k); if (i < c1) A.lasth[i] = lw[k]; }
         }
         mx = __reduce_max_sync(FULL, mx);
         if (lane == 0 && mx) atomicMax(&A.ctl->maxnb, mx);
@@ -348,6 +356,8 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
             }
             __syncthreads();
             u32 n_unres = 0;
+            u64 carry_v = 0;  // head candidate of the segment the warp's last full rows lay in
+            i32 carry_s = 0;
             for (int t = 0; t < ntiles; ++t) {
                 unsigned bal[GS_KPT];
                 u32 fl[GS_KPT];  // bit 0 start, bit 1 last, bit 2 branch class
@@ -429,13 +439,30 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                             const i32 sx = __shfl_up_sync(FULL, s, o);
                             if (lane >= o && sx == s && x > v) v = x;
                         }
-                        const i32 sn = __shfl_down_sync(FULL, s, 1);
-                        if (v && (lane == 31 || sn != s)) atomicMax((unsigned long long*)&A.seghead[s], v);
+                        const i32 s0 = __shfl_sync(FULL, s, 0), s31 = __shfl_sync(FULL, s, 31);
+                        if (s0 == s31) {  // the whole row lies in one segment: keep its maximum in the
+                                          // warp and post one atomic when the segment changes
+                            const u64 v31 = __shfl_sync(FULL, v, 31);
+                            if (carry_v && carry_s != s0) {
+                                if (lane == 0) atomicMax((unsigned long long*)&A.seghead[carry_s], carry_v);
+                                carry_v = 0;
+                            }
+                            carry_s = s0;
+                            if (v31 > carry_v) carry_v = v31;
+                        } else {
+                            if (carry_v) {
+                                if (lane == 0) atomicMax((unsigned long long*)&A.seghead[carry_s], carry_v);
+                                carry_v = 0;
+                            }
+                            const i32 sn = __shfl_down_sync(FULL, s, 1);
+                            if (v && (lane == 31 || sn != s)) atomicMax((unsigned long long*)&A.seghead[s], v);
+                        }
                         n_unres += __popc(__ballot_sync(FULL, un[k]));
                     }
                 }
                 __syncthreads();  // tsm.wv is reused by the next tile
             }
+            if (lane == 0 && carry_v) atomicMax((unsigned long long*)&A.seghead[carry_s], carry_v);
             if (lane == 0 && n_unres) atomicAdd(cnt, n_unres);
         }
         g.sync();
@@ -475,7 +502,9 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                     cmp[k] = un[k] && r[k] != h[k];
                     l[k] = na[k];  // r == h: the head itself
                 }
-                lcp_lockstep<SB, true>(H, ao, na, bo, nb, lo, cmp, l, round == 0);
+                u64 al[SB];
+                SUBS(k) al[k] = un[k] ? __ldcg(A.lasth + r[k]) : 0ull;
+                lcp_lockstep<SB, true>(H, ao, na, bo, nb, lo, cmp, l, round == 0, al);
                 u64 wa[SB], wb[SB];
                 SUBS(k) {
                     wa[k] = wb[k] = 0;
@@ -782,6 +811,7 @@ static void tree_layout(Arena& a, i64 N, int grid, TreeArgs& A) {
     A.bufs.val[1] = a.take<u32>(N);
     A.seg = a.take<u32>(N);
     A.srank = a.take<u32>(N);
+    A.lasth = a.take<u64>(N);
     A.seghead = a.take<u64>(N);
     A.segdepth = a.take<i32>(N);
     A.agg = a.take<i64>(grid);
