@@ -283,3 +283,24 @@ def test_full_size_configs(cfg):
                                       cluster_size=_dev(ot.cluster_size), arrival=_dev(wl.arrival))
     assert np.array_equal(_np(g_dem), oracle.demand(o_h, o_bo, cache.t_keys))
     assert np.array_equal(_np(g_ord), oracle.clpm_order(o_hit, ot.cluster_size, wl.arrival))
+
+
+def test_block_hash_ragged_queue():
+    """peek_block_hash on a ragged queue: every start alignment, empty and sub-block requests, a
+    request ending at the very end of the token pool, lengths around the 32-block chunk; two seeds."""
+    b = _b()
+    rng = np.random.default_rng(21)
+    lens = list(range(0, 200)) + [16 * n + d for n in (4, 5, 8, 31, 32, 33, 64, 65, 100) for d in (0, 1, 15)]
+    lens += [int(x) for x in rng.integers(0, 5000, size=3000)]
+    rng.shuffle(lens)
+    lens.append(16 * 7)  # the last request ends exactly at the pool end, on a block boundary
+    reqs = [rng.integers(-3, 128256, size=n).astype(np.int32) for n in lens]
+    toks, off = _csr(reqs)
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    o_bo2, o_h2 = oracle.block_hash(toks, off, 16, 0x9E3779B97F4A7C15)
+    d_tok, d_off = _dev(toks), _dev(off)
+    g_bo, g_h = b.peek_block_hash(d_tok, d_off, int(o_bo[-1]))
+    assert np.array_equal(_np(g_bo), o_bo)
+    assert np.array_equal(_np(g_h), o_h)
+    g_bo, g_h = b.peek_block_hash(d_tok, d_off, int(o_bo[-1]), seed=0x9E3779B97F4A7C15)
+    assert np.array_equal(_np(g_h), o_h2)
