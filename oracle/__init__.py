@@ -201,3 +201,59 @@ def clpm_order(hit, cluster_size, arrival=None):
     lib().orc_clpm_order(_p(hit, I32), _p(cluster_size, I32), _p(arr, I32),
                          ctypes.c_int64(N), _p(out, I32))
     return out
+
+
+def score(hashes, blk_off, block_size: int = 16):
+    """O6 ancestor score.  int64[N]."""
+    hashes = _c(hashes, np.uint64)
+    if hashes.shape[0] == 0:
+        hashes = np.zeros(1, dtype=np.uint64)
+    blk_off = _c(blk_off, np.int64)
+    N = blk_off.shape[0] - 1
+    out = np.zeros(N, dtype=np.int64)
+    lib().orc_score(_p(hashes, U64), _p(blk_off, I64), ctypes.c_int64(N), ctypes.c_int32(block_size),
+                    _p(out, I64))
+    return out
+
+
+def evict_score(hashes, blk_off, t_keys, block_size: int = 16):
+    """O7 eviction score per table slot (Eq. 2).  int64[S]."""
+    hashes = _c(hashes, np.uint64)
+    if hashes.shape[0] == 0:
+        hashes = np.zeros(1, dtype=np.uint64)
+    blk_off = _c(blk_off, np.int64)
+    t_keys = _c(t_keys, np.uint64)
+    N = blk_off.shape[0] - 1
+    out = np.zeros(t_keys.shape[0], dtype=np.int64)
+    lib().orc_evict_score(_p(hashes, U64), _p(blk_off, I64), ctypes.c_int64(N), ctypes.c_int32(block_size),
+                          _p(t_keys, U64), ctypes.c_int64(t_keys.shape[0]), _p(out, I64))
+    return out
+
+
+def sections(hashes, blk_off, hit, tau: int = 0, arrival=None):
+    """O8 warm / pioneer / sibling (Alg. 2).  int32[N] in {0, 1, 2}."""
+    hashes = _c(hashes, np.uint64)
+    if hashes.shape[0] == 0:
+        hashes = np.zeros(1, dtype=np.uint64)
+    blk_off = _c(blk_off, np.int64)
+    hit = _c(hit, np.int32)
+    arr = None if arrival is None else _c(arrival, np.int32)
+    N = blk_off.shape[0] - 1
+    out = np.zeros(N, dtype=np.int32)
+    lib().orc_sections(_p(hashes, U64), _p(blk_off, I64), ctypes.c_int64(N), _p(hit, I32),
+                       ctypes.c_int32(tau), _p(arr, I32), _p(out, I32))
+    return out
+
+
+def clpm_order_full(section, hit, score_, cluster_size, arrival=None):
+    """O9 the full Eq. 1 key.  int32[N] permutation."""
+    section = _c(section, np.int32)
+    hit = _c(hit, np.int32)
+    score_ = _c(score_, np.int64)
+    cluster_size = _c(cluster_size, np.int32)
+    arr = None if arrival is None else _c(arrival, np.int32)
+    N = hit.shape[0]
+    out = np.zeros(N, dtype=np.int32)
+    lib().orc_clpm_order_full(_p(section, I32), _p(hit, I32), _p(score_, I64), _p(cluster_size, I32),
+                              _p(arr, I32), ctypes.c_int64(N), _p(out, I32))
+    return out

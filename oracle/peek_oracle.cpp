@@ -24,6 +24,10 @@
 //                     paper worked example PAPER.md:55 (sizes 3/3/2), Fig. 6(a)
 //   orc_demand        nested-loop count; root-block demand = N
 //   orc_clpm_order    python sorted() of tuples; worked-example order
+//   orc_score / orc_evict_score / orc_sections / orc_clpm_order_full (NEXT-1 rows)
+//                     token-level brute force on tiny queues (path counts by tuple
+//                     prefixes, Alg. 2's sequential `seen` loop), closed forms on
+//                     planted queues, the worked example's pioneers and siblings
 // No function here is "parity unpinned".
 //
 // Threading: the per-request loops (hash, radix walk, hash probes) carry an
@@ -287,4 +291,97 @@ extern "C" i32 orc_has_sharing(const i32* group_size, i64 N) {
     for (i64 r = 0; r < N; ++r)
         if (group_size[r] >= 2) return 1;
     return 0;
+}
+
+// ===========================================================================
+// Next rows: the full Eq. 1 key and Eq. 2 score.
+// Readings R20-R23 in DESIGN.md.  Trie nodes exist at block granularity (R7), so
+// an edge is one block of B tokens and pending_count of the node reached by
+// block i of request r is the number of pending (request, block) pairs whose
+// chained hash equals k^r_i - the same count orc_demand takes per table slot.
+// ===========================================================================
+static void orc_pending_counts(const u64* hashes, i64 NB, std::unordered_map<u64, i64>& pc) {
+    pc.reserve((size_t)NB);
+    for (i64 x = 0; x < NB; ++x) pc[hashes[x]] += 1;
+}
+
+// O6. Ancestor score: score(r) = sum over the nodes v on r's path of
+// pending_count(v) * |edge(v)|, |edge| = B tokens per block (R20).
+extern "C" void orc_score(const u64* hashes, const i64* blk_off, i64 N, i32 block_size, i64* score) {
+    std::unordered_map<u64, i64> pc;
+    orc_pending_counts(hashes, blk_off[N], pc);
+    for (i64 r = 0; r < N; ++r) {
+        i64 s = 0;
+        for (i64 x = blk_off[r]; x < blk_off[r + 1]; ++x) s += pc[hashes[x]] * block_size;
+        score[r] = s;
+    }
+}
+
+// O7. Eviction score (Eq. 2): for the cached block b,
+// max over the ancestors v of b (b's own node included) of pending_count(v) * depth(v),
+// depth in tokens (R23).  Per table slot; a slot whose key is on no pending chain has no
+// pending ancestor that can be named through the keys-only table and scores 0 (R23).
+extern "C" void orc_evict_score(const u64* hashes, const i64* blk_off, i64 N, i32 block_size,
+                                const u64* t_keys, i64 S, i64* evict) {
+    std::unordered_map<u64, i64> pc;
+    orc_pending_counts(hashes, blk_off[N], pc);
+    std::unordered_map<u64, i64> slot_of;
+    slot_of.reserve((size_t)S);
+    for (i64 p = 0; p < S; ++p) {
+        evict[p] = 0;
+        if (t_keys[p] != ORC_EMPTY) slot_of.emplace(t_keys[p], p);
+    }
+    for (i64 r = 0; r < N; ++r) {
+        i64 best = 0;  // max over blocks 0..i of r's path
+        for (i64 x = blk_off[r]; x < blk_off[r + 1]; ++x) {
+            i64 depth_tokens = (x - blk_off[r] + 1) * block_size;
+            i64 v = pc[hashes[x]] * depth_tokens;
+            if (v > best) best = v;
+            auto it = slot_of.find(hashes[x]);
+            if (it != slot_of.end()) evict[it->second] = best;
+        }
+    }
+}
+
+// O8. Sections (Alg. 2 lines 3-13): in arrival order (ties by
+// request index), warm (0) if h > tau; else pioneer (1) if the prompt's first theta = 32 tokens
+// have not been seen this cycle, else sibling (2).  At block granularity (R22) the first
+// theta tokens are the first two blocks: the prefix key is k_1 for nb >= 2, k_0 for nb == 1
+// (a shorter prompt is a different prefix than any longer one), and a request with no full
+// block is never "seen".
+extern "C" void orc_sections(const u64* hashes, const i64* blk_off, i64 N, const i32* hit, i32 tau,
+                             const i32* arrival, i32* section) {
+    std::vector<i64> by_arrival((size_t)N);
+    for (i64 r = 0; r < N; ++r) by_arrival[(size_t)r] = r;
+    std::stable_sort(by_arrival.begin(), by_arrival.end(), [&](i64 a, i64 b) {
+        i32 aa = arrival ? arrival[a] : (i32)a, ab = arrival ? arrival[b] : (i32)b;
+        return aa < ab;
+    });
+    std::unordered_map<u64, int> seen2, seen1;  // by k_1 (nb >= 2) and by k_0 (nb == 1)
+    for (i64 q = 0; q < N; ++q) {
+        i64 r = by_arrival[(size_t)q];
+        if (hit[r] > tau) { section[r] = 0; continue; }
+        i64 nb = blk_off[r + 1] - blk_off[r];
+        if (nb == 0) { section[r] = 1; continue; }
+        std::unordered_map<u64, int>& seen = nb >= 2 ? seen2 : seen1;
+        u64 p = nb >= 2 ? hashes[blk_off[r] + 1] : hashes[blk_off[r]];
+        if (seen.count(p)) section[r] = 2;
+        else { section[r] = 1; seen[p] = 1; }
+    }
+}
+
+// O9. The full cLPM key of Eq. 1: (section, -h, -score, -|cluster|, arrival),
+// request index last (R14).
+extern "C" void orc_clpm_order_full(const i32* section, const i32* hit, const i64* score,
+                                    const i32* cluster_size, const i32* arrival, i64 N, i32* out) {
+    for (i64 r = 0; r < N; ++r) out[r] = (i32)r;
+    std::sort(out, out + N, [&](i32 a, i32 b) {
+        if (section[a] != section[b]) return section[a] < section[b];
+        if (hit[a] != hit[b]) return hit[a] > hit[b];
+        if (score[a] != score[b]) return score[a] > score[b];
+        if (cluster_size[a] != cluster_size[b]) return cluster_size[a] > cluster_size[b];
+        i32 aa = arrival ? arrival[a] : a, ab = arrival ? arrival[b] : b;
+        if (aa != ab) return aa < ab;
+        return a < b;
+    });
 }

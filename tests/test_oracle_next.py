@@ -1,0 +1,180 @@
+"""Pins of the NEXT-1 oracle functions (ancestor score, Eq. 2 eviction score,
+sections, the full Eq. 1 key) against definitions written at TOKEN level in pure Python -
+tuples of tokens, no hashes - plus closed forms and the paper's worked example."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2607_02525_b200 import workloads as W
+
+B = 16
+
+
+def _csr(seqs):
+    off = np.zeros(len(seqs) + 1, dtype=np.int64)
+    for i, s in enumerate(seqs):
+        off[i + 1] = off[i] + len(s)
+    toks = np.zeros(max(int(off[-1]), 1), dtype=np.int32)
+    for i, s in enumerate(seqs):
+        toks[off[i]:off[i + 1]] = s
+    return toks[:int(off[-1])], off
+
+
+def _hashes(seqs):
+    toks, off = _csr(seqs)
+    return oracle.block_hash(toks, off, B, 0)
+
+
+def _path_count(seqs, prefix):
+    """pending_count of the trie node spelled by `prefix` (a whole number of blocks): the pending
+    requests passing through or ending at it."""
+    n = len(prefix)
+    return sum(1 for s in seqs if len(s) >= n and tuple(s[:n]) == prefix)
+
+
+def bf_score(seqs):
+    """PAPER.md:102 score(r) = sum over r's path of pending_count(v) * |edge(v)|, one B-token edge
+    per block."""
+    out = []
+    for s in seqs:
+        nb = len(s) // B
+        out.append(sum(_path_count(seqs, tuple(s[:B * (i + 1)])) * B for i in range(nb)))
+    return out
+
+
+def bf_evict(seqs, prefix):
+    """Eq. 2 for the cached block spelled by `prefix`: max over its ancestors (itself included) of
+    pending_count * depth in tokens; 0 when no pending request passes through the block."""
+    if _path_count(seqs, prefix) == 0:
+        return 0
+    return max(_path_count(seqs, prefix[:B * (j + 1)]) * B * (j + 1) for j in range(len(prefix) // B))
+
+
+def bf_sections(seqs, hit, tau, arrival):
+    """Alg. 2 lines 3-13 as printed: arrival order, a `seen` set of the first
+    theta = 32 tokens - here the first two full blocks (one if there is only one; a request with no
+    full block is never seen: DESIGN.md R22)."""
+    order = sorted(range(len(seqs)), key=lambda r: (arrival[r], r))
+    seen = set()
+    sec = [None] * len(seqs)
+    for r in order:
+        if hit[r] > tau:
+            sec[r] = 0
+            continue
+        nb = len(seqs[r]) // B
+        if nb == 0:
+            sec[r] = 1
+            continue
+        p = tuple(seqs[r][:B * min(nb, 2)])
+        if p in seen:
+            sec[r] = 2
+        else:
+            sec[r] = 1
+            seen.add(p)
+    return sec
+
+
+def _tiny(rng, n, vocab=3):
+    stems = [rng.integers(0, vocab, size=int(rng.integers(0, 120))).tolist() for _ in range(5)]
+    seqs = []
+    for _ in range(n):
+        st = stems[int(rng.integers(0, 5))]
+        cut = int(rng.integers(0, len(st) + 1))
+        seqs.append(st[:cut] + rng.integers(0, vocab, size=int(rng.integers(0, 40))).tolist())
+    seqs += [list(seqs[0]), list(seqs[1][: len(seqs[1]) // 2]), [], [1] * 5, [1] * 16, [1] * 16, [1] * 17]
+    return seqs
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_bruteforce_next_rows(seed):
+    rng = np.random.default_rng(100 + seed)
+    seqs = _tiny(rng, 60)
+    N = len(seqs)
+    bo, h = _hashes(seqs)
+    # O6 score
+    assert oracle.score(h, bo, B).tolist() == bf_score(seqs)
+    # O7 evict score: a table over the blocks of some cached sequences (half of them pending)
+    cached = [seqs[i] for i in range(0, N, 3)] + [rng.integers(0, 3, size=64).tolist() for _ in range(5)]
+    cbo, ch = _hashes(cached)
+    keys = np.unique(ch)
+    t_keys = W.build_table(keys, 1 << 11)
+    prefix_of = {}
+    for ci, s in enumerate(cached):
+        for i in range(len(s) // B):
+            prefix_of[int(ch[cbo[ci] + i])] = tuple(s[:B * (i + 1)])
+    ev = oracle.evict_score(h, bo, t_keys, B)
+    for p in range(t_keys.shape[0]):
+        k = int(t_keys[p])
+        want = 0 if k == 0xFFFFFFFFFFFFFFFF else bf_evict(seqs, prefix_of[k])
+        assert int(ev[p]) == want, (p, want)
+    # every pending cached block scores at least its own pending_count * depth (the j = i term)
+    dem = oracle.demand(h, bo, t_keys)
+    assert np.all((ev > 0) == (dem > 0))
+    # O8 sections, with hits from an arbitrary (random) hit vector and two thresholds
+    hit = rng.integers(0, 40, size=N).astype(np.int32)
+    arrival = rng.permutation(N).astype(np.int32)
+    arrival[::7] = arrival[0]  # duplicate arrivals: the request index decides
+    for tau in (0, 20):
+        assert oracle.sections(h, bo, hit, tau, arrival).tolist() == bf_sections(seqs, hit, tau, arrival)
+    assert oracle.sections(h, bo, hit, 0, None).tolist() == bf_sections(seqs, hit, 0, list(range(N)))
+    # O9 full key
+    sec = oracle.sections(h, bo, hit, 0, arrival)
+    sc = oracle.score(h, bo, B)
+    cs = oracle.pending_tree(h, bo).cluster_size
+    want = sorted(range(N), key=lambda r: (int(sec[r]), -int(hit[r]), -int(sc[r]), -int(cs[r]), int(arrival[r]), r))
+    assert oracle.clpm_order_full(sec, hit, sc, cs, arrival).tolist() == want
+
+
+def test_closed_forms():
+    """N identical requests of nb blocks: every node on the path has pending_count N, so
+    score = B * N * nb and a cached block at depth i scores N * B * (i + 1); a cold queue of
+    identical prompts has one pioneer (the earliest arrival) and N - 1 siblings."""
+    N, nb = 37, 9
+    base = np.arange(B * nb).tolist()
+    seqs = [list(base) for _ in range(N)]
+    bo, h = _hashes(seqs)
+    assert oracle.score(h, bo, B).tolist() == [B * N * nb] * N
+    t_keys = W.build_table(np.unique(h), 64)
+    ev = oracle.evict_score(h, bo, t_keys, B)
+    chain = [int(x) for x in h[:nb]]
+    for i, k in enumerate(chain):
+        p = int(np.nonzero(t_keys == np.uint64(k))[0][0])
+        assert int(ev[p]) == N * B * (i + 1)
+    arrival = np.arange(N, dtype=np.int32)[::-1].copy()  # the LAST request arrived first
+    sec = oracle.sections(h, bo, np.zeros(N, np.int32), 0, arrival)
+    assert sec.tolist() == [2] * (N - 1) + [1]
+    # a deep lightly shared prefix above a heavily shared one: the max in Eq. 2 picks the ancestor
+    heavy = [np.arange(B).tolist() + [7] * B * 2 + [i] * B for i in range(10)]   # 10 share 3 blocks
+    bo, h = _hashes(heavy)
+    t_keys = W.build_table(np.unique(h), 64)
+    ev = oracle.evict_score(h, bo, t_keys, B)
+    leaf = int(h[bo[0] + 3])  # request 0's own 4th block: count 1 at depth 64 -> ancestor 10 * 48 wins
+    assert int(ev[int(np.nonzero(t_keys == np.uint64(leaf))[0][0])]) == 10 * B * 3
+
+
+def test_worked_example_sections_and_full_key():
+    """PAPER.md:55 queue A1,B1,C1,A2,B2,C2,A3,B3, all cold: the first request of each tenant is the
+    pioneer, the others are siblings, and Eq. 1 admits every pioneer before any
+    sibling; inside a section ties on h fall to the score (tenants of three before the tenant of
+    two), then arrival."""
+    rng = np.random.default_rng(1)
+    pre = {t: rng.integers(0, 1000, size=2048).tolist() for t in "ABC"}
+    names = ["A1", "B1", "C1", "A2", "B2", "C2", "A3", "B3"]
+    reqs = [pre[n[0]] + rng.integers(0, 1000, size=32).tolist() for n in names]
+    bo, h = _hashes(reqs)
+    N = len(reqs)
+    hit = np.zeros(N, np.int32)
+    arrival = np.arange(N, dtype=np.int32)
+    sec = oracle.sections(h, bo, hit, 0, arrival)
+    assert sec.tolist() == [1, 1, 1, 2, 2, 2, 2, 2]
+    sc = oracle.score(h, bo, B)
+    # 128 shared blocks counted by the tenant's size, 2 own blocks counted once
+    assert sc.tolist() == [B * (128 * n + 2) for n in (3, 3, 2, 3, 3, 2, 3, 3)]
+    cs = oracle.pending_tree(h, bo).cluster_size
+    order = oracle.clpm_order_full(sec, hit, sc, cs, arrival)
+    assert [names[i] for i in order] == ["A1", "B1", "C1", "A2", "B2", "A3", "B3", "C2"]
+    # a warm request (h > tau) goes first whatever its cluster
+    hit[5] = 512
+    sec = oracle.sections(h, bo, hit, 0, arrival)
+    assert sec[5] == 0
+    assert names[oracle.clpm_order_full(sec, hit, sc, cs, arrival)[0]] == "C2"
