@@ -11,6 +11,8 @@
  *   peek_lpm           per-request hit length against the engine's prefix cache: a radix cache
  *                      (Alg. 1) and/or a flat block-hash table
  *                      ("per-request find_longest_cache_hit")
+ *   (next rows: peek_clpm_signals - sections, ancestor score, Eq. 2 eviction
+ *    score - and peek_clpm_order_full, the five-part key of Eq. 1; declared further down)
  *   peek_demand_rank   per-cached-block pending demand for the eviction hook (PAPER.md:115-119
  *                      Eq. 2 pending_count; :281 inverted index block_hash -> demand) and the cLPM
  *                      admission order, sub-key (-h, -|cluster|, arrival) of Eq. 1
@@ -67,7 +69,9 @@ enum {
     PEEK_CALL_BLOCK_HASH = 0,
     PEEK_CALL_LPM = 1,
     PEEK_CALL_PENDING_TREE = 2,
-    PEEK_CALL_DEMAND_RANK = 3
+    PEEK_CALL_DEMAND_RANK = 3,
+    PEEK_CALL_CLPM_SIGNALS = 4,
+    PEEK_CALL_CLPM_ORDER_FULL = 5
 };
 /* Bytes of device scratch `call_id` needs for the given sizes [host out].  N requests, T tokens,
  * NB hashed blocks, S table slots, V radix nodes; pass 0 for sizes a call does not use. */
@@ -172,6 +176,34 @@ peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* blk_off, int
                              const peek_table* table /*host struct*/, const int32_t* hit,
                              const int32_t* cluster_size, const int32_t* arrival, int32_t* demand,
                              int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream);
+
+/* ---- a9/a10: the remaining signals of Eq. 1 and Eq. 2 ------------------ */
+/* Read off the pending tree (order, lcp of peek_pending_tree) - DESIGN.md R20-R23.
+ * section     int32[N] OUT by request (NULL to skip; needs hit): 0 warm if hit[r] > tau; else
+ *             1 pioneer if r has the smallest (arrival, index) among the cold requests that share its
+ *             first theta = 32 tokens (= two blocks; one block for a one-block prompt; a request with
+ *             no full block is always a pioneer), else 2 sibling.  Equivalent to the sequential
+ *             `seen` loop of Alg. 2 in arrival order.  arrival NULL => the index.
+ * score       int64[N] OUT by request (NULL to skip): ancestor score of PAPER.md:102,
+ *             16 * sum over the blocks i of r of pending_count(block i of r), pending_count = number
+ *             of pending (request, block) pairs with that chained hash.
+ * evict_score int64[S] OUT (NULL to skip; needs hashes, table): Eq. 2 per table
+ *             slot - for a slot whose key is block i of some pending chain, the maximum over
+ *             j <= i of pending_count(block j) * 16 * (j + 1); 0 for empty slots and for slots on no
+ *             pending chain (zero-demand victims).  Lowest evicts first.
+ * All pointers device; hit, arrival, hashes may be NULL when the outputs that need them are. */
+peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* blk_off, int64_t N,
+                              const int32_t* order, const int32_t* lcp, const int32_t* hit, int32_t tau,
+                              const int32_t* arrival, const peek_table* table /*host struct*/,
+                              int32_t* section, int64_t* score, int64_t* evict_score,
+                              void* ws, int64_t ws_bytes, void* stream);
+
+/* clpm_order int32[N] OUT request indices sorted ascending by the full key of Eq. 1
+ *            (section[r], -hit[r], -score[r], -cluster_size[r], arrival[r], r); arrival NULL => r.
+ * All inputs device arrays by request; all but arrival required. */
+peek_status peek_clpm_order_full(const int32_t* section, const int32_t* hit, const int64_t* score,
+                                 const int32_t* cluster_size, const int32_t* arrival, int64_t N,
+                                 int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream);
 
 /* ---- options: tuning and test hooks ------------------------------------------------------- */
 /* Process-wide, not thread-safe against concurrent calls; results never depend on them.

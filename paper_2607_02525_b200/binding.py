@@ -18,10 +18,12 @@ LIB_PATH = os.path.join(_HERE, "libpeek.so")
 _lib = None
 
 CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
+CALL_CLPM_SIGNALS, CALL_CLPM_ORDER_FULL = 4, 5
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
            "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
-           "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank"]
+           "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
+           "peek_clpm_signals", "peek_clpm_order_full"]
 
 
 class PeekError(RuntimeError):
@@ -71,6 +73,11 @@ def lib():
         L.peek_demand_rank.restype = i32
         L.peek_demand_rank.argtypes = [vp, vp, i64, vp, vp, ctypes.POINTER(_Table), vp, vp, vp, vp, vp,
                                        vp, i64, vp]
+        L.peek_clpm_signals.restype = i32
+        L.peek_clpm_signals.argtypes = [vp, vp, i64, vp, vp, vp, i32, vp, ctypes.POINTER(_Table), vp, vp, vp,
+                                        vp, i64, vp]
+        L.peek_clpm_order_full.restype = i32
+        L.peek_clpm_order_full.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, i64, vp]
         L.peek_bench_random_gather.restype = i32
         L.peek_bench_random_gather.argtypes = [vp, i64, i64, u64, vp, vp]
         _lib = L
@@ -240,6 +247,42 @@ def peek_demand_rank(hashes=None, blk_off=None, tree: Optional[PendingTree] = No
                                 _ptr(arrival), _ptr(demand), _ptr(out), _ptr(ws), nbytes, _stream())
     _check(st, "peek_demand_rank")
     return demand, out
+
+
+def peek_clpm_signals(hashes, blk_off, tree: PendingTree, hit: Optional[torch.Tensor] = None, tau: int = 0,
+                      arrival: Optional[torch.Tensor] = None, t_keys: Optional[torch.Tensor] = None,
+                      want_section: Optional[bool] = None, want_score: bool = True,
+                      want_evict: Optional[bool] = None):
+    """a9.
+    Returns (section int32[N] | None, score int64[N] | None, evict_score int64[S] | None)."""
+    N = int(blk_off.shape[0]) - 1
+    dev = blk_off.device
+    want_section = hit is not None if want_section is None else want_section
+    want_evict = t_keys is not None if want_evict is None else want_evict
+    S = int(t_keys.shape[0]) if t_keys is not None else 0
+    section = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N] if want_section else None
+    score = torch.empty(max(N, 1), dtype=torch.int64, device=dev)[:N] if want_score else None
+    evict = torch.empty(S, dtype=torch.int64, device=dev) if want_evict else None
+    ct = _Table(_ptr(t_keys, U64), S) if t_keys is not None else None
+    ws, nbytes = _ws(CALL_CLPM_SIGNALS, dev, N=N, S=S)
+    st = lib().peek_clpm_signals(_ptr(hashes) if hashes is not None and hashes.numel() else None, _ptr(blk_off), N,
+                                 _ptr(tree.order), _ptr(tree.lcp), _ptr(hit), int(tau), _ptr(arrival),
+                                 ctypes.byref(ct) if ct is not None else None, _ptr(section), _ptr(score),
+                                 _ptr(evict), _ptr(ws), nbytes, _stream())
+    _check(st, "peek_clpm_signals")
+    return section, score, evict
+
+
+def peek_clpm_order_full(section, hit, score, cluster_size, arrival=None):
+    """a10: the five-part key of Eq. 1.  int32[N] permutation."""
+    N = int(hit.shape[0])
+    dev = hit.device
+    out = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N]
+    ws, nbytes = _ws(CALL_CLPM_ORDER_FULL, dev, N=N)
+    st = lib().peek_clpm_order_full(_ptr(section), _ptr(hit), _ptr(score), _ptr(cluster_size), _ptr(arrival), N,
+                                    _ptr(out), _ptr(ws), nbytes, _stream())
+    _check(st, "peek_clpm_order_full")
+    return out
 
 
 OPT_LPM_STRATEGY, OPT_LPM_WINDOW, OPT_GRID_LIMIT = 1, 2, 3

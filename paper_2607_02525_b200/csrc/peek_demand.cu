@@ -13,11 +13,6 @@
 namespace peek {
 
 // ---- demand -----------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_mintree_level(MinTree mt, int k) {
-    i64 gw = ((i64)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    i64 nw = ((i64)gridDim.x * blockDim.x) >> 5;
-    mintree_build_level(mt, k, gw, nw, threadIdx.x & 31);
-}
 
 __device__ __forceinline__ i64 table_slot_from(const u64* __restrict__ t_keys, u64 mask, u64 key, u64 p,
                                               u64 tk) {  // tk = t_keys[p] already loaded
@@ -235,6 +230,111 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
     PEEK_MARK(4);
 }
 
+// ---- the full Eq. 1 key: (section, -h, -score, -|cluster|, arrival), index last ----
+// Five parts, least significant first: arrival, cluster size, score, hit, section.  Their ranges
+// are measured, consecutive parts are packed greedily into 64-bit keys, and every pack is one
+// stable pair sort on top of the previous order (config 5: 20 + 5 + 35 bits, then 15 + 2 bits).
+struct FullCtl {
+    u32 bar, pad;
+    unsigned long long mx[5], mn[5];  // max of the image, max of its complement (= ~min)
+};
+struct FullArgs {
+    const i32 *section, *hit, *csize, *arrival;
+    const i64* score;
+    i64 N;
+    i32* out;
+    FullCtl* ctl;
+    GsBufs bufs;
+};
+__device__ __forceinline__ u64 full_part(const FullArgs& A, int q, u32 r) {
+    switch (q) {
+        case 0: return A.arrival ? (u64)img_asc(__ldg(A.arrival + r)) : (u64)r;
+        case 1: return (u64)img_desc(__ldg(A.csize + r));
+        case 2: return ~((u64)__ldg(A.score + r) ^ 0x8000000000000000ull);
+        case 3: return (u64)img_desc(__ldg(A.hit + r));
+        default: return (u64)img_asc(__ldg(A.section + r));
+    }
+}
+
+__global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort_full(FullArgs A) {
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    __shared__ GsSmem ssm;
+    __shared__ unsigned long long s_mm[10];
+    const GsStage stg = gs_stage(dyn_smem);
+    const i64 N = A.N;
+    const i64 gtid = (i64)blockIdx.x * GS_THREADS + threadIdx.x, gsize = (i64)gridDim.x * GS_THREADS;
+    Grid g{&A.ctl->bar, 0};
+    {
+        u64 mx[5] = {0, 0, 0, 0, 0}, mn[5] = {0, 0, 0, 0, 0};
+        for (i64 r = gtid; r < N; r += gsize) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+                const u64 v = full_part(A, q, (u32)r);
+                mx[q] = v > mx[q] ? v : mx[q];
+                mn[q] = ~v > mn[q] ? ~v : mn[q];
+            }
+        }
+        if (threadIdx.x < 10) s_mm[threadIdx.x] = 0;
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+            atomicMax(&s_mm[q], (unsigned long long)mx[q]);
+            atomicMax(&s_mm[5 + q], (unsigned long long)mn[q]);
+        }
+        __syncthreads();
+        if (threadIdx.x < 5) atomicMax(&A.ctl->mx[threadIdx.x], s_mm[threadIdx.x]);
+        else if (threadIdx.x < 10) atomicMax(&A.ctl->mn[threadIdx.x - 5], s_mm[threadIdx.x]);
+    }
+    g.sync();
+    u64 lo[5];
+    int bits[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+        lo[q] = ~__ldcg(&A.ctl->mn[q]);
+        const u64 span = __ldcg(&A.ctl->mx[q]) - lo[q];
+        bits[q] = span == 0 ? 0 : bits_for(span);  // a constant part takes no key bits
+    }
+    int src = -1;  // buffer holding the current order; -1: the identity
+    int q0 = 0;
+    while (q0 < 5) {
+        int q1 = q0, total = 0;
+        while (q1 < 5 && total + bits[q1] <= 64) { total += bits[q1]; ++q1; }
+        // parts q0 .. q1-1 form this sort's key, part q0 in the low bits
+        auto make_key = [&](u32 r) -> u64 {
+            u64 key = 0;
+            int sh = 0;
+            for (int q = q0; q < q1; ++q) {
+                if (bits[q]) { key |= (full_part(A, q, r) - lo[q]) << sh; sh += bits[q]; }
+            }
+            return key;
+        };
+        const u64 vary = total >= 64 ? ~0ull : ((1ull << total) - 1ull);
+        if (src < 0) {
+            src = grid_sort_pairs_gen(A.bufs, N, vary, g, ssm, stg, [&](i64 i, u64& k, u32& v) {
+                v = (u32)i;
+                k = make_key((u32)i);
+            });
+        } else if (vary) {
+            for (i64 j = gtid; j < N; j += gsize) A.bufs.key[src][j] = make_key(__ldcg(&A.bufs.val[src][j]));
+            g.sync();
+            src = grid_sort_pairs(A.bufs, N, vary, g, ssm, stg, src);
+            g.sync();
+        }
+        q0 = q1;
+    }
+    const u32* res = A.bufs.val[src];
+    for (i64 j = gtid; j < N; j += gsize) A.out[j] = (i32)__ldcg(res + j);
+}
+
+static void full_layout(Arena& a, i64 N, int grid, FullArgs& A) {
+    A.ctl = a.take<FullCtl>(1);
+    A.bufs.hist = a.take<u32>(gs_hist_words(grid));  // directly after ctl: one memset clears both
+    A.bufs.key[0] = a.take<u64>(N);
+    A.bufs.key[1] = a.take<u64>(N);
+    A.bufs.val[0] = a.take<u32>(N);
+    A.bufs.val[1] = a.take<u32>(N);
+}
+
 static void rank_layout(Arena& a, i64 N, int grid, RankArgs& A) {
     A.ctl = a.take<RankCtl>(1);
     A.bufs.hist = a.take<u32>(gs_hist_words(grid));  // directly after ctl: one memset clears both
@@ -245,6 +345,13 @@ static void rank_layout(Arena& a, i64 N, int grid, RankArgs& A) {
 }
 
 static constexpr int RANK_MAX_GRID = 1024;  // workspace sizing bound on the cooperative grid
+
+i64 clpm_order_full_ws_bytes(i64 N) {
+    Arena a(nullptr);
+    FullArgs A;
+    full_layout(a, N, 1024, A);
+    return a.used;
+}
 
 i64 demand_rank_ws_bytes(i64 N, i64 S) {
     (void)S;
@@ -293,12 +400,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
         MinTree mt;
         mintree_layout(mt, lcp, N, mt_buf);
         Prof pr(PROF_DEMAND, st, mt.levels);
-        for (int k = 1; k < mt.levels; ++k) {
-            i64 warps = mt.n[k];
-            unsigned grid = (unsigned)((warps * 32 + 255) / 256);
-            if (grid > 148u * 8u) grid = 148u * 8u;
-            k_mintree_level<<<grid, 256, 0, st>>>(mt, k);
-        }
+        mintree_build(mt, st);
         unsigned grid = (unsigned)(((N + 31) / 32 * 32 + DM_THREADS - 1) / DM_THREADS);
         k_demand<<<grid, DM_THREADS, 0, st>>>(hashes, blk_off, N, order, lcp, mt, table->t_keys,
                                       (u64)(table->S - 1), demand);
@@ -321,6 +423,42 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
                                               GS_STAGE_BYTES, st));
     }
     PEEK_CUDA(cudaGetLastError());
+    return PEEK_OK;
+}
+
+extern "C" peek_status peek_clpm_order_full(const int32_t* section, const int32_t* hit, const int64_t* score,
+                                            const int32_t* cluster_size, const int32_t* arrival, int64_t N,
+                                            int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream) {
+    if (N < 0 || N >= 0x7fffffffLL) { set_error("peek_clpm_order_full: N out of range"); return PEEK_ERR_INVALID_ARG; }
+    if (N == 0) return PEEK_OK;
+    if (!section || !hit || !score || !cluster_size || !clpm_order) {
+        set_error("peek_clpm_order_full: NULL argument");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < clpm_order_full_ws_bytes(N)) {
+        set_error("peek_clpm_order_full: workspace NULL, misaligned or too small");
+        return PEEK_ERR_WORKSPACE;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    Arena a(ws);
+    FullArgs A;
+    full_layout(a, N, 1024, A);
+    A.section = section; A.hit = hit; A.score = score; A.csize = cluster_size; A.arrival = arrival;
+    A.N = N; A.out = clpm_order;
+    int grid = persistent_ctas();
+    if (grid > 1024) grid = 1024;
+    i64 want = (N + GS_THREADS - 1) / GS_THREADS;
+    if (want < grid) grid = (int)(want < 1 ? 1 : want);
+    PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(1024)) - (char*)A.ctl), st));
+    static bool attr_set = false;
+    if (!attr_set) {
+        PEEK_CUDA(cudaFuncSetAttribute(k_clpm_sort_full, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
+        attr_set = true;
+    }
+    void* params[] = {&A};
+    Prof pr(PROF_RANK_FULL, st, 1);
+    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort_full, dim3(grid), dim3(GS_THREADS), params,
+                                          GS_STAGE_BYTES, st));
     return PEEK_OK;
 }
 

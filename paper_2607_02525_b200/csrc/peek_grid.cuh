@@ -234,6 +234,22 @@ __device__ __forceinline__ void mintree_build_level(const MinTree& mt, int k, i6
     }
 }
 
+// stand-alone build of all levels (one small launch per level) for the non-persistent kernels;
+// static: every translation unit that includes this header gets its own copy
+static __global__ void __launch_bounds__(256) k_mintree_level(MinTree mt, int k) {
+    i64 gw = ((i64)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    i64 nw = ((i64)gridDim.x * blockDim.x) >> 5;
+    mintree_build_level(mt, k, gw, nw, threadIdx.x & 31);
+}
+static inline void mintree_build(const MinTree& mt, cudaStream_t st) {
+    for (int k = 1; k < mt.levels; ++k) {
+        i64 warps = mt.n[k];
+        unsigned grid = (unsigned)((warps * 32 + 255) / 256);
+        if (grid > 148u * 8u) grid = 148u * 8u;
+        k_mintree_level<<<grid, 256, 0, st>>>(mt, k);
+    }
+}
+
 // largest p <= j with L0x[p] < cd   (requires one to exist, e.g. L0x[0] = 0 < cd)
 __device__ __forceinline__ i64 nsv_prev_less(const MinTree& mt, i64 j, i32 cd) {
     int k = 0;

@@ -98,8 +98,27 @@ def run_pipeline(toks, off, radix, t_keys, arrival, check_tree_free=True):
     if t_keys is not None:
         assert np.array_equal(_np(g_dem), oracle.demand(o_h, o_bo, t_keys))
     assert np.array_equal(_np(g_ord), oracle.clpm_order(hit_np, ot.cluster_size, arrival))
+    check_next_rows(b, g_h, g_bo, gt, o_h, o_bo, ot, hit_np, arrival, t_keys, d_keys)
     torch.cuda.synchronize()
     return dict(N=N, NB=NB)
+
+
+def check_next_rows(b, g_h, g_bo, gt, o_h, o_bo, ot, hit_np, arrival, t_keys, d_keys):
+    """peek_clpm_signals / peek_clpm_order_full against the oracle."""
+    d_hit = _dev(hit_np)
+    d_arr = _dev(arrival) if arrival is not None else None
+    o_score = oracle.score(o_h, o_bo, 16)
+    taus = [0, int(np.median(hit_np))] if hit_np.shape[0] else [0]
+    for tau in taus:
+        g_sec, g_score, g_ev = b.peek_clpm_signals(g_h, g_bo, gt, hit=d_hit, tau=tau, arrival=d_arr, t_keys=d_keys)
+        o_sec = oracle.sections(o_h, o_bo, hit_np, tau, arrival)
+        assert np.array_equal(_np(g_sec), o_sec), "section tau=%d" % tau
+        assert np.array_equal(_np(g_score), o_score), "score"
+        if t_keys is not None:
+            assert np.array_equal(_np(g_ev), oracle.evict_score(o_h, o_bo, t_keys, 16)), "evict_score"
+        g_full = b.peek_clpm_order_full(g_sec, d_hit, g_score, gt.cluster_size, d_arr)
+        assert np.array_equal(_np(g_full), oracle.clpm_order_full(o_sec, hit_np, o_score, ot.cluster_size, arrival)), \
+            "full cLPM order tau=%d" % tau
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
@@ -283,6 +302,7 @@ def test_full_size_configs(cfg):
                                       cluster_size=_dev(ot.cluster_size), arrival=_dev(wl.arrival))
     assert np.array_equal(_np(g_dem), oracle.demand(o_h, o_bo, cache.t_keys))
     assert np.array_equal(_np(g_ord), oracle.clpm_order(o_hit, ot.cluster_size, wl.arrival))
+    check_next_rows(b, g_h, g_bo, gt, o_h, o_bo, ot, o_hit, wl.arrival, cache.t_keys, d_keys)
 
 
 def test_block_hash_ragged_queue():
