@@ -258,6 +258,30 @@ def gather_ceiling(inp, dev):
     return out
 
 
+def next_rows_timing(inp, out):
+    """SURVEY.md 8(f) NEXT-1 calls (sections, ancestor score, Eq. 2 eviction score, five-part Eq. 1
+    key) on the step's outputs: reported beside the step, not part of it."""
+    from paper_2607_02525_b200 import binding as B
+    tree, h, bo, hit = out["tree"], out["h"], out["bo"], out["hit"]
+
+    def timed(fn, n=3):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            r = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n, r
+
+    ms_sig, (sec, sc, ev) = timed(lambda: B.peek_clpm_signals(h, bo, tree, hit=hit, tau=0, arrival=inp.arrival,
+                                                              t_keys=inp.keys))
+    ms_ord, _ = timed(lambda: B.peek_clpm_order_full(sec, hit, sc, tree.cluster_size, inp.arrival))
+    return {"peek_clpm_signals_ms": ms_sig, "peek_clpm_order_full_ms": ms_ord,
+            "sections_warm_pioneer_sibling": torch.bincount(sec, minlength=3).tolist()[:3]}
+
+
 def measured_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -486,7 +510,7 @@ def run_peek(args):
                        "l2": "256 MB buffer written between timed steps; inputs %.1f GB" % (inp.T * 4 / 1e9)},
             "tokens_matched_per_s": world * sum_hit * args.steps / (t_ms * 1e-3),
             "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roofline, "calls": calls,
-            "random_sector_gather_ceiling": ceil}
+            "random_sector_gather_ceiling": ceil, "next_rows": next_rows_timing(inp, out)}
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(inp.wl, inp.cache, args.cpu_seconds)
     print(json.dumps(line), flush=True)

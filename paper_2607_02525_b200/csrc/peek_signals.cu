@@ -176,9 +176,18 @@ __device__ __forceinline__ i64 sg_table_slot(const u64* __restrict__ t_keys, u64
     }
 }
 
-// one warp per sorted position: its steps shallow to deep (the deep-to-shallow walk gives each
-// step; what lies above a step on the position's own range is re-walked - steps per position are
-// few), every cached block of a step gets max(E_in, shallower steps, count * its own depth)
+// A warp owns 32 consecutive sorted positions (the work distribution of k_demand): lane q describes
+// position j0 + q - its chain, the range [l0, nb) of blocks that first appear there, its deepest
+// shared step (blocks [lo1, l1) shared with positions j+1 .. t1-1) and the running maxima that
+// apply above that step and above the unshared tail - then the new blocks of the 32 positions are
+// flattened and handed out one per lane.  The value of a block is max(E_in, own steps down to it);
+// blocks of shallower nested steps take a per-lane walk.
+static constexpr int EV_WARPS = SG_THREADS / 32;
+struct EvictMeta {
+    i64 b0[32], above1[32], above_tail[32];
+    i32 l0[32], l1[32], lo1[32], cnt1[32];
+};
+
 __global__ void __launch_bounds__(SG_THREADS) k_evict_write(const u64* __restrict__ hashes,
                                                            const i64* __restrict__ blk_off, i64 N,
                                                            const i32* __restrict__ order,
@@ -187,29 +196,83 @@ __global__ void __launch_bounds__(SG_THREADS) k_evict_write(const u64* __restric
                                                            const i32* __restrict__ which,
                                                            const u64* __restrict__ t_keys, u64 mask,
                                                            i64* __restrict__ evict) {
-    const int lane = threadIdx.x & 31;
-    const i64 j = ((i64)blockIdx.x * SG_THREADS + threadIdx.x) >> 5;
-    if (j >= N) return;
+    __shared__ EvictMeta sm[EV_WARPS];
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const i64 j0 = (((i64)blockIdx.x * SG_THREADS + threadIdx.x) >> 5) * 32;
+    if (j0 >= N) return;
     const i64* ein = *which ? ein_b : ein_a;
-    const i64 r = order[j];
-    const i64 b0 = blk_off[r], nb = blk_off[r + 1] - b0;
-    const i64 l0 = lcp[j];
-    const i64 e_in = ein[j];
-    for_steps_desc(mt, j, l0, nb - 1, [&](i64 i_lo, i64 i_hi, i64 t) {
-        i64 above = e_in;
-        if (i_lo > l0) {
-            const i64 o = own_max(mt, j, l0, i_lo - 1);
-            if (o > above) above = o;
+    EvictMeta& M = sm[w];
+    const i64 j = j0 + lane;
+    i32 n_new = 0;
+    i64 e_in = 0;
+    {
+        const bool valid = j < N;
+        i64 b0 = 0;
+        i32 nb = 0, l0 = 0, l1 = 0;
+        if (valid) {
+            const i64 r = __ldg(order + j);
+            b0 = __ldg(blk_off + r);
+            nb = (i32)(__ldg(blk_off + r + 1) - b0);
+            l0 = __ldg(lcp + j);
+            l1 = j + 1 < N ? __ldg(lcp + j + 1) : 0;
+            n_new = nb - l0;
+            e_in = ein[j];
         }
-        const i64 c16 = (t - j) * 16;
-        for (i64 i = i_lo + lane; i <= i_hi; i += 32) {
-            const i64 p = sg_table_slot(t_keys, mask, __ldg(hashes + b0 + i));
-            if (p >= 0) {
-                const i64 own = c16 * (i + 1);
-                evict[p] = own > above ? own : above;
-            }
+        i32 lo1 = l1, cnt1 = 1;
+        i64 above1 = e_in, above_tail = e_in;
+        if (valid && l1 > l0) {
+            const i64 t = nsv_next_less(mt, j + 1, l1);
+            const i32 lt = mt.val(0, t);
+            lo1 = lt > l0 ? lt : l0;
+            cnt1 = (i32)(t - j);
+            if (lo1 > l0) { const i64 o = own_max(mt, j, l0, lo1 - 1); if (o > above1) above1 = o; }
+            const i64 v1 = (i64)cnt1 * 16 * l1;  // the deepest shared step's maximum
+            above_tail = v1 > above1 ? v1 : above1;
         }
-    });
+        M.b0[lane] = b0; M.l0[lane] = l0; M.l1[lane] = l1; M.lo1[lane] = lo1; M.cnt1[lane] = cnt1;
+        M.above1[lane] = above1; M.above_tail[lane] = above_tail;
+    }
+    i32 pre = n_new;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const i32 t = __shfl_up_sync(FULL, pre, o);
+        if (lane >= o) pre += t;
+    }
+    const i32 total = __shfl_sync(FULL, pre, 31);
+    const i32 excl = pre - n_new;
+    __syncwarp();
+    for (i32 base = 0; base < total; base += 32) {
+        const i32 it = base + lane;
+        const bool act = it < total;
+        const i32 itc = act ? it : total - 1;
+        int lo = 0, hi = 31;  // first position q with pre[q] > itc
+#pragma unroll
+        for (int s = 0; s < 5; ++s) {
+            const int mid = (lo + hi) >> 1;
+            const i32 v = __shfl_sync(FULL, pre, mid);
+            if (v > itc) hi = mid; else lo = mid + 1;
+        }
+        const int q = lo;
+        const i32 i = M.l0[q] + (itc - __shfl_sync(FULL, excl, q));
+        const u64 key = __ldg(hashes + M.b0[q] + i);
+        const i64 eq = __shfl_sync(FULL, e_in, q);
+        i64 val;
+        if (i >= M.l1[q]) {
+            const i64 own = (i64)16 * (i + 1);
+            val = own > M.above_tail[q] ? own : M.above_tail[q];
+        } else if (i >= M.lo1[q]) {
+            const i64 own = (i64)M.cnt1[q] * 16 * (i + 1);
+            val = own > M.above1[q] ? own : M.above1[q];
+        } else {
+            const i64 own = own_max(mt, j0 + q, M.l0[q], i);
+            val = own > eq ? own : eq;
+        }
+        if (act) {
+            const i64 p = sg_table_slot(t_keys, mask, key);
+            if (p >= 0) evict[p] = val;
+        }
+    }
 }
 
 // ---- sections ------------------------------------------------------------------------------------
@@ -337,7 +400,7 @@ extern "C" peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* 
         i64 n = N;
         void* params[] = {&n, &W.par[0], &W.ein[0], &W.par[1], &W.ein[1], &W.ctl, &W.which};
         PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_evict_jump, dim3(jgrid), dim3(1024), params, 0, st));
-        const unsigned wgrid = (unsigned)((N * 32 + SG_THREADS - 1) / SG_THREADS);
+        const unsigned wgrid = (unsigned)(((N + 31) / 32 * 32 + SG_THREADS - 1) / SG_THREADS);
         k_evict_write<<<wgrid, SG_THREADS, 0, st>>>(hashes, blk_off, N, order, lcp, mt, W.ein[0], W.ein[1], W.which,
                                                    table->t_keys, (u64)(table->S - 1), evict_score);
     }
