@@ -330,15 +330,21 @@ def oracle_pass(wl, cache, n_sample: int):
 
 
 def cpu_baseline(wl, cache, budget_s: float):
+    """The oracle as it stands on a bounded prefix of the workload sized for about budget_s seconds
+    of CPU work.  The pass has a fixed part (the demand map over the whole table) and a part
+    linear in the requests; the sample is grown from the measured marginal cost."""
     import oracle
-    n = min(wl.N, 2048)
-    dt = oracle_pass(wl, cache, n)
-    # scale the sample to the time budget (the fixed cost of the demand map does not scale)
-    if wl.N > n:
-        n2 = int(min(wl.N, max(n, n * budget_s / max(dt, 1e-3) * 0.5)))
-        if n2 > n:
-            n = n2
-            dt = oracle_pass(wl, cache, n)
+    n1 = min(wl.N, 2048)
+    t1 = oracle_pass(wl, cache, n1)
+    n, dt = n1, t1
+    if wl.N > n1:
+        n2 = int(min(wl.N, max(n1 * 4, n1 * budget_s / max(t1, 1e-3) * 0.25)))
+        t2 = oracle_pass(wl, cache, n2)
+        n, dt = n2, t2
+        marginal = max((t2 - t1) / max(n2 - n1, 1), 1e-9)
+        n3 = int(min(wl.N, n2 + max(0.0, budget_s - t2) / marginal * 0.8))
+        if n3 > n2 * 1.5 and t2 < 0.5 * budget_s:
+            n, dt = n3, oracle_pass(wl, cache, n3)
     return {"value": n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
             "sample": "first %d of %d requests of the same workload, same cache, one pass of "
                       "hash+tree+lpm(radix,hash)+demand+rank in %.2f s" % (n, wl.N, dt)}
