@@ -257,3 +257,13 @@ def clpm_order_full(section, hit, score_, cluster_size, arrival=None):
     lib().orc_clpm_order_full(_p(section, I32), _p(hit, I32), _p(score_, I64), _p(cluster_size, I32),
                               _p(arr, I32), ctypes.c_int64(N), _p(out, I32))
     return out
+
+
+def group_major(lane_order, cluster_id):
+    """O10 group-major admission order (worked example PAPER.md:55).  int32[N]."""
+    lane_order = _c(lane_order, np.int32)
+    cluster_id = _c(cluster_id, np.int64)
+    N = lane_order.shape[0]
+    out = np.zeros(N, dtype=np.int32)
+    lib().orc_group_major(_p(lane_order, I32), _p(cluster_id, I64), ctypes.c_int64(N), _p(out, I32))
+    return out

@@ -385,3 +385,24 @@ extern "C" void orc_clpm_order_full(const i32* section, const i32* hit, const i6
         return a < b;
     });
 }
+
+// O10. Group-major admission ("emits all members of one cluster contiguously";
+// worked example PAPER.md:55).  Reading R24: walking the cache-locality lane (Eq. 1 order), the
+// first member of a cluster pulls the rest of its cluster right behind it, in lane order; i.e.
+// requests are ordered by (lane position of their cluster's first member, own lane position).
+// A singleton is its own cluster (its cluster_id is unique).
+extern "C" void orc_group_major(const i32* lane_order, const i64* cluster_id, i64 N, i32* out) {
+    std::vector<i64> pos((size_t)N);
+    for (i64 p = 0; p < N; ++p) pos[(size_t)lane_order[p]] = p;
+    std::unordered_map<i64, i64> first;
+    for (i64 p = 0; p < N; ++p) {
+        i64 c = cluster_id[lane_order[p]];
+        if (!first.count(c)) first[c] = p;
+    }
+    for (i64 r = 0; r < N; ++r) out[r] = (i32)r;
+    std::sort(out, out + N, [&](i32 a, i32 b) {
+        i64 fa = first[cluster_id[a]], fb = first[cluster_id[b]];
+        if (fa != fb) return fa < fb;
+        return pos[(size_t)a] < pos[(size_t)b];
+    });
+}

@@ -178,3 +178,43 @@ def test_worked_example_sections_and_full_key():
     sec = oracle.sections(h, bo, hit, 0, arrival)
     assert sec[5] == 0
     assert names[oracle.clpm_order_full(sec, hit, sc, cs, arrival)[0]] == "C2"
+
+
+def test_group_major_reproduces_the_papers_printed_order():
+    """"PEEK reorders the queue by cluster via the pending tree to
+    A1, A2, A3, B1, B2, B3, C1, C2" - the one admission order the paper prints."""
+    rng = np.random.default_rng(1)
+    pre = {t: rng.integers(0, 1000, size=2048).tolist() for t in "ABC"}
+    names = ["A1", "B1", "C1", "A2", "B2", "C2", "A3", "B3"]
+    reqs = [pre[n[0]] + rng.integers(0, 1000, size=32).tolist() for n in names]
+    bo, h = _hashes(reqs)
+    N = len(reqs)
+    hit = np.zeros(N, np.int32)
+    arrival = np.arange(N, dtype=np.int32)
+    tr = oracle.pending_tree(h, bo)
+    sec = oracle.sections(h, bo, hit, 0, arrival)
+    lane_a = oracle.clpm_order_full(sec, hit, oracle.score(h, bo, B), tr.cluster_size, arrival)
+    gm = oracle.group_major(lane_a, tr.cluster_id)
+    assert [names[i] for i in gm] == ["A1", "A2", "A3", "B1", "B2", "B3", "C1", "C2"]
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_group_major_definition(seed):
+    """Brute force of the reading: walk the lane; an unseen cluster emits all its members in lane
+    order.  Clusters come out contiguous and the result is a permutation."""
+    rng = np.random.default_rng(300 + seed)
+    seqs = _tiny(rng, 50)
+    N = len(seqs)
+    bo, h = _hashes(seqs)
+    tr = oracle.pending_tree(h, bo)
+    lane = rng.permutation(N).astype(np.int32)
+    want, done = [], set()
+    for r in lane.tolist():
+        c = int(tr.cluster_id[r])
+        if c in done:
+            continue
+        done.add(c)
+        want += [x for x in lane.tolist() if int(tr.cluster_id[x]) == c]
+    got = oracle.group_major(lane, tr.cluster_id).tolist()
+    assert got == want
+    assert sorted(got) == list(range(N))
