@@ -71,7 +71,8 @@ enum {
     PEEK_CALL_PENDING_TREE = 2,
     PEEK_CALL_DEMAND_RANK = 3,
     PEEK_CALL_CLPM_SIGNALS = 4,
-    PEEK_CALL_CLPM_ORDER_FULL = 5
+    PEEK_CALL_CLPM_ORDER_FULL = 5,
+    PEEK_CALL_CLPM_GROUP_MAJOR = 6
 };
 /* Bytes of device scratch `call_id` needs for the given sizes [host out].  N requests, T tokens,
  * NB hashed blocks, S table slots, V radix nodes; pass 0 for sizes a call does not use. */
@@ -204,6 +205,15 @@ peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* blk_off, in
 peek_status peek_clpm_order_full(const int32_t* section, const int32_t* hit, const int64_t* score,
                                  const int32_t* cluster_size, const int32_t* arrival, int64_t N,
                                  int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream);
+
+/* a11 (first part): group-major admission (worked example
+ * PAPER.md:55; R24).
+ * lane_order int32[N] a permutation of the requests (the cache-locality lane: peek_clpm_order_full)
+ * cluster_id int64[N] by request (peek_pending_tree)
+ * gm_order   int32[N] OUT requests ordered by (lane position of the first member of their cluster,
+ *            own lane position): every cluster comes out contiguous, right behind its first member. */
+peek_status peek_clpm_group_major(const int32_t* lane_order, const int64_t* cluster_id, int64_t N,
+                                  int32_t* gm_order, void* ws, int64_t ws_bytes, void* stream);
 
 /* ---- options: tuning and test hooks ------------------------------------------------------- */
 /* Process-wide, not thread-safe against concurrent calls; results never depend on them.

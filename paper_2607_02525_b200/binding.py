@@ -18,12 +18,12 @@ LIB_PATH = os.path.join(_HERE, "libpeek.so")
 _lib = None
 
 CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
-CALL_CLPM_SIGNALS, CALL_CLPM_ORDER_FULL = 4, 5
+CALL_CLPM_SIGNALS, CALL_CLPM_ORDER_FULL, CALL_CLPM_GROUP_MAJOR = 4, 5, 6
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
            "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
-           "peek_clpm_signals", "peek_clpm_order_full"]
+           "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major"]
 
 
 class PeekError(RuntimeError):
@@ -78,6 +78,8 @@ def lib():
                                         vp, i64, vp]
         L.peek_clpm_order_full.restype = i32
         L.peek_clpm_order_full.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, i64, vp]
+        L.peek_clpm_group_major.restype = i32
+        L.peek_clpm_group_major.argtypes = [vp, vp, i64, vp, vp, i64, vp]
         L.peek_bench_random_gather.restype = i32
         L.peek_bench_random_gather.argtypes = [vp, i64, i64, u64, vp, vp]
         _lib = L
@@ -282,6 +284,17 @@ def peek_clpm_order_full(section, hit, score, cluster_size, arrival=None):
     st = lib().peek_clpm_order_full(_ptr(section), _ptr(hit), _ptr(score), _ptr(cluster_size), _ptr(arrival), N,
                                     _ptr(out), _ptr(ws), nbytes, _stream())
     _check(st, "peek_clpm_order_full")
+    return out
+
+
+def peek_clpm_group_major(lane_order, cluster_id):
+    """a11: group-major admission order.  int32[N] permutation."""
+    N = int(lane_order.shape[0])
+    dev = lane_order.device
+    out = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N]
+    ws, nbytes = _ws(CALL_CLPM_GROUP_MAJOR, dev, N=N)
+    st = lib().peek_clpm_group_major(_ptr(lane_order), _ptr(cluster_id), N, _ptr(out), _ptr(ws), nbytes, _stream())
+    _check(st, "peek_clpm_group_major")
     return out
 
 

@@ -73,6 +73,7 @@ i64 pending_tree_ws_bytes(i64 N);
 i64 demand_rank_ws_bytes(i64 N, i64 S);
 i64 clpm_signals_ws_bytes(i64 N);
 i64 clpm_order_full_ws_bytes(i64 N);
+i64 group_major_ws_bytes(i64 N);
 void lpm_set_option(int key, i64 v);
 
 }  // namespace peek
@@ -108,6 +109,7 @@ extern "C" peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t 
         case PEEK_CALL_DEMAND_RANK: *out_bytes = peek::demand_rank_ws_bytes(N, S); break;
         case PEEK_CALL_CLPM_SIGNALS: *out_bytes = peek::clpm_signals_ws_bytes(N); break;
         case PEEK_CALL_CLPM_ORDER_FULL: *out_bytes = peek::clpm_order_full_ws_bytes(N); break;
+        case PEEK_CALL_CLPM_GROUP_MAJOR: *out_bytes = peek::group_major_ws_bytes(N); break;
         default:
             peek::set_error("peek_workspace_bytes: unknown call_id %d", call_id);
             return PEEK_ERR_INVALID_ARG;

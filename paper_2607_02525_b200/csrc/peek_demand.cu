@@ -346,6 +346,79 @@ static void rank_layout(Arena& a, i64 N, int grid, RankArgs& A) {
 
 static constexpr int RANK_MAX_GRID = 1024;  // workspace sizing bound on the cooperative grid
 
+// ---- group-major admission (R24) -----------------------------------------
+// order by (lane position of the cluster's first member, own lane position).  The first member is
+// an atomicMin per cluster through an open-addressed table keyed by cluster_id (clusters nested
+// on the same leftmost leaf differ in depth, so the id, not the leaf, is the key); then one pair sort.
+struct GmCtl { u32 bar, pad; };
+struct GmArgs {
+    const i32* lane;
+    const i64* cluster_id;
+    i64 N;
+    i32* out;
+    GmCtl* ctl;
+    GsBufs bufs;
+    unsigned long long* tkeys;  // H slots, all-ones = empty
+    u32* tfirst;                // H slots
+    u32* slot;                  // N: table slot of the cluster of the request at lane position p
+    u64 hmask;
+};
+
+__global__ void __launch_bounds__(GS_THREADS, 1) k_group_major(GmArgs A) {
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    __shared__ GsSmem ssm;
+    const GsStage stg = gs_stage(dyn_smem);
+    const i64 N = A.N;
+    const i64 gtid = (i64)blockIdx.x * GS_THREADS + threadIdx.x, gsize = (i64)gridDim.x * GS_THREADS;
+    Grid g{&A.ctl->bar, 0};
+    for (i64 p = gtid; p < N; p += gsize) {
+        const u32 r = (u32)__ldg(A.lane + p);
+        const unsigned long long cid = (unsigned long long)__ldg(A.cluster_id + r);
+        u64 h = mix64(cid) & A.hmask;
+        for (;;) {
+            const unsigned long long prev = atomicCAS(A.tkeys + h, ~0ull, cid);
+            if (prev == ~0ull || prev == cid) break;
+            h = (h + 1) & A.hmask;
+        }
+        atomicMin(A.tfirst + h, (u32)p);
+        A.slot[p] = (u32)h;
+    }
+    g.sync();
+    const int nbits = bits_for((u64)(N > 1 ? N - 1 : 1));
+    const int src = grid_sort_pairs_gen(A.bufs, N, nbits >= 32 ? ~0ull : ((1ull << (2 * nbits)) - 1ull), g, ssm, stg,
+                                        [&](i64 p, u64& k, u32& v) {
+        v = (u32)__ldg(A.lane + p);
+        k = ((u64)__ldcg(A.tfirst + __ldcg(A.slot + p)) << nbits) | (u64)p;
+    });
+    const u32* res = A.bufs.val[src];
+    for (i64 j = gtid; j < N; j += gsize) A.out[j] = (i32)__ldcg(res + j);
+}
+
+static i64 gm_table_slots(i64 N) {
+    i64 h = 64;
+    while (h < 2 * N) h <<= 1;
+    return h;
+}
+static void gm_layout(Arena& a, i64 N, int grid, GmArgs& A) {
+    A.ctl = a.take<GmCtl>(1);
+    A.bufs.hist = a.take<u32>(gs_hist_words(grid));  // directly after ctl: one memset clears both
+    A.bufs.key[0] = a.take<u64>(N);
+    A.bufs.key[1] = a.take<u64>(N);
+    A.bufs.val[0] = a.take<u32>(N);
+    A.bufs.val[1] = a.take<u32>(N);
+    const i64 H = gm_table_slots(N);
+    A.tkeys = a.take<unsigned long long>(H);
+    A.tfirst = a.take<u32>(H);  // directly after tkeys: one 0xff memset covers both
+    A.slot = a.take<u32>(N);
+    A.hmask = (u64)(H - 1);
+}
+i64 group_major_ws_bytes(i64 N) {
+    Arena a(nullptr);
+    GmArgs A;
+    gm_layout(a, N, 1024, A);
+    return a.used;
+}
+
 i64 clpm_order_full_ws_bytes(i64 N) {
     Arena a(nullptr);
     FullArgs A;
@@ -458,6 +531,41 @@ extern "C" peek_status peek_clpm_order_full(const int32_t* section, const int32_
     void* params[] = {&A};
     Prof pr(PROF_RANK_FULL, st, 1);
     PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort_full, dim3(grid), dim3(GS_THREADS), params,
+                                          GS_STAGE_BYTES, st));
+    return PEEK_OK;
+}
+
+extern "C" peek_status peek_clpm_group_major(const int32_t* lane_order, const int64_t* cluster_id, int64_t N,
+                                             int32_t* gm_order, void* ws, int64_t ws_bytes, void* stream) {
+    if (N < 0 || N >= 0x7fffffffLL) { set_error("peek_clpm_group_major: N out of range"); return PEEK_ERR_INVALID_ARG; }
+    if (N == 0) return PEEK_OK;
+    if (!lane_order || !cluster_id || !gm_order) {
+        set_error("peek_clpm_group_major: NULL argument");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < group_major_ws_bytes(N)) {
+        set_error("peek_clpm_group_major: workspace NULL, misaligned or too small");
+        return PEEK_ERR_WORKSPACE;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    Arena a(ws);
+    GmArgs A;
+    gm_layout(a, N, 1024, A);
+    A.lane = lane_order; A.cluster_id = cluster_id; A.N = N; A.out = gm_order;
+    int grid = persistent_ctas();
+    if (grid > 1024) grid = 1024;
+    i64 want = (N + GS_THREADS - 1) / GS_THREADS;
+    if (want < grid) grid = (int)(want < 1 ? 1 : want);
+    PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(1024)) - (char*)A.ctl), st));
+    PEEK_CUDA(cudaMemsetAsync(A.tkeys, 0xff, (size_t)((char*)(A.tfirst + (A.hmask + 1)) - (char*)A.tkeys), st));
+    static bool attr_set = false;
+    if (!attr_set) {
+        PEEK_CUDA(cudaFuncSetAttribute(k_group_major, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
+        attr_set = true;
+    }
+    void* params[] = {&A};
+    Prof pr(PROF_RANK_FULL, st, 1);
+    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_group_major, dim3(grid), dim3(GS_THREADS), params,
                                           GS_STAGE_BYTES, st));
     return PEEK_OK;
 }

@@ -119,6 +119,8 @@ def check_next_rows(b, g_h, g_bo, gt, o_h, o_bo, ot, hit_np, arrival, t_keys, d_
         g_full = b.peek_clpm_order_full(g_sec, d_hit, g_score, gt.cluster_size, d_arr)
         assert np.array_equal(_np(g_full), oracle.clpm_order_full(o_sec, hit_np, o_score, ot.cluster_size, arrival)), \
             "full cLPM order tau=%d" % tau
+        g_gm = b.peek_clpm_group_major(g_full, gt.cluster_id)
+        assert np.array_equal(_np(g_gm), oracle.group_major(_np(g_full), ot.cluster_id)), "group-major order"
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
