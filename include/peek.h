@@ -72,7 +72,8 @@ enum {
     PEEK_CALL_DEMAND_RANK = 3,
     PEEK_CALL_CLPM_SIGNALS = 4,
     PEEK_CALL_CLPM_ORDER_FULL = 5,
-    PEEK_CALL_CLPM_GROUP_MAJOR = 6
+    PEEK_CALL_CLPM_GROUP_MAJOR = 6,
+    PEEK_CALL_OFFLINE_PHASE1 = 7
 };
 /* Bytes of device scratch `call_id` needs for the given sizes [host out].  N requests, T tokens,
  * NB hashed blocks, S table slots, V radix nodes; pass 0 for sizes a call does not use. */
@@ -214,6 +215,19 @@ peek_status peek_clpm_order_full(const int32_t* section, const int32_t* hit, con
  *            own lane position): every cluster comes out contiguous, right behind its first member. */
 peek_status peek_clpm_group_major(const int32_t* lane_order, const int64_t* cluster_id, int64_t N,
                                   int32_t* gm_order, void* ws, int64_t ws_bytes, void* stream);
+
+/* a12: PEEK-offline phase 1 (R25).
+ * depth_blocks the trie covers the first depth_blocks blocks of every chain (the paper's D = 128
+ *              tokens = 8), 1..16
+ * order        int32[N] OUT the permutation of the depth-first traversal that emits a node's
+ *              terminators first (ascending request index) and visits children in descending
+ *              subtree request count (ties: smallest request index below)
+ * guards       double[4] OUT (device): duplication (fraction of requests whose whole chain equals an
+ *              earlier request's), coverage (fraction sharing >= 2 blocks = 32 tokens with another),
+ *              mean sharing depth in tokens over the first depth_blocks blocks, and 1.0 if any
+ *              guard fires (duplication > 0.5, coverage < 0.1, depth < 64), else 0.0 */
+peek_status peek_offline_phase1(const uint64_t* hashes, const int64_t* blk_off, int64_t N, int32_t depth_blocks,
+                                int32_t* order, double* guards, void* ws, int64_t ws_bytes, void* stream);
 
 /* ---- options: tuning and test hooks ------------------------------------------------------- */
 /* Process-wide, not thread-safe against concurrent calls; results never depend on them.

@@ -267,3 +267,18 @@ def group_major(lane_order, cluster_id):
     out = np.zeros(N, dtype=np.int32)
     lib().orc_group_major(_p(lane_order, I32), _p(cluster_id, I64), ctypes.c_int64(N), _p(out, I32))
     return out
+
+
+def offline_phase1(hashes, blk_off, depth_blocks: int = 8):
+    """O11 PEEK-offline phase 1.  Returns (order int32[N],
+    guards float64[4] = duplication, coverage, mean sharing depth in tokens, fired)."""
+    hashes = _c(hashes, np.uint64)
+    if hashes.shape[0] == 0:
+        hashes = np.zeros(1, dtype=np.uint64)
+    blk_off = _c(blk_off, np.int64)
+    N = blk_off.shape[0] - 1
+    out = np.zeros(N, dtype=np.int32)
+    guards = np.zeros(4, dtype=np.float64)
+    lib().orc_offline_phase1(_p(hashes, U64), _p(blk_off, I64), ctypes.c_int64(N), ctypes.c_int32(depth_blocks),
+                             _p(out, I32), guards.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    return out, guards

@@ -406,3 +406,88 @@ extern "C" void orc_group_major(const i32* lane_order, const i64* cluster_id, i6
         return pos[(size_t)a] < pos[(size_t)b];
     });
 }
+
+// O11. PEEK-offline phase 1: a prefix trie over the first D = 128 tokens of
+// every prompt (= the first 8 blocks, R7); each node records the requests terminating there and
+// its subtree request count; a depth-first traversal that visits children in DESCENDING
+// subtree-count order emits the permutation.  Reading R25: a node first emits its terminators in
+// ascending request index; children with equal counts go by the smallest request index below them.
+// Guards: duplication = fraction of requests whose whole chain equals that of an
+// earlier request; coverage = fraction of requests sharing >= 32 tokens (2 blocks) with another;
+// depth = mean over the requests of 16 * (leading blocks, of the first `depth_blocks`, shared
+// with another request).  guards[3] = 1 if duplication > 0.5 or coverage < 0.1 or depth < 64.
+namespace {
+struct OffNode {
+    std::unordered_map<u64, int> child;
+    std::vector<i32> term;
+    i64 count = 0;
+    i32 minidx = 0x7fffffff;
+};
+}  // namespace
+extern "C" void orc_offline_phase1(const u64* hashes, const i64* blk_off, i64 N, i32 depth_blocks,
+                                   i32* order, double* guards) {
+    std::vector<OffNode> nodes(1);
+    std::vector<std::vector<int>> path((size_t)N);
+    for (i64 r = 0; r < N; ++r) {
+        int v = 0;
+        nodes[0].count += 1;
+        if ((i32)r < nodes[0].minidx) nodes[0].minidx = (i32)r;
+        i64 L = blk_off[r + 1] - blk_off[r];
+        if (L > depth_blocks) L = depth_blocks;
+        for (i64 i = 0; i < L; ++i) {
+            u64 k = hashes[blk_off[r] + i];
+            auto it = nodes[(size_t)v].child.find(k);
+            int c;
+            if (it == nodes[(size_t)v].child.end()) {
+                c = (int)nodes.size();
+                nodes[(size_t)v].child.emplace(k, c);
+                nodes.emplace_back();
+            } else c = it->second;
+            v = c;
+            nodes[(size_t)v].count += 1;
+            if ((i32)r < nodes[(size_t)v].minidx) nodes[(size_t)v].minidx = (i32)r;
+            path[(size_t)r].push_back(v);
+        }
+        nodes[(size_t)v].term.push_back((i32)r);
+    }
+    i64 out = 0;
+    std::vector<int> stack{0};
+    while (!stack.empty()) {  // explicit stack: children pushed in reverse visiting order
+        int v = stack.back();
+        stack.pop_back();
+        for (i32 r : nodes[(size_t)v].term) order[out++] = r;  // inserted in ascending index
+        std::vector<int> ch;
+        for (auto& kv : nodes[(size_t)v].child) ch.push_back(kv.second);
+        std::sort(ch.begin(), ch.end(), [&](int a, int b) {
+            if (nodes[(size_t)a].count != nodes[(size_t)b].count) return nodes[(size_t)a].count > nodes[(size_t)b].count;
+            return nodes[(size_t)a].minidx < nodes[(size_t)b].minidx;
+        });
+        for (auto it = ch.rbegin(); it != ch.rend(); ++it) stack.push_back(*it);
+    }
+    // guards
+    std::unordered_map<u64, std::vector<i64>> by_last;  // (last hash) -> requests, to find equal chains
+    i64 dup = 0, cov = 0;
+    double depth_sum = 0;
+    std::unordered_map<u64, int> seen_chain;
+    for (i64 r = 0; r < N; ++r) {
+        i64 nb = blk_off[r + 1] - blk_off[r];
+        // whole-chain identity: same length and same words
+        bool is_dup = false;
+        u64 tag = nb ? hashes[blk_off[r + 1] - 1] : 0x1234567ull;
+        for (i64 q : by_last[tag]) {
+            i64 nq = blk_off[q + 1] - blk_off[q];
+            if (nq == nb && std::equal(hashes + blk_off[r], hashes + blk_off[r + 1], hashes + blk_off[q])) { is_dup = true; break; }
+        }
+        by_last[tag].push_back(r);
+        if (is_dup) ++dup;
+        const std::vector<int>& p = path[(size_t)r];
+        if (p.size() >= 2 && nodes[(size_t)p[1]].count >= 2) ++cov;
+        i64 d = 0;
+        while (d < (i64)p.size() && nodes[(size_t)p[(size_t)d]].count >= 2) ++d;
+        depth_sum += 16.0 * (double)d;
+    }
+    guards[0] = N ? (double)dup / (double)N : 0.0;
+    guards[1] = N ? (double)cov / (double)N : 0.0;
+    guards[2] = N ? depth_sum / (double)N : 0.0;
+    guards[3] = (guards[0] > 0.5 || guards[1] < 0.1 || guards[2] < 64.0) ? 1.0 : 0.0;
+}

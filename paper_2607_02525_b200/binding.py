@@ -18,12 +18,12 @@ LIB_PATH = os.path.join(_HERE, "libpeek.so")
 _lib = None
 
 CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
-CALL_CLPM_SIGNALS, CALL_CLPM_ORDER_FULL, CALL_CLPM_GROUP_MAJOR = 4, 5, 6
+CALL_CLPM_SIGNALS, CALL_CLPM_ORDER_FULL, CALL_CLPM_GROUP_MAJOR, CALL_OFFLINE_PHASE1 = 4, 5, 6, 7
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
            "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
-           "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major"]
+           "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1"]
 
 
 class PeekError(RuntimeError):
@@ -80,6 +80,8 @@ def lib():
         L.peek_clpm_order_full.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, i64, vp]
         L.peek_clpm_group_major.restype = i32
         L.peek_clpm_group_major.argtypes = [vp, vp, i64, vp, vp, i64, vp]
+        L.peek_offline_phase1.restype = i32
+        L.peek_offline_phase1.argtypes = [vp, vp, i64, i32, vp, vp, vp, i64, vp]
         L.peek_bench_random_gather.restype = i32
         L.peek_bench_random_gather.argtypes = [vp, i64, i64, u64, vp, vp]
         _lib = L
@@ -296,6 +298,20 @@ def peek_clpm_group_major(lane_order, cluster_id):
     st = lib().peek_clpm_group_major(_ptr(lane_order), _ptr(cluster_id), N, _ptr(out), _ptr(ws), nbytes, _stream())
     _check(st, "peek_clpm_group_major")
     return out
+
+
+def peek_offline_phase1(hashes, blk_off, depth_blocks: int = 8):
+    """a12: PEEK-offline phase 1.  Returns (order int32[N],
+    guards float64[4] on the device: duplication, coverage, mean sharing depth in tokens, fired)."""
+    N = int(blk_off.shape[0]) - 1
+    dev = blk_off.device
+    order = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N]
+    guards = torch.zeros(4, dtype=torch.float64, device=dev)
+    ws, nbytes = _ws(CALL_OFFLINE_PHASE1, dev, N=N)
+    st = lib().peek_offline_phase1(_ptr(hashes) if hashes is not None and hashes.numel() else None, _ptr(blk_off),
+                                   N, int(depth_blocks), _ptr(order), _ptr(guards), _ptr(ws), nbytes, _stream())
+    _check(st, "peek_offline_phase1")
+    return order, guards
 
 
 OPT_LPM_STRATEGY, OPT_LPM_WINDOW, OPT_GRID_LIMIT = 1, 2, 3

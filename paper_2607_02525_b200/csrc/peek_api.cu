@@ -36,7 +36,7 @@ int sm_count() {
 // ---- tracing ---------------------------------------------------------------------------
 static const char* const g_prof_names[PROF_NSLOTS] = {
     "hash.nb_scan", "hash.content", "hash.chain", "tree.persistent", "lpm.radix_walk", "lpm.hash_probe",
-    "lpm.resolve_scan", "demand.count", "rank.clpm_sort", "signals.clpm", "rank.full_key"};
+    "lpm.resolve_scan", "demand.count", "rank.clpm_sort", "signals.clpm", "rank.full_key", "offline.phase1"};
 static constexpr int PROF_RING = 512;
 struct ProfSlotState {
     cudaEvent_t ev[PROF_RING][2];
@@ -74,6 +74,7 @@ i64 demand_rank_ws_bytes(i64 N, i64 S);
 i64 clpm_signals_ws_bytes(i64 N);
 i64 clpm_order_full_ws_bytes(i64 N);
 i64 group_major_ws_bytes(i64 N);
+i64 offline_phase1_ws_bytes(i64 N);
 void lpm_set_option(int key, i64 v);
 
 }  // namespace peek
@@ -110,6 +111,7 @@ extern "C" peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t 
         case PEEK_CALL_CLPM_SIGNALS: *out_bytes = peek::clpm_signals_ws_bytes(N); break;
         case PEEK_CALL_CLPM_ORDER_FULL: *out_bytes = peek::clpm_order_full_ws_bytes(N); break;
         case PEEK_CALL_CLPM_GROUP_MAJOR: *out_bytes = peek::group_major_ws_bytes(N); break;
+        case PEEK_CALL_OFFLINE_PHASE1: *out_bytes = peek::offline_phase1_ws_bytes(N); break;
         default:
             peek::set_error("peek_workspace_bytes: unknown call_id %d", call_id);
             return PEEK_ERR_INVALID_ARG;

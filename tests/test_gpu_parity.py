@@ -121,6 +121,11 @@ def check_next_rows(b, g_h, g_bo, gt, o_h, o_bo, ot, hit_np, arrival, t_keys, d_
             "full cLPM order tau=%d" % tau
         g_gm = b.peek_clpm_group_major(g_full, gt.cluster_id)
         assert np.array_equal(_np(g_gm), oracle.group_major(_np(g_full), ot.cluster_id)), "group-major order"
+    for depth in (8, 3):
+        g_off, g_guards = b.peek_offline_phase1(g_h, g_bo, depth)
+        o_off, o_guards = oracle.offline_phase1(o_h, o_bo, depth)
+        assert np.array_equal(_np(g_off), o_off), "offline phase 1 order depth=%d" % depth
+        assert np.array_equal(g_guards.cpu().numpy(), o_guards), "offline guards depth=%d" % depth
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])

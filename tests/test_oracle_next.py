@@ -218,3 +218,75 @@ def test_group_major_definition(seed):
     got = oracle.group_major(lane, tr.cluster_id).tolist()
     assert got == want
     assert sorted(got) == list(range(N))
+
+
+def bf_offline(seqs, depth_blocks=8):
+    """PAPER.md:572 written with token tuples: trie over the first depth_blocks blocks, DFS with the
+    children of a node in descending subtree count (ties: smallest request index below), the
+    requests ending at a node first."""
+    N = len(seqs)
+    key = [tuple(s[:B * min(len(s) // B, depth_blocks)]) for s in seqs]   # truncated, whole blocks
+
+    def below(prefix):
+        return [r for r in range(N) if key[r][:len(prefix)] == prefix]
+
+    out = []
+
+    def visit(prefix):
+        out.extend(r for r in range(N) if key[r] == prefix)
+        kids = sorted({key[r][:len(prefix) + B] for r in below(prefix) if len(key[r]) > len(prefix)},
+                      key=lambda c: (-len(below(c)), min(below(c))))
+        for c in kids:
+            visit(c)
+
+    visit(())
+    return out
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_offline_phase1_bruteforce(seed):
+    rng = np.random.default_rng(500 + seed)
+    seqs = _tiny(rng, 40)
+    seqs += [list(rng.integers(0, 3, size=200)) for _ in range(6)]
+    for d in (8, 2):
+        bo, h = _hashes(seqs)
+        order, guards = oracle.offline_phase1(h, bo, d)
+        assert order.tolist() == bf_offline(seqs, d)
+    # guards from the definitions
+    N = len(seqs)
+    bo, h = _hashes(seqs)
+    order, guards = oracle.offline_phase1(h, bo, 8)
+    blocks = [tuple(s[:B * (len(s) // B)]) for s in seqs]
+    dup = sum(1 for r in range(N) if any(blocks[q] == blocks[r] for q in range(r)))
+    cov = sum(1 for r in range(N) if len(blocks[r]) >= 2 * B and
+              any(q != r and blocks[q][:2 * B] == blocks[r][:2 * B] for q in range(N)))
+    depth = 0
+    for r in range(N):
+        d = 0
+        while d < min(len(blocks[r]) // B, 8) and any(q != r and blocks[q][:B * (d + 1)] == blocks[r][:B * (d + 1)]
+                                                     for q in range(N)):
+            d += 1
+        depth += B * d
+    assert abs(guards[0] - dup / N) < 1e-12 and abs(guards[1] - cov / N) < 1e-12 and abs(guards[2] - depth / N) < 1e-9
+
+
+def test_offline_phase1_worked_example_and_guards():
+    """The tenants of PAPER.md:55 share their first 128 tokens, so phase 1 emits the tenants in
+    descending size (ties by first request): the printed A1,A2,A3,B1,B2,B3,C1,C2.  A queue of
+    unrelated prompts trips the coverage guard; a queue of exact duplicates the duplication guard."""
+    rng = np.random.default_rng(1)
+    pre = {t: rng.integers(0, 1000, size=2048).tolist() for t in "ABC"}
+    names = ["A1", "B1", "C1", "A2", "B2", "C2", "A3", "B3"]
+    reqs = [pre[n[0]] + rng.integers(0, 1000, size=32).tolist() for n in names]
+    bo, h = _hashes(reqs)
+    order, guards = oracle.offline_phase1(h, bo, 8)
+    assert [names[i] for i in order] == ["A1", "A2", "A3", "B1", "B2", "B3", "C1", "C2"]
+    assert guards.tolist() == [0.0, 1.0, 128.0, 0.0]
+    lonely = [rng.integers(0, 1000, size=300).tolist() for _ in range(20)]
+    bo, h = _hashes(lonely)
+    order, guards = oracle.offline_phase1(h, bo, 8)
+    assert order.tolist() == list(range(20)) and guards[1] == 0.0 and guards[3] == 1.0
+    same = [list(lonely[0]) for _ in range(10)]
+    bo, h = _hashes(same)
+    order, guards = oracle.offline_phase1(h, bo, 8)
+    assert guards[0] == 0.9 and guards[3] == 1.0
