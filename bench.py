@@ -277,8 +277,12 @@ def next_rows_timing(inp, out):
 
     ms_sig, (sec, sc, ev) = timed(lambda: B.peek_clpm_signals(h, bo, tree, hit=hit, tau=0, arrival=inp.arrival,
                                                               t_keys=inp.keys))
-    ms_ord, _ = timed(lambda: B.peek_clpm_order_full(sec, hit, sc, tree.cluster_size, inp.arrival))
+    ms_ord, lane = timed(lambda: B.peek_clpm_order_full(sec, hit, sc, tree.cluster_size, inp.arrival))
+    ms_gm, _ = timed(lambda: B.peek_clpm_group_major(lane, tree.cluster_id))
+    ms_off, (_, guards) = timed(lambda: B.peek_offline_phase1(h, bo, 8))
     return {"peek_clpm_signals_ms": ms_sig, "peek_clpm_order_full_ms": ms_ord,
+            "peek_clpm_group_major_ms": ms_gm, "peek_offline_phase1_ms": ms_off,
+            "offline_guards_dup_cov_depth_fired": guards.cpu().tolist(),
             "sections_warm_pioneer_sibling": torch.bincount(sec, minlength=3).tolist()[:3]}
 
 
