@@ -282,3 +282,22 @@ def offline_phase1(hashes, blk_off, depth_blocks: int = 8):
     lib().orc_offline_phase1(_p(hashes, U64), _p(blk_off, I64), ctypes.c_int64(N), ctypes.c_int32(depth_blocks),
                              _p(out, I32), guards.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
     return out, guards
+
+
+def radix_demand(tokens, tok_off, radix: Radix):
+    """O12 per-radix-node pending demand (R26).  int32[V], node 0 (root) = N."""
+    tokens = _c(tokens, np.int32)
+    if tokens.shape[0] == 0:
+        tokens = np.zeros(1, dtype=np.int32)
+    tok_off = _c(tok_off, np.int64)
+    N = tok_off.shape[0] - 1
+    V = radix.n_tok_len.shape[0]
+    out = np.zeros(V, dtype=np.int32)
+    e_first = radix.e_first_tok if radix.e_first_tok.shape[0] else np.zeros(1, np.int32)
+    e_child = radix.e_child if radix.e_child.shape[0] else np.zeros(1, np.int32)
+    c_tok = radix.c_tokens if radix.c_tokens.shape[0] else np.zeros(1, np.int32)
+    lib().orc_radix_demand(_p(tokens, I32), _p(tok_off, I64), ctypes.c_int64(N), _p(_c(c_tok, np.int32), I32),
+                           _p(_c(radix.n_tok_off, np.int64), I64), _p(_c(radix.n_tok_len, np.int32), I32),
+                           _p(_c(radix.n_child_off, np.int32), I32), _p(_c(e_first, np.int32), I32),
+                           _p(_c(e_child, np.int32), I32), ctypes.c_int32(V), _p(out, I32))
+    return out

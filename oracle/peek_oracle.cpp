@@ -491,3 +491,35 @@ extern "C" void orc_offline_phase1(const u64* hashes, const i64* blk_off, i64 N,
     guards[2] = N ? depth_sum / (double)N : 0.0;
     guards[3] = (guards[0] > 0.5 || guards[1] < 0.1 || guards[2] < 64.0) ? 1.0 : 0.0;
 }
+
+// O12. Per-radix-node pending demand (the SGLang-side counterpart of the
+// block_hash -> demand index, "PeekDemandStrategy scores candidate nodes").
+// Reading R26: node_demand[v] = number of pending requests whose longest-prefix match enters v
+// (matches at least one token of v's label); the root, whose label is empty, is entered by every
+// request, so node_demand[root] = N.  Same walk as orc_lpm_radix.
+extern "C" void orc_radix_demand(const i32* tokens, const i64* tok_off, i64 N, const i32* c_tokens,
+                                 const i64* n_tok_off, const i32* n_tok_len, const i32* n_child_off,
+                                 const i32* e_first_tok, const i32* e_child, i32 V, i32* node_demand) {
+    for (i32 v = 0; v < V; ++v) node_demand[v] = 0;
+    for (i64 r = 0; r < N; ++r) {
+        const i32* s = tokens + tok_off[r];
+        i64 len = tok_off[r + 1] - tok_off[r];
+        i32 v = 0;
+        i64 d = 0;
+        node_demand[0] += 1;
+        for (;;) {
+            if (d == len) break;
+            i32 u = -1;
+            for (i32 e = n_child_off[v]; e < n_child_off[v + 1]; ++e)
+                if (e_first_tok[e] == s[d]) { u = e_child[e]; break; }
+            if (u < 0) break;
+            node_demand[u] += 1;  // the first token of the edge matched: u is entered
+            const i32* lab = c_tokens + n_tok_off[u];
+            i64 L = n_tok_len[u], m = 0;
+            while (m < L && d + m < len && lab[m] == s[d + m]) ++m;
+            d += m;
+            if (m < L) break;
+            v = u;
+        }
+    }
+}

@@ -290,3 +290,56 @@ def test_offline_phase1_worked_example_and_guards():
     bo, h = _hashes(same)
     order, guards = oracle.offline_phase1(h, bo, 8)
     assert guards[0] == 0.9 and guards[3] == 1.0
+
+
+def _radix_of(seqs):
+    toks, off = _csr(seqs)
+    n = len(seqs)
+    pcs = W.Pieces(np.ascontiguousarray(toks), off[:-1].copy(), np.diff(off), np.arange(n + 1, dtype=np.int64))
+    radix, _ = W.build_radix(pcs, B, 0)
+    return radix
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_radix_demand_bruteforce(seed):
+    """node_demand[v] = requests whose LCP with the cached string spelled root -> v goes past the
+    depth at which v starts (R26); the root counts every request."""
+    rng = np.random.default_rng(700 + seed)
+    cached = [s for s in _tiny(rng, 12) if len(s)]
+    reqs = _tiny(rng, 50)
+    radix = _radix_of(cached)
+    orad = oracle.Radix(radix.c_tokens, radix.n_tok_off, radix.n_tok_len, radix.n_child_off,
+                        radix.e_first_tok, radix.e_child)
+    toks, off = _csr(reqs)
+    got = oracle.radix_demand(toks, off, orad)
+    V = radix.n_tok_len.shape[0]
+    # path string and start depth of every node, by a walk over the flattened arrays
+    path = {0: []}
+    stack = [0]
+    while stack:
+        v = stack.pop()
+        for e in range(int(radix.n_child_off[v]), int(radix.n_child_off[v + 1])):
+            u = int(radix.e_child[e])
+            lab = radix.c_tokens[int(radix.n_tok_off[u]): int(radix.n_tok_off[u]) + int(radix.n_tok_len[u])].tolist()
+            path[u] = path[v] + lab
+            stack.append(u)
+    assert len(path) == V
+
+    def lcp(a, b):
+        n = 0
+        for x, y in zip(a, b):
+            if x != y:
+                break
+            n += 1
+        return n
+
+    for v in range(V):
+        start = len(path[v]) - int(radix.n_tok_len[v])
+        want = len(reqs) if v == 0 else sum(1 for r in reqs if lcp(r, path[v]) > start)
+        assert int(got[v]) == want, v
+    assert int(got[0]) == len(reqs)
+    # consistency with the hit lengths: a request enters exactly the nodes above its hit depth
+    hr = oracle.lpm_radix(toks, off, orad)
+    assert int(got.sum()) - len(reqs) == sum(
+        sum(1 for v in range(1, V) if lcp(r, path[v]) > len(path[v]) - int(radix.n_tok_len[v])) for r in reqs)
+    assert all(int(h) <= len(r) for h, r in zip(hr, reqs))
