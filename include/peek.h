@@ -207,6 +207,14 @@ peek_status peek_clpm_order_full(const int32_t* section, const int32_t* hit, con
                                  const int32_t* cluster_size, const int32_t* arrival, int64_t N,
                                  int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream);
 
+/* a9b: per-radix-node pending demand (R26), the radix-cache
+ * counterpart of `demand`: node_demand[v] int32[V] OUT = pending requests whose longest-prefix match
+ * enters node v (matches >= 1 token of its label); node_demand[0] (root) = N.
+ * hit_radix int32[N] must be peek_lpm's radix-mode result for the same queue and cache. */
+peek_status peek_radix_demand(const int32_t* tokens, const int64_t* tok_off, int64_t N,
+                              const peek_radix* radix /*host struct*/, const int32_t* hit_radix,
+                              int32_t* node_demand, void* stream);
+
 /* a11 (first part): group-major admission (worked example
  * PAPER.md:55; R24).
  * lane_order int32[N] a permutation of the requests (the cache-locality lane: peek_clpm_order_full)

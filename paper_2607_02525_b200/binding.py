@@ -23,7 +23,7 @@ EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_worksp
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
            "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
-           "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1"]
+           "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1", "peek_radix_demand"]
 
 
 class PeekError(RuntimeError):
@@ -80,6 +80,8 @@ def lib():
         L.peek_clpm_order_full.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, i64, vp]
         L.peek_clpm_group_major.restype = i32
         L.peek_clpm_group_major.argtypes = [vp, vp, i64, vp, vp, i64, vp]
+        L.peek_radix_demand.restype = i32
+        L.peek_radix_demand.argtypes = [vp, vp, i64, ctypes.POINTER(_Radix), vp, vp, vp]
         L.peek_offline_phase1.restype = i32
         L.peek_offline_phase1.argtypes = [vp, vp, i64, i32, vp, vp, vp, i64, vp]
         L.peek_bench_random_gather.restype = i32
@@ -297,6 +299,18 @@ def peek_clpm_group_major(lane_order, cluster_id):
     ws, nbytes = _ws(CALL_CLPM_GROUP_MAJOR, dev, N=N)
     st = lib().peek_clpm_group_major(_ptr(lane_order), _ptr(cluster_id), N, _ptr(out), _ptr(ws), nbytes, _stream())
     _check(st, "peek_clpm_group_major")
+    return out
+
+
+def peek_radix_demand(tokens, tok_off, radix: Radix, hit_radix):
+    """a9b: per-radix-node pending demand (R26).  int32[V], node 0 = N."""
+    N = int(tok_off.shape[0]) - 1
+    V = int(radix.n_tok_len.shape[0])
+    out = torch.empty(V, dtype=torch.int32, device=tok_off.device)
+    cr = radix._c()
+    st = lib().peek_radix_demand(_ptr(tokens) if tokens is not None and tokens.numel() else None, _ptr(tok_off), N,
+                                 ctypes.byref(cr), _ptr(hit_radix), _ptr(out), _stream())
+    _check(st, "peek_radix_demand")
     return out
 
 

@@ -508,6 +508,32 @@ __global__ void __launch_bounds__(DWH_THREADS) k_lpm_hash_dual(const u64* __rest
     }
 }
 
+// ---- per-radix-node pending demand (R26) ------------------------
+// node_demand[v] = pending requests whose match enters node v.  The hit length is known, so a warp
+// re-descends its request by child lookups only (no label compares) down to depth hit[r] and counts
+// every node on the way; the root (entered by all) is written directly.
+__global__ void __launch_bounds__(LPM_THREADS) k_radix_demand(const i32* __restrict__ tokens,
+                                                             const i64* __restrict__ tok_off, i64 N,
+                                                             RadixDev R, const i32* __restrict__ hit,
+                                                             i32* __restrict__ node_demand) {
+    const int lane = threadIdx.x & 31;
+    const i64 r = ((i64)blockIdx.x * LPM_THREADS + threadIdx.x) >> 5;
+    if (r >= N) return;
+    const i32* __restrict__ s = tokens + tok_off[r];
+    const i64 h = hit[r];
+    i32 v = 0;
+    i64 d = 0;
+    while (d < h) {  // tokens [0, h) are cached: the edge starting with s[d] exists
+        const i32 e = find_child(R.e_first_tok, __ldg(R.n_child_off + v), __ldg(R.n_child_off + v + 1), __ldg(s + d), lane);
+        if (e < 0) break;  // cannot happen for a hit produced by peek_lpm on the same cache
+        const i32 u = __ldg(R.e_child + e);
+        if (lane == 0) atomicAdd(node_demand + u, 1);
+        d += __ldg(R.n_tok_len + u);
+        v = u;
+    }
+}
+__global__ void k_radix_demand_root(i32* node_demand, i32 n) { node_demand[0] = n; }
+
 i64 lpm_ws_bytes(i64 N) {  // speculative path: W per mode and the scan partials
     Arena a(nullptr);
     a.take<i32>(N);
@@ -610,6 +636,33 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
             else k_lpm_hash<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), hit_hash);
         }
         if (spec) resolve(Wh, hit_hash);
+    }
+    PEEK_CUDA(cudaGetLastError());
+    return PEEK_OK;
+}
+
+
+extern "C" peek_status peek_radix_demand(const int32_t* tokens, const int64_t* tok_off, int64_t N,
+                                         const peek_radix* radix, const int32_t* hit_radix,
+                                         int32_t* node_demand, void* stream) {
+    if (N < 0 || N >= 0x7fffffffLL) { set_error("peek_radix_demand: N out of range"); return PEEK_ERR_INVALID_ARG; }
+    if (!radix || radix->V < 1 || !node_demand || !radix->n_child_off || !radix->n_tok_len ||
+        (radix->E > 0 && (!radix->e_first_tok || !radix->e_child))) {
+        set_error("peek_radix_demand: incomplete peek_radix or NULL output");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    if (N > 0 && (!tokens || !tok_off || !hit_radix)) {
+        set_error("peek_radix_demand: NULL argument");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    PEEK_CUDA(cudaMemsetAsync(node_demand, 0, sizeof(i32) * (size_t)radix->V, st));
+    Prof pr(PROF_SIGNALS, st, 2);
+    k_radix_demand_root<<<1, 1, 0, st>>>(node_demand, (i32)N);
+    if (N > 0) {
+        RadixDev R{radix->c_tokens, radix->n_tok_off, radix->n_tok_len, radix->n_child_off, radix->e_first_tok, radix->e_child};
+        const unsigned grid = (unsigned)((N * 32 + LPM_THREADS - 1) / LPM_THREADS);
+        k_radix_demand<<<grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, hit_radix, node_demand);
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;

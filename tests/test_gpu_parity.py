@@ -90,6 +90,10 @@ def run_pipeline(toks, off, radix, t_keys, arrival, check_tree_free=True):
         b.set_option(b.OPT_LPM_STRATEGY, b.LPM_AUTO)
         b.set_option(b.OPT_LPM_WINDOW, 0)
 
+    if radix is not None:  # per-radix-node demand from the (verified) radix hits
+        g_nd = b.peek_radix_demand(d_tok, d_off, d_radix, _dev(o_hr))
+        assert np.array_equal(_np(g_nd), oracle.radix_demand(toks, off, _orc_radix(radix))), "node_demand"
+
     hit_np = o_hr if o_hr is not None else o_hh
     d_hit = _dev(hit_np)
     d_arr = _dev(arrival) if arrival is not None else None
@@ -304,6 +308,8 @@ def test_full_size_configs(cfg, seed):
         # mirrored, prefix-closed table: the two modes agree up to block rounding
         assert np.array_equal(o_hh, 16 * (o_hr // 16))
         o_hit = o_hr
+        g_nd = b.peek_radix_demand(d_tok, d_off, d_radix, g_hr)
+        assert np.array_equal(_np(g_nd), oracle.radix_demand(toks, off, _orc_radix(cache.radix))), "node_demand"
 
     g_dem, g_ord = b.peek_demand_rank(g_h, g_bo, tree=gt, t_keys=d_keys, hit=_dev(o_hit),
                                       cluster_size=_dev(ot.cluster_size), arrival=_dev(wl.arrival))
