@@ -301,3 +301,24 @@ def radix_demand(tokens, tok_off, radix: Radix):
                            _p(_c(radix.n_child_off, np.int32), I32), _p(_c(e_first, np.int32), I32),
                            _p(_c(e_child, np.int32), I32), ctypes.c_int32(V), _p(out, I32))
     return out
+
+
+def lane_b(section, hit, arrival=None):
+    """O13 fairness lane order (Alg. 2 line 18).  int32[N]."""
+    section = _c(section, np.int32)
+    hit = _c(hit, np.int32)
+    arr = None if arrival is None else _c(arrival, np.int32)
+    N = hit.shape[0]
+    out = np.zeros(N, dtype=np.int32)
+    lib().orc_lane_b(_p(section, I32), _p(hit, I32), _p(arr, I32), ctypes.c_int64(N), _p(out, I32))
+    return out
+
+
+def dynamic_lane(cluster_size, age_pressure: float, prev: float):
+    """O14 dynamic-lane controller.  Returns (new 1 - alpha, singleton_frac)."""
+    cluster_size = _c(cluster_size, np.int32)
+    out = np.zeros(2, dtype=np.float64)
+    lib().orc_dynamic_lane(_p(cluster_size, I32), ctypes.c_int64(cluster_size.shape[0]),
+                           ctypes.c_double(age_pressure), ctypes.c_double(prev),
+                           out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    return float(out[0]), float(out[1])

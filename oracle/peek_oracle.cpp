@@ -523,3 +523,35 @@ extern "C" void orc_radix_demand(const i32* tokens, const i64* tok_off, i64 N, c
         }
     }
 }
+
+// O13. Fairness lane (Alg. 2 line 18): R_B = sort by
+// (section, arrival, -h), request index last (R14).
+extern "C" void orc_lane_b(const i32* section, const i32* hit, const i32* arrival, i64 N, i32* out) {
+    for (i64 r = 0; r < N; ++r) out[r] = (i32)r;
+    std::sort(out, out + N, [&](i32 a, i32 b) {
+        if (section[a] != section[b]) return section[a] < section[b];
+        i32 aa = arrival ? arrival[a] : a, ab = arrival ? arrival[b] : b;
+        if (aa != ab) return aa < ab;
+        if (hit[a] != hit[b]) return hit[a] > hit[b];
+        return a < b;
+    });
+}
+
+// O14. Dynamic-lane controller (Alg. 2 line 20):
+// 1 - alpha <- EMA_{beta=0.3}(clamp(0.15 + 0.5*singleton_frac + 0.3*age_pressure, 0.10, 0.60)),
+// singleton_frac = fraction of requests in no cluster (cluster_size == 1).  Reading R27: the EMA is
+// new = beta * x + (1 - beta) * previous, in double precision, each product and sum rounded once.
+extern "C" void orc_dynamic_lane(const i32* cluster_size, i64 N, double age_pressure, double prev,
+                                 double* out) {
+    i64 single = 0;
+    for (i64 r = 0; r < N; ++r) single += cluster_size[r] == 1;
+    volatile double sf = N ? (double)single / (double)N : 0.0;
+    volatile double a = 0.5 * sf, b = 0.3 * age_pressure;
+    volatile double x = 0.15 + a;
+    x = x + b;
+    if (x < 0.10) x = 0.10;
+    if (x > 0.60) x = 0.60;
+    volatile double p = 0.3 * x, q = 0.7 * prev;
+    out[0] = p + q;  // the new fairness share 1 - alpha
+    out[1] = sf;
+}

@@ -343,3 +343,25 @@ def test_radix_demand_bruteforce(seed):
     assert int(got.sum()) - len(reqs) == sum(
         sum(1 for v in range(1, V) if lcp(r, path[v]) > len(path[v]) - int(radix.n_tok_len[v])) for r in reqs)
     assert all(int(h) <= len(r) for h, r in zip(hr, reqs))
+
+
+def test_lane_b_and_dynamic_lane():
+    rng = np.random.default_rng(9)
+    N = 200
+    sec = rng.integers(0, 3, size=N).astype(np.int32)
+    hit = rng.integers(0, 5, size=N).astype(np.int32)
+    arr = rng.integers(0, 40, size=N).astype(np.int32)   # many duplicate arrivals
+    want = sorted(range(N), key=lambda r: (int(sec[r]), int(arr[r]), -int(hit[r]), r))
+    assert oracle.lane_b(sec, hit, arr).tolist() == want
+    assert oracle.lane_b(sec, hit, None).tolist() == sorted(range(N), key=lambda r: (int(sec[r]), r))
+    # the fairness share ramps from 0.15 (cluster dominated) toward 0.60
+    cs = np.full(100, 7, np.int32)
+    new, sf = oracle.dynamic_lane(cs, 0.0, 0.15)
+    assert sf == 0.0 and abs(new - 0.15) < 1e-15            # fixed point of the EMA at the floor
+    cs[:] = 1
+    new, sf = oracle.dynamic_lane(cs, 1.0, 0.60)
+    assert sf == 1.0 and abs(new - 0.60) < 1e-15            # clamp(0.95) = 0.60
+    cs[:50] = 3
+    new, sf = oracle.dynamic_lane(cs, 0.5, 0.3)
+    x = min(max(0.15 + 0.5 * 0.5 + 0.3 * 0.5, 0.10), 0.60)
+    assert sf == 0.5 and abs(new - (0.3 * x + 0.7 * 0.3)) < 1e-15
