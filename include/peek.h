@@ -224,6 +224,21 @@ peek_status peek_radix_demand(const int32_t* tokens, const int64_t* tok_off, int
 peek_status peek_clpm_group_major(const int32_t* lane_order, const int64_t* cluster_id, int64_t N,
                                   int32_t* gm_order, void* ws, int64_t ws_bytes, void* stream);
 
+/* a11b: the fairness lane of Alg. 2 line 18: request indices sorted ascending by
+ * (section[r], arrival[r], -hit[r], r); arrival NULL => r.  Workspace: PEEK_CALL_CLPM_ORDER_FULL. */
+peek_status peek_clpm_lane_b(const int32_t* section, const int32_t* hit, const int32_t* arrival, int64_t N,
+                             int32_t* lane_b_order, void* ws, int64_t ws_bytes, void* stream);
+
+/* a11c: the dynamic-lane controller of PAPER.md:111-113 (Alg. 2 line 20; R27):
+ * out[0] = 0.3 * clamp(0.15 + 0.5 * singleton_frac + 0.3 * age_pressure, 0.10, 0.60)
+ *          + 0.7 * prev_fair_share     (the new fairness share 1 - alpha, double, every product and
+ *          sum rounded once), out[1] = singleton_frac = fraction of requests with cluster_size == 1.
+ * out double[2] device; age_pressure = min(1, oldest singleton wait / 2 s) is the engine's to supply.
+ * Workspace: >= 256 bytes.  The stride interleave of Alg. 2 line 22 is not part of this library: the
+ * paper does not define it beyond its name. */
+peek_status peek_dynamic_lane(const int32_t* cluster_size, int64_t N, double age_pressure,
+                              double prev_fair_share, double* out, void* ws, int64_t ws_bytes, void* stream);
+
 /* a12: PEEK-offline phase 1 (R25).
  * depth_blocks the trie covers the first depth_blocks blocks of every chain (the paper's D = 128
  *              tokens = 8), 1..16

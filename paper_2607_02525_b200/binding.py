@@ -23,7 +23,8 @@ EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_worksp
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
            "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
-           "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1", "peek_radix_demand"]
+           "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1", "peek_radix_demand",
+           "peek_clpm_lane_b", "peek_dynamic_lane"]
 
 
 class PeekError(RuntimeError):
@@ -80,6 +81,10 @@ def lib():
         L.peek_clpm_order_full.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, i64, vp]
         L.peek_clpm_group_major.restype = i32
         L.peek_clpm_group_major.argtypes = [vp, vp, i64, vp, vp, i64, vp]
+        L.peek_clpm_lane_b.restype = i32
+        L.peek_clpm_lane_b.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp]
+        L.peek_dynamic_lane.restype = i32
+        L.peek_dynamic_lane.argtypes = [vp, i64, ctypes.c_double, ctypes.c_double, vp, vp, i64, vp]
         L.peek_radix_demand.restype = i32
         L.peek_radix_demand.argtypes = [vp, vp, i64, ctypes.POINTER(_Radix), vp, vp, vp]
         L.peek_offline_phase1.restype = i32
@@ -299,6 +304,30 @@ def peek_clpm_group_major(lane_order, cluster_id):
     ws, nbytes = _ws(CALL_CLPM_GROUP_MAJOR, dev, N=N)
     st = lib().peek_clpm_group_major(_ptr(lane_order), _ptr(cluster_id), N, _ptr(out), _ptr(ws), nbytes, _stream())
     _check(st, "peek_clpm_group_major")
+    return out
+
+
+def peek_clpm_lane_b(section, hit, arrival=None):
+    """a11b: fairness lane order (Alg. 2 line 18).  int32[N] permutation."""
+    N = int(hit.shape[0])
+    dev = hit.device
+    out = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N]
+    ws, nbytes = _ws(CALL_CLPM_ORDER_FULL, dev, N=N)
+    st = lib().peek_clpm_lane_b(_ptr(section), _ptr(hit), _ptr(arrival), N, _ptr(out), _ptr(ws), nbytes, _stream())
+    _check(st, "peek_clpm_lane_b")
+    return out
+
+
+def peek_dynamic_lane(cluster_size, age_pressure: float, prev_fair_share: float):
+    """a11c: dynamic-lane controller.  float64[2] on the device:
+    (new fairness share 1 - alpha, singleton_frac)."""
+    N = int(cluster_size.shape[0])
+    dev = cluster_size.device
+    out = torch.zeros(2, dtype=torch.float64, device=dev)
+    ws = torch.empty(256, dtype=torch.uint8, device=dev)
+    st = lib().peek_dynamic_lane(_ptr(cluster_size), N, float(age_pressure), float(prev_fair_share), _ptr(out),
+                                 _ptr(ws), 256, _stream())
+    _check(st, "peek_dynamic_lane")
     return out
 
 

@@ -245,9 +245,11 @@ struct FullArgs {
     i32* out;
     FullCtl* ctl;
     GsBufs bufs;
+    int nparts;       // key parts in use, least significant first
+    int part[5];      // which: 0 arrival asc, 1 cluster size desc, 2 score desc, 3 hit desc, 4 section asc
 };
 __device__ __forceinline__ u64 full_part(const FullArgs& A, int q, u32 r) {
-    switch (q) {
+    switch (A.part[q]) {
         case 0: return A.arrival ? (u64)img_asc(__ldg(A.arrival + r)) : (u64)r;
         case 1: return (u64)img_desc(__ldg(A.csize + r));
         case 2: return ~((u64)__ldg(A.score + r) ^ 0x8000000000000000ull);
@@ -269,9 +271,11 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort_full(FullArgs A) {
         for (i64 r = gtid; r < N; r += gsize) {
 #pragma unroll
             for (int q = 0; q < 5; ++q) {
-                const u64 v = full_part(A, q, (u32)r);
-                mx[q] = v > mx[q] ? v : mx[q];
-                mn[q] = ~v > mn[q] ? ~v : mn[q];
+                if (q < A.nparts) {
+                    const u64 v = full_part(A, q, (u32)r);
+                    mx[q] = v > mx[q] ? v : mx[q];
+                    mn[q] = ~v > mn[q] ? ~v : mn[q];
+                }
             }
         }
         if (threadIdx.x < 10) s_mm[threadIdx.x] = 0;
@@ -292,13 +296,14 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort_full(FullArgs A) {
     for (int q = 0; q < 5; ++q) {
         lo[q] = ~__ldcg(&A.ctl->mn[q]);
         const u64 span = __ldcg(&A.ctl->mx[q]) - lo[q];
-        bits[q] = span == 0 ? 0 : bits_for(span);  // a constant part takes no key bits
+        bits[q] = (span == 0 || q >= A.nparts) ? 0 : bits_for(span);  // a constant part takes no key bits
     }
     int src = -1;  // buffer holding the current order; -1: the identity
     int q0 = 0;
-    while (q0 < 5) {
+    const int NP = A.nparts;
+    while (q0 < NP) {
         int q1 = q0, total = 0;
-        while (q1 < 5 && total + bits[q1] <= 64) { total += bits[q1]; ++q1; }
+        while (q1 < NP && total + bits[q1] <= 64) { total += bits[q1]; ++q1; }
         // parts q0 .. q1-1 form this sort's key, part q0 in the low bits
         auto make_key = [&](u32 r) -> u64 {
             u64 key = 0;
@@ -499,25 +504,9 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
     return PEEK_OK;
 }
 
-extern "C" peek_status peek_clpm_order_full(const int32_t* section, const int32_t* hit, const int64_t* score,
-                                            const int32_t* cluster_size, const int32_t* arrival, int64_t N,
-                                            int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream) {
-    if (N < 0 || N >= 0x7fffffffLL) { set_error("peek_clpm_order_full: N out of range"); return PEEK_ERR_INVALID_ARG; }
-    if (N == 0) return PEEK_OK;
-    if (!section || !hit || !score || !cluster_size || !clpm_order) {
-        set_error("peek_clpm_order_full: NULL argument");
-        return PEEK_ERR_INVALID_ARG;
-    }
-    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < clpm_order_full_ws_bytes(N)) {
-        set_error("peek_clpm_order_full: workspace NULL, misaligned or too small");
-        return PEEK_ERR_WORKSPACE;
-    }
-    cudaStream_t st = (cudaStream_t)stream;
+static peek_status launch_sort_full(FullArgs& A, i64 N, void* ws, cudaStream_t st) {
     Arena a(ws);
-    FullArgs A;
     full_layout(a, N, 1024, A);
-    A.section = section; A.hit = hit; A.score = score; A.csize = cluster_size; A.arrival = arrival;
-    A.N = N; A.out = clpm_order;
     int grid = persistent_ctas();
     if (grid > 1024) grid = 1024;
     i64 want = (N + GS_THREADS - 1) / GS_THREADS;
@@ -532,6 +521,80 @@ extern "C" peek_status peek_clpm_order_full(const int32_t* section, const int32_
     Prof pr(PROF_RANK_FULL, st, 1);
     PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort_full, dim3(grid), dim3(GS_THREADS), params,
                                           GS_STAGE_BYTES, st));
+    return PEEK_OK;
+}
+
+extern "C" peek_status peek_clpm_order_full(const int32_t* section, const int32_t* hit, const int64_t* score,
+                                            const int32_t* cluster_size, const int32_t* arrival, int64_t N,
+                                            int32_t* clpm_order, void* ws, int64_t ws_bytes, void* stream) {
+    if (N < 0 || N >= 0x7fffffffLL) { set_error("peek_clpm_order_full: N out of range"); return PEEK_ERR_INVALID_ARG; }
+    if (N == 0) return PEEK_OK;
+    if (!section || !hit || !score || !cluster_size || !clpm_order) {
+        set_error("peek_clpm_order_full: NULL argument");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < clpm_order_full_ws_bytes(N)) {
+        set_error("peek_clpm_order_full: workspace NULL, misaligned or too small");
+        return PEEK_ERR_WORKSPACE;
+    }
+    FullArgs A;
+    A.section = section; A.hit = hit; A.score = score; A.csize = cluster_size; A.arrival = arrival;
+    A.N = N; A.out = clpm_order;
+    A.nparts = 5;
+    for (int q = 0; q < 5; ++q) A.part[q] = q;  // arrival, cluster, score, hit, section
+    return launch_sort_full(A, N, ws, (cudaStream_t)stream);
+}
+
+// fairness lane of Alg. 2 line 18: (section, arrival, -h), index last
+extern "C" peek_status peek_clpm_lane_b(const int32_t* section, const int32_t* hit, const int32_t* arrival,
+                                        int64_t N, int32_t* lane_b_order, void* ws, int64_t ws_bytes, void* stream) {
+    if (N < 0 || N >= 0x7fffffffLL) { set_error("peek_clpm_lane_b: N out of range"); return PEEK_ERR_INVALID_ARG; }
+    if (N == 0) return PEEK_OK;
+    if (!section || !hit || !lane_b_order) { set_error("peek_clpm_lane_b: NULL argument"); return PEEK_ERR_INVALID_ARG; }
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < clpm_order_full_ws_bytes(N)) {
+        set_error("peek_clpm_lane_b: workspace NULL, misaligned or too small");
+        return PEEK_ERR_WORKSPACE;
+    }
+    FullArgs A;
+    A.section = section; A.hit = hit; A.score = nullptr; A.csize = nullptr; A.arrival = arrival;
+    A.N = N; A.out = lane_b_order;
+    A.nparts = 3;
+    A.part[0] = 3; A.part[1] = 0; A.part[2] = 4; A.part[3] = A.part[4] = 0;  // hit desc, arrival, section
+    return launch_sort_full(A, N, ws, (cudaStream_t)stream);
+}
+
+// ---- dynamic-lane controller (Alg. 2 line 20; R27) ---------------------
+__global__ void __launch_bounds__(256) k_count_singletons(const i32* __restrict__ cs, i64 N, unsigned long long* cnt) {
+    u32 c = 0;
+    for (i64 r = (i64)blockIdx.x * 256 + threadIdx.x; r < N; r += (i64)gridDim.x * 256) c += cs[r] == 1;
+    c = __reduce_add_sync(0xffffffffu, c);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(cnt, (unsigned long long)c);
+}
+__global__ void k_dynamic_lane(const unsigned long long* cnt, i64 N, double age, double prev, double* out) {
+    // every product and sum rounded once (no fused multiply-add), as the plain definition does
+    const double sf = N ? __ddiv_rn((double)*cnt, (double)N) : 0.0;
+    double x = __dadd_rn(__dadd_rn(0.15, __dmul_rn(0.5, sf)), __dmul_rn(0.3, age));
+    if (x < 0.10) x = 0.10;
+    if (x > 0.60) x = 0.60;
+    out[0] = __dadd_rn(__dmul_rn(0.3, x), __dmul_rn(0.7, prev));
+    out[1] = sf;
+}
+extern "C" peek_status peek_dynamic_lane(const int32_t* cluster_size, int64_t N, double age_pressure,
+                                         double prev_fair_share, double* out, void* ws, int64_t ws_bytes,
+                                         void* stream) {
+    if (N < 0 || !out || (N > 0 && !cluster_size)) { set_error("peek_dynamic_lane: bad argument"); return PEEK_ERR_INVALID_ARG; }
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < 256) { set_error("peek_dynamic_lane: workspace"); return PEEK_ERR_WORKSPACE; }
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* cnt = (unsigned long long*)ws;
+    PEEK_CUDA(cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), st));
+    Prof pr(PROF_RANK_FULL, st, 2);
+    if (N > 0) {
+        unsigned grid = (unsigned)((N + 255) / 256);
+        if (grid > 148u * 8u) grid = 148u * 8u;
+        k_count_singletons<<<grid, 256, 0, st>>>(cluster_size, N, cnt);
+    }
+    k_dynamic_lane<<<1, 1, 0, st>>>(cnt, N, age_pressure, prev_fair_share, out);
+    PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;
 }
 

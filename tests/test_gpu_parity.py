@@ -123,8 +123,13 @@ def check_next_rows(b, g_h, g_bo, gt, o_h, o_bo, ot, hit_np, arrival, t_keys, d_
         g_full = b.peek_clpm_order_full(g_sec, d_hit, g_score, gt.cluster_size, d_arr)
         assert np.array_equal(_np(g_full), oracle.clpm_order_full(o_sec, hit_np, o_score, ot.cluster_size, arrival)), \
             "full cLPM order tau=%d" % tau
+        g_lb = b.peek_clpm_lane_b(g_sec, d_hit, d_arr)
+        assert np.array_equal(_np(g_lb), oracle.lane_b(o_sec, hit_np, arrival)), "lane B order"
         g_gm = b.peek_clpm_group_major(g_full, gt.cluster_id)
         assert np.array_equal(_np(g_gm), oracle.group_major(_np(g_full), ot.cluster_id)), "group-major order"
+    for age, prev in ((0.0, 0.15), (0.37, 0.3), (1.0, 0.6)):
+        g_dl = b.peek_dynamic_lane(gt.cluster_size, age, prev).cpu().numpy()
+        assert g_dl.tolist() == list(oracle.dynamic_lane(ot.cluster_size, age, prev)), "dynamic lane"
     for depth in (8, 3):
         g_off, g_guards = b.peek_offline_phase1(g_h, g_bo, depth)
         o_off, o_guards = oracle.offline_phase1(o_h, o_bo, depth)
