@@ -742,6 +742,25 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
             else if (go[k]) { if ((i & 31) == 0) { pa[k] = (i >> 5) - 1; lv[k] = 1; } else pa[k] = i - 1; }
             any |= go[k];
         }
+        // Most runs are short: the 32 positions of this warp row, the row before and the row after
+        // sit in three registers per lane, and a lane scans its neighbours with shuffles; only
+        // the searches that leave that window fall through to the walk on the min hierarchy.
+        i32 w_prev = 0, w_cur = 0, w_next = 0;
+        if (SB == 1) {
+            const i64 i = IDX(t, hb * SB);
+            w_cur = i < N ? __ldcg(A.lcp + i) : 0;
+            w_next = i + 32 < N ? __ldcg(A.lcp + i + 32) : 0;
+            w_prev = i >= 32 ? __ldcg(A.lcp + i - 32) : 0;
+            bool g0 = go[0];
+            for (int d = 1; d < 64 && __any_sync(FULL, g0); ++d) {
+                const int idx = lane - d;
+                const i32 x0 = __shfl_sync(FULL, w_cur, idx & 31), xu = __shfl_sync(FULL, w_prev, idx & 31);
+                if (g0 && idx >= -32 && (idx >= 0 ? x0 : xu) < cd[0]) { pa[0] = (i - lane) + idx; g0 = false; }
+            }
+            if (go[0] && g0) { pa[0] = (i - lane) - 33; lv[0] = 0; }  // left the window (index >= 0 then)
+            go[0] = g0;
+            any = g0;
+        }
         while (any) {
             i32 v[SB];
             SUBS(k) v[k] = go[k] ? mt.val(lv[k], pa[k]) : 0;
@@ -768,6 +787,18 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                 if (((i + 1) & 31) == 31 || i + 1 == mt.n[0] - 1) { pb[k] = ((i + 1) >> 5) + 1; lv[k] = 1; } else pb[k] = i + 2;
             }
             any |= go[k];
+        }
+        if (SB == 1) {
+            const i64 i = IDX(t, hb * SB);
+            bool g0 = go[0];
+            for (int d = 1; d < 64 && __any_sync(FULL, g0); ++d) {
+                const int idx = lane + d;
+                const i32 x0 = __shfl_sync(FULL, w_cur, idx & 31), xn = __shfl_sync(FULL, w_next, idx & 31);
+                if (g0 && idx < 64 && (idx < 32 ? x0 : xn) < cd[0]) { pb[0] = (i - lane) + idx; g0 = false; }
+            }
+            if (go[0] && g0) { pb[0] = (i - lane) + 64; lv[0] = 0; }  // left the window (index <= N then)
+            go[0] = g0;
+            any = g0;
         }
         while (any) {
             i32 v[SB];
