@@ -73,7 +73,8 @@ enum {
     PEEK_CALL_CLPM_SIGNALS = 4,
     PEEK_CALL_CLPM_ORDER_FULL = 5,
     PEEK_CALL_CLPM_GROUP_MAJOR = 6,
-    PEEK_CALL_OFFLINE_PHASE1 = 7
+    PEEK_CALL_OFFLINE_PHASE1 = 7,
+    PEEK_CALL_PENDING_TREE_UPDATE = 8 /* pass N = N_new, T = N_old, NB = M */
 };
 /* Bytes of device scratch `call_id` needs for the given sizes [host out].  N requests, T tokens,
  * NB hashed blocks, S table slots, V radix nodes; pass 0 for sizes a call does not use. */
@@ -238,6 +239,22 @@ peek_status peek_clpm_lane_b(const int32_t* section, const int32_t* hit, const i
  * paper does not define it beyond its name. */
 peek_status peek_dynamic_lane(const int32_t* cluster_size, int64_t N, double age_pressure,
                               double prev_fair_share, double* out, void* ws, int64_t ws_bytes, void* stream);
+
+/* a13: incremental maintenance of the pending tree (PAPER.md:21, :94, :287:
+ * the paper inserts and removes requests instead of rebuilding).  The new queue has N_new requests:
+ * the survivors of the old queue, renumbered by `remap`, and M arrivals at indices
+ * N_new - M .. N_new - 1; hashes / blk_off describe the NEW queue (survivors' chains unchanged).
+ * old_order, old_lcp int32[N_old]  the previous result of peek_pending_tree / _update
+ * remap     int32[N_old]           old request index -> new index, -1 = removed; increasing on the
+ *                                  survivors (so that identical chains stay ordered by index)
+ * Outputs as peek_pending_tree, and equal to what it returns on the new queue, without sorting the
+ * survivors again: compaction + the arrivals' own sort + a bisection merge.  Pays off when M << N. */
+peek_status peek_pending_tree_update(const uint64_t* hashes, const int64_t* blk_off, int64_t N_new, int64_t M,
+                                     const int32_t* old_order, const int32_t* old_lcp, int64_t N_old,
+                                     const int32_t* remap, int32_t* order, int32_t* lcp, int32_t* group_id,
+                                     int32_t* group_size, int32_t* cluster_depth, int32_t* cluster_size,
+                                     int64_t* cluster_id, int32_t* n_groups, void* ws, int64_t ws_bytes,
+                                     void* stream);
 
 /* a12: PEEK-offline phase 1 (R25).
  * depth_blocks the trie covers the first depth_blocks blocks of every chain (the paper's D = 128

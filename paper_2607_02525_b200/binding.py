@@ -19,12 +19,13 @@ _lib = None
 
 CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
 CALL_CLPM_SIGNALS, CALL_CLPM_ORDER_FULL, CALL_CLPM_GROUP_MAJOR, CALL_OFFLINE_PHASE1 = 4, 5, 6, 7
+CALL_PENDING_TREE_UPDATE = 8
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
            "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
            "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1", "peek_radix_demand",
-           "peek_clpm_lane_b", "peek_dynamic_lane"]
+           "peek_clpm_lane_b", "peek_dynamic_lane", "peek_pending_tree_update"]
 
 
 class PeekError(RuntimeError):
@@ -81,6 +82,8 @@ def lib():
         L.peek_clpm_order_full.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, i64, vp]
         L.peek_clpm_group_major.restype = i32
         L.peek_clpm_group_major.argtypes = [vp, vp, i64, vp, vp, i64, vp]
+        L.peek_pending_tree_update.restype = i32
+        L.peek_pending_tree_update.argtypes = [vp, vp, i64, i64, vp, vp, i64, vp] + [vp] * 8 + [vp, i64, vp]
         L.peek_clpm_lane_b.restype = i32
         L.peek_clpm_lane_b.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp]
         L.peek_dynamic_lane.restype = i32
@@ -305,6 +308,30 @@ def peek_clpm_group_major(lane_order, cluster_id):
     st = lib().peek_clpm_group_major(_ptr(lane_order), _ptr(cluster_id), N, _ptr(out), _ptr(ws), nbytes, _stream())
     _check(st, "peek_clpm_group_major")
     return out
+
+
+def peek_pending_tree_update(hashes, blk_off, M: int, old: PendingTree, remap, signals: bool = True) -> PendingTree:
+    """a13: incremental maintenance.  hashes / blk_off describe the NEW queue
+    (survivors renumbered by remap, then M arrivals); returns what peek_pending_tree would."""
+    N = int(blk_off.shape[0]) - 1
+    N_old = int(old.order.shape[0])
+    dev = blk_off.device
+    i32 = lambda: torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N]
+    t = PendingTree(i32(), i32(), i32() if signals else None, i32() if signals else None,
+                    i32() if signals else None, i32() if signals else None,
+                    torch.empty(max(N, 1), dtype=torch.int64, device=dev)[:N] if signals else None,
+                    torch.zeros(1, dtype=torch.int32, device=dev) if signals else None)
+    L = lib()
+    nb = ctypes.c_int64(0)
+    _check(L.peek_workspace_bytes(CALL_PENDING_TREE_UPDATE, N, N_old, int(M), 0, 0, ctypes.byref(nb)), "peek_workspace_bytes")
+    ws = torch.empty(max(int(nb.value), 256), dtype=torch.uint8, device=dev)
+    st = L.peek_pending_tree_update(_ptr(hashes) if hashes is not None and hashes.numel() else None, _ptr(blk_off),
+                                    N, int(M), _ptr(old.order), _ptr(old.lcp), N_old, _ptr(remap),
+                                    _ptr(t.order), _ptr(t.lcp), _ptr(t.group_id), _ptr(t.group_size),
+                                    _ptr(t.cluster_depth), _ptr(t.cluster_size), _ptr(t.cluster_id), _ptr(t.n_groups),
+                                    _ptr(ws), int(nb.value), _stream())
+    _check(st, "peek_pending_tree_update")
+    return t
 
 
 def peek_clpm_lane_b(section, hit, arrival=None):

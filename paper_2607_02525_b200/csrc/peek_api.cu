@@ -75,6 +75,7 @@ i64 clpm_signals_ws_bytes(i64 N);
 i64 clpm_order_full_ws_bytes(i64 N);
 i64 group_major_ws_bytes(i64 N);
 i64 offline_phase1_ws_bytes(i64 N);
+i64 pending_tree_update_ws_bytes(i64 N_old, i64 N_new, i64 M);
 void lpm_set_option(int key, i64 v);
 
 }  // namespace peek
@@ -98,7 +99,7 @@ extern "C" int32_t peek_version(void) { return 100; }
 
 extern "C" peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t T, int64_t NB,
                                             int64_t S, int64_t V, int64_t* out_bytes) {
-    (void)T; (void)NB; (void)V;
+    (void)V;
     if (!out_bytes || N < 0 || S < 0) {
         peek::set_error("peek_workspace_bytes: bad argument");
         return PEEK_ERR_INVALID_ARG;
@@ -112,6 +113,10 @@ extern "C" peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t 
         case PEEK_CALL_CLPM_ORDER_FULL: *out_bytes = peek::clpm_order_full_ws_bytes(N); break;
         case PEEK_CALL_CLPM_GROUP_MAJOR: *out_bytes = peek::group_major_ws_bytes(N); break;
         case PEEK_CALL_OFFLINE_PHASE1: *out_bytes = peek::offline_phase1_ws_bytes(N); break;
+        case PEEK_CALL_PENDING_TREE_UPDATE:  // N = N_new, T = N_old, NB = M
+            if (T < 0 || NB < 0) { peek::set_error("peek_workspace_bytes: bad sizes"); return PEEK_ERR_INVALID_ARG; }
+            *out_bytes = peek::pending_tree_update_ws_bytes(T, N, NB);
+            break;
         default:
             peek::set_error("peek_workspace_bytes: unknown call_id %d", call_id);
             return PEEK_ERR_INVALID_ARG;

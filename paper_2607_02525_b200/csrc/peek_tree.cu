@@ -43,6 +43,7 @@ struct TreeArgs {
     i32 *order, *lcp, *group_id, *group_size, *cluster_depth, *cluster_size;
     i64* cluster_id;
     i32* n_groups;
+    int signals_only;  // order and lcp are given: only groups and clusters are computed
     // workspace
     TreeCtl* ctl;
     GsBufs bufs;      // (sort key, request) by position, ping-pong
@@ -256,6 +257,7 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
     auto IDX = [&](int t, int k) -> i64 { return c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane; };
     PEEK_MARK(1);
 
+    if (!A.signals_only) {  // build order + lcp; otherwise they are inputs (peek_pending_tree_update)
     // ---- phase 0: max chain length, identity order ----
     {
         u32 mx = 0;
@@ -578,6 +580,7 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
             }
         }
     }
+    }  // !signals_only
     PEEK_MARK(20);
     const bool want_groups = A.group_id || A.group_size || A.n_groups;
     const bool want_clusters = A.cluster_depth || A.cluster_size || A.cluster_id;
@@ -863,6 +866,35 @@ i64 pending_tree_ws_bytes(i64 N) {
 
 using namespace peek;
 
+// enqueue k_pending_tree (build, or signals only on a given order + lcp); ws holds pending_tree_ws_bytes(N)
+static peek_status tree_launch(const u64* hashes, const i64* blk_off, i64 N, i32* order, i32* lcp,
+                               i32* group_id, i32* group_size, i32* cluster_depth, i32* cluster_size,
+                               i64* cluster_id, i32* n_groups, int signals_only, void* ws, cudaStream_t st) {
+    int grid = persistent_ctas();  // one CTA of GS_THREADS per SM, all co-resident (cooperative launch)
+    if (grid > MAX_GRID) grid = MAX_GRID;
+    i64 want = (N + GS_THREADS - 1) / GS_THREADS;  // no point in more CTAs than work
+    if (want < grid) grid = (int)(want < 1 ? 1 : want);
+    Arena a(ws);
+    TreeArgs A;
+    A.hashes = hashes; A.blk_off = blk_off; A.N = N;
+    A.order = order; A.lcp = lcp; A.group_id = group_id; A.group_size = group_size;
+    A.cluster_depth = cluster_depth; A.cluster_size = cluster_size; A.cluster_id = cluster_id;
+    A.n_groups = n_groups;
+    A.signals_only = signals_only;
+    tree_layout(a, N, MAX_GRID, A);
+    PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(MAX_GRID)) - (char*)A.ctl), st));
+    void* params[] = {&A};
+    Prof pr(PROF_TREE, st, 1);
+    static bool attr_set = false;
+    if (!attr_set) {
+        PEEK_CUDA(cudaFuncSetAttribute(k_pending_tree, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
+        attr_set = true;
+    }
+    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(GS_THREADS), params,
+                                          GS_STAGE_BYTES, st));
+    return PEEK_OK;
+}
+
 extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* blk_off, int64_t N,
                                          int32_t* order, int32_t* lcp, int32_t* group_id,
                                          int32_t* group_size, int32_t* cluster_depth,
@@ -875,28 +907,228 @@ extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* 
         set_error("peek_pending_tree: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;
     }
-    cudaStream_t st = (cudaStream_t)stream;
-    int grid = persistent_ctas();  // one CTA of GS_THREADS per SM, all co-resident (cooperative launch)
-    if (grid > MAX_GRID) grid = MAX_GRID;
-    i64 want = (N + GS_THREADS - 1) / GS_THREADS;  // no point in more CTAs than work
-    if (want < grid) grid = (int)(want < 1 ? 1 : want);
-    Arena a(ws);
-    TreeArgs A;
-    A.hashes = hashes; A.blk_off = blk_off; A.N = N;
-    A.order = order; A.lcp = lcp; A.group_id = group_id; A.group_size = group_size;
-    A.cluster_depth = cluster_depth; A.cluster_size = cluster_size; A.cluster_id = cluster_id;
-    A.n_groups = n_groups;
-    tree_layout(a, N, MAX_GRID, A);
-    PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(MAX_GRID)) - (char*)A.ctl), st));
-    void* params[] = {&A};
-    Prof pr(PROF_TREE, st, 1);
-    static bool attr_set = false;
-    if (!attr_set) {
-        PEEK_CUDA(cudaFuncSetAttribute(k_pending_tree, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
-        attr_set = true;
+    return tree_launch(hashes, blk_off, N, order, lcp, group_id, group_size, cluster_depth, cluster_size,
+                       cluster_id, n_groups, 0, ws, (cudaStream_t)stream);
+}
+
+// ---- a13 peek_pending_tree_update: incremental maintenance -----------------
+// the paper keeps its pending tree incrementally (insert / remove O(D) per
+// request) instead of rebuilding it every cycle.  Here the tree is (order, lcp); a cycle's delta -
+// some requests admitted (removed), M arrivals appended - is applied without sorting the survivors:
+//   1  compaction: the survivors keep their relative order; the LCP across a run of removed
+//      positions is the minimum over the run (an ordered segmented-min scan)
+//   2  the M arrivals are sorted among themselves by the batch build (k_pending_tree on M requests)
+//   3  merge: every arrival bisects for its place among the survivors (chain comparisons by the
+//      depth bisection of chain_lcp) and learns its LCP with both neighbours
+//   4  placement: a prefix sum of the insertion counts shifts the survivors; every adjacent LCP
+//      of the merged order is one of: the compacted LCP, a batch LCP, or a neighbour LCP from 3
+//   5  groups and clusters from the merged (order, lcp): k_pending_tree in signals-only mode
+// The result is by construction what peek_pending_tree returns on the new queue (the parity tests
+// compare it with the oracle's rebuild).
+namespace peek {
+
+struct UpdCtl { u32 bar, pad; i64 S; };
+struct UpdArgs {
+    const u64* hashes;
+    const i64* blk_off;
+    i64 N_old, N_new, M;
+    const i32 *old_order, *old_lcp, *remap;
+    i32 *order, *lcp;
+    UpdCtl* ctl;
+    i32 *s_order, *s_lcp;        // survivors, compacted (<= N_old)
+    const i32 *b_order, *b_lcp;  // the arrivals' own tree (M), local indices
+    i32 *ins, *lcpL, *lcpR;      // per arrival: survivors before it, LCP with the survivor on either side
+    i64* hist;                   // N_old + 1: arrivals inserted directly before survivor p (p = S: at the end)
+    i32* rfix;                   // N_old + 1: LCP of survivor p with the arrival directly before it
+    u64* agg;                    // gridDim scratch of the grid scans
+};
+
+// ordered grid-wide inclusive scan (associative op, NOT necessarily commutative)
+template <typename T, typename Op, typename Load, typename Store>
+__device__ void grid_inscan_ordered(i64 n, Load load, Store store, Op op, T ident, T* agg, T* smem, Grid& g) {
+    const i64 chunk = (((n + gridDim.x - 1) / gridDim.x) + blockDim.x - 1) / blockDim.x * blockDim.x;
+    const i64 c0 = min((i64)blockIdx.x * chunk, n), c1 = min(c0 + chunk, n);
+    T carry = ident;
+    for (i64 b = c0; b < c1; b += blockDim.x) {
+        const i64 i = b + threadIdx.x;
+        T tt;
+        block_inscan(i < c1 ? load(i) : ident, op, ident, smem, &tt);
+        carry = op(carry, tt);
     }
-    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(GS_THREADS), params,
-                                          GS_STAGE_BYTES, st));
+    if (threadIdx.x == 0) agg[blockIdx.x] = carry;
+    g.sync();
+    {   // what the chunks before mine add up to, in order: a contiguous slice of them per thread
+        const int per = ((int)blockIdx.x + (int)blockDim.x - 1) / (int)blockDim.x;
+        T acc = ident;
+        for (int c = (int)threadIdx.x * per; c < min(((int)threadIdx.x + 1) * per, (int)blockIdx.x); ++c) acc = op(acc, agg[c]);
+        block_inscan(acc, op, ident, smem, &carry);
+    }
+    for (i64 b = c0; b < c1; b += blockDim.x) {
+        const i64 i = b + threadIdx.x;
+        T tt;
+        const T inc = block_inscan(i < c1 ? load(i) : ident, op, ident, smem, &tt);
+        if (i < c1) store(i, op(carry, inc));
+        carry = op(carry, tt);
+    }
+    g.sync();
+}
+
+// survivors kept so far | min LCP since the last kept position | "a segment starts here" flag
+__device__ __forceinline__ u64 upd_pack(u32 cnt, u32 mn, u32 flag) { return ((u64)cnt << 32) | ((u64)mn << 1) | flag; }
+__device__ __forceinline__ u64 upd_op(u64 a, u64 b) {
+    const u32 cnt = (u32)(a >> 32) + (u32)(b >> 32);
+    const u32 am = (u32)(a & 0xffffffffu) >> 1, bm = (u32)(b & 0xffffffffu) >> 1;
+    if (b & 1) return ((u64)cnt << 32) | ((u64)bm << 1) | 1u;
+    return ((u64)cnt << 32) | ((u64)(am < bm ? am : bm) << 1) | (a & 1);
+}
+
+// order of an arrival x against a survivor y: -1 x first, +1 y first (ties: the survivor, whose
+// request index is smaller); *l = their LCP in blocks
+__device__ __forceinline__ int upd_cmp(const u64* __restrict__ H, const i64* __restrict__ BO, i64 x, i64 y, i32* l) {
+    const i64 bx = BO[x], nx = BO[x + 1] - bx, by = BO[y], ny = BO[y + 1] - by;
+    const i64 m = chain_lcp(H + bx, nx, H + by, ny, 0);
+    *l = (i32)m;
+    if (m == ny) return 1;   // y is a prefix of x, or equal
+    if (m == nx) return -1;  // x is a proper prefix of y
+    return __ldg(H + bx + m) < __ldg(H + by + m) ? -1 : 1;
+}
+
+static constexpr int UP_THREADS = 512;
+
+__global__ void __launch_bounds__(UP_THREADS) k_tree_update(UpdArgs A) {
+    __shared__ u64 s64[UP_THREADS / 32 + 2];
+    Grid g{&A.ctl->bar, 0};
+    const i64 gtid = (i64)blockIdx.x * UP_THREADS + threadIdx.x, gsize = (i64)gridDim.x * UP_THREADS;
+    const u64* __restrict__ H = A.hashes;
+    const i64* __restrict__ BO = A.blk_off;
+    // ---- 1: compaction of the survivors ----
+    for (i64 p = gtid; p <= A.N_old; p += gsize) { A.hist[p] = 0; A.rfix[p] = -1; }
+    if (gtid == 0) A.ctl->S = 0;
+    {
+        auto keep = [&](i64 j) -> bool { return __ldg(A.remap + __ldg(A.old_order + j)) >= 0; };
+        auto load = [&](i64 j) -> u64 {
+            return upd_pack(keep(j) ? 1u : 0u, (u32)__ldg(A.old_lcp + j), (j == 0 || keep(j - 1)) ? 1u : 0u);
+        };
+        auto store = [&](i64 j, u64 v) {
+            if (keep(j)) {
+                const i64 ps = (i64)(v >> 32) - 1;
+                A.s_order[ps] = __ldg(A.remap + __ldg(A.old_order + j));
+                A.s_lcp[ps] = (i32)((u32)(v & 0xffffffffu) >> 1);
+            }
+            if (j == A.N_old - 1) A.ctl->S = (i64)(v >> 32);
+        };
+        grid_inscan_ordered<u64>(A.N_old, load, store, [](u64 a, u64 b) { return upd_op(a, b); },
+                                 upd_pack(0, 0x7fffffffu, 0), A.agg, s64, g);
+    }
+    const i64 S = A.N_old > 0 ? __ldcg(&A.ctl->S) : 0;
+    // ---- 3: every arrival bisects for its place among the survivors ----
+    const i64 first_new = A.N_new - A.M;
+    for (i64 q = gtid; q < A.M; q += gsize) {
+        const i64 x = first_new + __ldg(A.b_order + q);
+        i64 lo = 0, hi = S;
+        while (lo < hi) {  // survivors before lo sort at or before x, from hi on after x
+            const i64 mid = (lo + hi) >> 1;
+            i32 l;
+            if (upd_cmp(H, BO, x, __ldcg(A.s_order + mid), &l) > 0) lo = mid + 1; else hi = mid;
+        }
+        i32 lL = 0, lR = 0;
+        if (lo > 0) upd_cmp(H, BO, x, __ldcg(A.s_order + lo - 1), &lL);
+        if (lo < S) upd_cmp(H, BO, x, __ldcg(A.s_order + lo), &lR);
+        A.ins[q] = (i32)lo; A.lcpL[q] = lL; A.lcpR[q] = lR;
+        atomicAdd((unsigned long long*)(A.hist + lo), 1ull);
+    }
+    g.sync();
+    // ---- 4: placement ----
+    for (i64 q = gtid; q < A.M; q += gsize) {
+        const i32 in = A.ins[q];
+        const i64 pos = (i64)in + q;
+        A.order[pos] = (i32)(first_new + __ldg(A.b_order + q));
+        A.lcp[pos] = (q > 0 && A.ins[q - 1] == in) ? __ldg(A.b_lcp + q) : A.lcpL[q];
+        if (q == A.M - 1 || A.ins[q + 1] != in) A.rfix[in] = A.lcpR[q];  // the arrival right before survivor `in`
+    }
+    {
+        auto load = [&](i64 p) -> u64 { return (u64)__ldcg(A.hist + p); };
+        auto store = [&](i64 p, u64 inc) {
+            if (p < S) {
+                const i64 pos = p + (i64)inc;
+                A.order[pos] = __ldcg(A.s_order + p);
+                const i32 fix = __ldcg(A.rfix + p);
+                A.lcp[pos] = fix >= 0 ? fix : __ldcg(A.s_lcp + p);
+            }
+        };
+        grid_inscan_ordered<u64>(S + 1, load, store, [](u64 a, u64 b) { return a + b; }, (u64)0, A.agg, s64, g);
+    }
+}
+
+struct UpdWs { UpdArgs A; i32 *b_order, *b_lcp; void* tree_ws; };
+static void update_layout(Arena& a, i64 N_old, i64 N_new, i64 M, UpdWs& W) {
+    UpdArgs& A = W.A;
+    A.ctl = a.take<UpdCtl>(1);
+    A.s_order = a.take<i32>(N_old); A.s_lcp = a.take<i32>(N_old);
+    W.b_order = a.take<i32>(M); W.b_lcp = a.take<i32>(M);
+    A.ins = a.take<i32>(M); A.lcpL = a.take<i32>(M); A.lcpR = a.take<i32>(M);
+    A.hist = a.take<i64>(N_old + 1);
+    A.rfix = a.take<i32>(N_old + 1);
+    A.agg = a.take<u64>(MAX_GRID);
+    W.tree_ws = a.take<char>(pending_tree_ws_bytes(N_new > M ? N_new : M));
+}
+i64 pending_tree_update_ws_bytes(i64 N_old, i64 N_new, i64 M) {
+    Arena a(nullptr);
+    UpdWs W;
+    update_layout(a, N_old, N_new, M, W);
+    return a.used;
+}
+
+}  // namespace peek
+
+using namespace peek;
+
+extern "C" peek_status peek_pending_tree_update(const uint64_t* hashes, const int64_t* blk_off, int64_t N_new,
+                                                int64_t M, const int32_t* old_order, const int32_t* old_lcp,
+                                                int64_t N_old, const int32_t* remap, int32_t* order,
+                                                int32_t* lcp, int32_t* group_id, int32_t* group_size,
+                                                int32_t* cluster_depth, int32_t* cluster_size,
+                                                int64_t* cluster_id, int32_t* n_groups, void* ws,
+                                                int64_t ws_bytes, void* stream) {
+    if (N_new < 0 || N_new >= 0x7fffffffLL || N_old < 0 || N_old >= 0x7fffffffLL || M < 0 || M > N_new) {
+        set_error("peek_pending_tree_update: sizes out of range");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    if (N_new == 0) return PEEK_OK;
+    if (!blk_off || !order || !lcp || (N_old > 0 && (!old_order || !old_lcp || !remap))) {
+        set_error("peek_pending_tree_update: NULL argument");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < pending_tree_update_ws_bytes(N_old, N_new, M)) {
+        set_error("peek_pending_tree_update: workspace NULL, misaligned or too small");
+        return PEEK_ERR_WORKSPACE;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    Arena a(ws);
+    UpdWs W;
+    update_layout(a, N_old, N_new, M, W);
+    if (M > 0) {  // the arrivals' own tree: their chains are requests N_new - M .. N_new - 1
+        peek_status rc = tree_launch(hashes, blk_off + (N_new - M), M, W.b_order, W.b_lcp, nullptr, nullptr,
+                                     nullptr, nullptr, nullptr, nullptr, 0, W.tree_ws, st);
+        if (rc != PEEK_OK) return rc;
+    }
+    UpdArgs& A = W.A;
+    A.hashes = hashes; A.blk_off = blk_off; A.N_old = N_old; A.N_new = N_new; A.M = M;
+    A.old_order = old_order; A.old_lcp = old_lcp; A.remap = remap; A.order = order; A.lcp = lcp;
+    A.b_order = W.b_order; A.b_lcp = W.b_lcp;
+    PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, sizeof(UpdCtl), st));
+    int grid = persistent_ctas();
+    if (grid > MAX_GRID) grid = MAX_GRID;
+    i64 want = ((N_old > M ? N_old : M) + UP_THREADS - 1) / UP_THREADS;
+    if (want < grid) grid = (int)(want < 1 ? 1 : want);
+    {
+        void* params[] = {&A};
+        Prof pr(PROF_TREE, st, 1);
+        PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_tree_update, dim3(grid), dim3(UP_THREADS), params, 0, st));
+    }
+    if (group_id || group_size || n_groups || cluster_depth || cluster_size || cluster_id)
+        return tree_launch(hashes, blk_off, N_new, order, lcp, group_id, group_size, cluster_depth, cluster_size,
+                           cluster_id, n_groups, 1, W.tree_ws, st);
     return PEEK_OK;
 }
 

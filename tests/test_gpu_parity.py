@@ -342,3 +342,89 @@ def test_block_hash_ragged_queue():
     assert np.array_equal(_np(g_h), o_h)
     g_bo, g_h = b.peek_block_hash(d_tok, d_off, int(o_bo[-1]), seed=0x9E3779B97F4A7C15)
     assert np.array_equal(_np(g_h), o_h2)
+
+
+def _update_case(b, old_reqs, keep_mask, arrivals):
+    """old queue -> (remove ~keep_mask, append arrivals) -> peek_pending_tree_update must equal the
+    oracle's rebuild on the new queue, every output."""
+    toks, off = _csr(old_reqs)
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    d_h = _dev(o_h.view(np.int64), torch.uint64) if o_h.shape[0] else torch.zeros(0, dtype=torch.uint64, device=DEV)
+    old = b.peek_pending_tree(d_h, _dev(o_bo)) if len(old_reqs) else b.PendingTree(
+        *[torch.zeros(0, dtype=torch.int32, device=DEV)] * 6, torch.zeros(0, dtype=torch.int64, device=DEV),
+        torch.zeros(1, dtype=torch.int32, device=DEV))
+    survivors = [r for r, k in zip(old_reqs, keep_mask) if k]
+    remap = np.full(len(old_reqs), -1, dtype=np.int32)
+    remap[np.nonzero(keep_mask)[0]] = np.arange(len(survivors), dtype=np.int32)
+    new_reqs = survivors + arrivals
+    ntoks, noff = _csr(new_reqs)
+    n_bo, n_h = oracle.block_hash(ntoks, noff, 16, 0)
+    want = oracle.pending_tree(n_h, n_bo)
+    dn_h = _dev(n_h.view(np.int64), torch.uint64) if n_h.shape[0] else torch.zeros(0, dtype=torch.uint64, device=DEV)
+    d_remap = _dev(remap) if len(old_reqs) else torch.zeros(0, dtype=torch.int32, device=DEV)
+    got = b.peek_pending_tree_update(dn_h, _dev(n_bo), len(arrivals), old, d_remap)
+    for name in ("order", "lcp", "group_id", "group_size", "cluster_depth", "cluster_size", "cluster_id"):
+        assert np.array_equal(_np(getattr(got, name)), getattr(want, name)), name
+    assert int(got.n_groups.item()) == want.n_groups
+    return got
+
+
+def test_pending_tree_update_matches_rebuild():
+    """removals (scattered, in long runs, all, none) and arrivals (new chains,
+    copies of surviving and of removed chains, prefixes and extensions of survivors, empty and
+    sub-block prompts), chained over several cycles."""
+    b = _b()
+    rng = np.random.default_rng(31)
+    reqs, stems = _nested_queue(rng, 6000)
+    N = len(reqs)
+
+    def arrivals(n, pool):
+        out = []
+        for _ in range(n):
+            kind = int(rng.integers(0, 6))
+            base = pool[int(rng.integers(0, len(pool)))]
+            if kind == 0:
+                out.append(base.copy())
+            elif kind == 1:
+                out.append(base[: int(rng.integers(0, len(base) + 1))].copy())
+            elif kind == 2:
+                out.append(np.concatenate([base, rng.integers(0, 4, size=int(rng.integers(1, 60)))]).astype(np.int32))
+            elif kind == 3:
+                out.append(rng.integers(0, 4, size=int(rng.integers(0, 300))).astype(np.int32))
+            elif kind == 4:
+                out.append(np.zeros(int(rng.integers(0, 20)), np.int32))
+            else:
+                s = stems[int(rng.integers(0, len(stems)))]
+                out.append(np.concatenate([s[: int(rng.integers(0, len(s) + 1))], rng.integers(0, 4, size=8)]).astype(np.int32))
+        return out
+
+    keep = rng.random(N) > 0.02
+    _update_case(b, reqs, keep, arrivals(100, reqs))                      # small delta
+    keep = rng.random(N) > 0.5
+    keep[1000:3000] = False                                               # a long run removed
+    _update_case(b, reqs, keep, arrivals(2500, reqs))                     # large delta
+    _update_case(b, reqs, np.zeros(N, bool), arrivals(300, reqs))         # everything removed
+    _update_case(b, reqs, np.ones(N, bool), [])                           # nothing changes
+    _update_case(b, reqs, np.ones(N, bool), arrivals(1, reqs))
+    _update_case(b, [], np.zeros(0, bool), arrivals(500, reqs))           # empty old queue
+    keep = rng.random(N) > 0.3
+    keep[0] = keep[-1] = False
+    _update_case(b, reqs, keep, [])                                       # removals only
+    # several cycles on top of each other, each from the previous UPDATE result
+    cur = reqs
+    toks, off = _csr(cur)
+    bo, h = oracle.block_hash(toks, off, 16, 0)
+    tree = b.peek_pending_tree(_dev(h.view(np.int64), torch.uint64), _dev(bo))
+    for cycle in range(4):
+        keep = rng.random(len(cur)) > 0.1
+        arr = arrivals(400, cur)
+        survivors = [r for r, k in zip(cur, keep) if k]
+        remap = np.full(len(cur), -1, dtype=np.int32)
+        remap[np.nonzero(keep)[0]] = np.arange(len(survivors), dtype=np.int32)
+        cur = survivors + arr
+        toks, off = _csr(cur)
+        bo, h = oracle.block_hash(toks, off, 16, 0)
+        tree = b.peek_pending_tree_update(_dev(h.view(np.int64), torch.uint64), _dev(bo), len(arr), tree, _dev(remap))
+        want = oracle.pending_tree(h, bo)
+        assert np.array_equal(_np(tree.order), want.order) and np.array_equal(_np(tree.lcp), want.lcp), cycle
+        assert np.array_equal(_np(tree.cluster_size), want.cluster_size), cycle
