@@ -90,6 +90,10 @@ __device__ __forceinline__ u32 ld_acquire_u32(const u32* p) {
 // caller's running target (starts at 0, same in every thread).  The gpu-scope fences publish
 // this CTA's writes and drop stale L1 lines before the next phase reads other CTAs' data.
 __device__ __forceinline__ void grid_barrier(u32* ctr, u32& epoch) {
+    if (gridDim.x == 1) {  // small inputs run in one CTA: a CTA barrier is a grid barrier
+        __syncthreads();
+        return;
+    }
     epoch += gridDim.x;
     __syncthreads();
     if (threadIdx.x == 0) {

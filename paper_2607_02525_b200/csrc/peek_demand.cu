@@ -42,17 +42,18 @@ __global__ void __launch_bounds__(DM_THREADS) k_demand(const u64* __restrict__ h
                                                       const i32* __restrict__ order,
                                                       const i32* __restrict__ lcp, MinTree mt,
                                                       const u64* __restrict__ t_keys, u64 mask,
-                                                      i32* __restrict__ demand) {
+                                                      i32* __restrict__ demand, int ppw) {
+    // ppw = positions per warp (1..32): few long chains (small N) spread over more warps
     __shared__ DemandMeta sm[DM_WARPS];
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const i64 j0 = (((i64)blockIdx.x * DM_THREADS + threadIdx.x) >> 5) * 32;
+    const i64 j0 = (((i64)blockIdx.x * DM_THREADS + threadIdx.x) >> 5) * ppw;
     if (j0 >= N) return;
     DemandMeta& M = sm[w];
     const i64 j = j0 + lane;
     i32 n_new = 0;
     {
-        const bool valid = j < N;
+        const bool valid = lane < ppw && j < N;
         i64 b0 = 0;
         i32 nb = 0, l0 = 0, l1 = 0;
         if (valid) {
@@ -479,9 +480,12 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
         mintree_layout(mt, lcp, N, mt_buf);
         Prof pr(PROF_DEMAND, st, mt.levels);
         mintree_build(mt, st);
-        unsigned grid = (unsigned)(((N + 31) / 32 * 32 + DM_THREADS - 1) / DM_THREADS);
+        int ppw = 32;  // at least ~16 K warps when the queue is small
+        while (ppw > 1 && N / ppw < 16384) ppw >>= 1;
+        const i64 warps = (N + ppw - 1) / ppw;
+        unsigned grid = (unsigned)((warps * 32 + DM_THREADS - 1) / DM_THREADS);
         k_demand<<<grid, DM_THREADS, 0, st>>>(hashes, blk_off, N, order, lcp, mt, table->t_keys,
-                                      (u64)(table->S - 1), demand);
+                                      (u64)(table->S - 1), demand, ppw);
     }
     if (clpm_order) {
         A.hit = hit; A.csize = cluster_size; A.arrival = arrival; A.N = N; A.out = clpm_order;

@@ -195,11 +195,11 @@ __global__ void __launch_bounds__(SG_THREADS) k_evict_write(const u64* __restric
                                                            const i64* ein_a, const i64* ein_b,
                                                            const i32* __restrict__ which,
                                                            const u64* __restrict__ t_keys, u64 mask,
-                                                           i64* __restrict__ evict) {
+                                                           i64* __restrict__ evict, int ppw) {
     __shared__ EvictMeta sm[EV_WARPS];
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const i64 j0 = (((i64)blockIdx.x * SG_THREADS + threadIdx.x) >> 5) * 32;
+    const i64 j0 = (((i64)blockIdx.x * SG_THREADS + threadIdx.x) >> 5) * ppw;  // ppw positions per warp
     if (j0 >= N) return;
     const i64* ein = *which ? ein_b : ein_a;
     EvictMeta& M = sm[w];
@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(SG_THREADS) k_evict_write(const u64* __restric
     i32 n_new = 0;
     i64 e_in = 0;
     {
-        const bool valid = j < N;
+        const bool valid = lane < ppw && j < N;
         i64 b0 = 0;
         i32 nb = 0, l0 = 0, l1 = 0;
         if (valid) {
@@ -400,9 +400,12 @@ extern "C" peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* 
         i64 n = N;
         void* params[] = {&n, &W.par[0], &W.ein[0], &W.par[1], &W.ein[1], &W.ctl, &W.which};
         PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_evict_jump, dim3(jgrid), dim3(1024), params, 0, st));
-        const unsigned wgrid = (unsigned)(((N + 31) / 32 * 32 + SG_THREADS - 1) / SG_THREADS);
+        int ppw = 32;
+        while (ppw > 1 && N / ppw < 16384) ppw >>= 1;
+        const i64 ewarps = (N + ppw - 1) / ppw;
+        const unsigned wgrid = (unsigned)((ewarps * 32 + SG_THREADS - 1) / SG_THREADS);
         k_evict_write<<<wgrid, SG_THREADS, 0, st>>>(hashes, blk_off, N, order, lcp, mt, W.ein[0], W.ein[1], W.which,
-                                                   table->t_keys, (u64)(table->S - 1), evict_score);
+                                                   table->t_keys, (u64)(table->S - 1), evict_score, ppw);
     }
     if (section) {
         PEEK_CUDA(cudaMemsetAsync(W.runmin, 0xff, sizeof(unsigned long long) * (size_t)N, st));
