@@ -210,6 +210,33 @@ __device__ __forceinline__ int grid_sort_pairs_gen(const GsBufs& b, i64 n, u64 v
     const i64 c0 = min((i64)blockIdx.x * C, n), c1 = min(c0 + C, n);
     const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
     int cur = HAS_GEN ? -1 : start_buf;  // -1: the generator is the source
+    if (gridDim.x == 1 && n <= GS_THREADS) {
+        // Small inputs (one CTA, one pair per thread): no passes at all - every pair counts the
+        // pairs that sort before it (smaller key, or equal key and earlier position) against the
+        // keys held in shared memory, and is written straight to that rank.  Queues of the size
+        // the paper runs (60-200 requests) take this path.
+        if (!HAS_GEN && vary == 0) return start_buf;
+        const int dstb = cur < 0 ? 0 : cur ^ 1;
+        const int t = threadIdx.x;
+        u64 key = ~0ull;
+        u32 val = 0;
+        if (t < n) {
+            if constexpr (HAS_GEN) gen((i64)t, key, val);
+            else { key = __ldcg(b.key[cur] + t); val = __ldcg(b.val[cur] + t); }
+        }
+        stg.key[t] = key;
+        __syncthreads();
+        u32 rank = 0;
+        const int nn = (int)n;
+#pragma unroll 4
+        for (int j = 0; j < nn; ++j) {
+            const u64 kj = stg.key[j];
+            rank += (kj < key || (kj == key && j < t)) ? 1u : 0u;
+        }
+        if (t < n) { b.key[dstb][rank] = key; b.val[dstb][rank] = val; }
+        __syncthreads();
+        return dstb;
+    }
     const GsHist gh = gs_hist(b.hist);
     int pass = 0;
     if (HAS_GEN && vary == 0) vary = 1;  // one (trivial) pass materialises the pairs
