@@ -322,3 +322,14 @@ def dynamic_lane(cluster_size, age_pressure: float, prev: float):
                            ctypes.c_double(age_pressure), ctypes.c_double(prev),
                            out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
     return float(out[0]), float(out[1])
+
+
+def stride_interleave(lane_a, lane_b, alpha: float):
+    """O15 stride interleave of the two lanes (Alg. 2 line 22; R28).  int32[N]."""
+    lane_a = _c(lane_a, np.int32)
+    lane_b = _c(lane_b, np.int32)
+    N = lane_a.shape[0]
+    out = np.zeros(N, dtype=np.int32)
+    lib().orc_stride_interleave(_p(lane_a, I32), _p(lane_b, I32), ctypes.c_int64(N), ctypes.c_double(alpha),
+                                _p(out, I32))
+    return out

@@ -555,3 +555,26 @@ extern "C" void orc_dynamic_lane(const i32* cluster_size, i64 N, double age_pres
     out[0] = p + q;  // the new fairness share 1 - alpha
     out[1] = sf;
 }
+
+// O15. Stride interleave of the two lanes (Alg. 2 line 22; "a fraction
+// alpha of admissions come from Lane A, 1 - alpha from Lane B").  The paper names the routine but
+// does not define it.  Reading R28: admission slot k = 0, 1, ... belongs to Lane A iff
+// floor((k+1)*alpha) > floor(k*alpha) - after any k slots Lane A has had floor(k*alpha) of them and
+// Lane B's slots are never more than ceil(1/(1-alpha)) apart - else to Lane B; the lane admits its
+// first request not admitted yet.  Both lanes list every request, so neither runs dry early.
+extern "C" void orc_stride_interleave(const i32* lane_a, const i32* lane_b, i64 N, double alpha, i32* out) {
+    std::vector<char> done((size_t)N, 0);
+    i64 ia = 0, ib = 0;
+    for (i64 k = 0; k < N; ++k) {
+        volatile double x0 = (double)k * alpha, x1 = (double)(k + 1) * alpha;
+        bool from_a = (i64)x1 > (i64)x0;  // alpha in [0, 1]: the products are >= 0, truncation = floor
+        if (from_a) {
+            while (done[(size_t)lane_a[ia]]) ++ia;
+            out[k] = lane_a[ia];
+        } else {
+            while (done[(size_t)lane_b[ib]]) ++ib;
+            out[k] = lane_b[ib];
+        }
+        done[(size_t)out[k]] = 1;
+    }
+}

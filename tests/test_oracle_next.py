@@ -365,3 +365,36 @@ def test_lane_b_and_dynamic_lane():
     new, sf = oracle.dynamic_lane(cs, 0.5, 0.3)
     x = min(max(0.15 + 0.5 * 0.5 + 0.3 * 0.5, 0.10), 0.60)
     assert sf == 0.5 and abs(new - (0.3 * x + 0.7 * 0.3)) < 1e-15
+
+
+def test_stride_interleave_properties_and_closed_forms():
+    """a fraction alpha of the admissions come from Lane A; the fairness lane (whose
+    head is the oldest request) advances at least every ceil(1 / (1 - alpha)) slots."""
+    import math
+    rng = np.random.default_rng(4)
+    N = 500
+    a = rng.permutation(N).astype(np.int32)
+    b = rng.permutation(N).astype(np.int32)
+    pos_a = np.argsort(a)
+    pos_b = np.argsort(b)
+    for alpha in (0.7, 0.4, 0.85, 0.9):
+        out = oracle.stride_interleave(a, b, alpha)
+        assert sorted(out.tolist()) == list(range(N))
+        # replay: which lane admitted each slot is fixed by alpha alone
+        from_a = [math.floor((k + 1) * alpha) > math.floor(k * alpha) for k in range(N)]
+        for k in (10, 100, 499):
+            assert sum(from_a[:k]) == math.floor(k * alpha)
+        gaps = np.diff([k for k in range(N) if not from_a[k]])
+        assert gaps.max() <= math.ceil(1 / (1 - alpha))
+        # every slot admits, from its lane, a request all of whose lane predecessors are admitted
+        seen = set()
+        for k, r in enumerate(out.tolist()):
+            lane_pos, lane = (pos_a, a) if from_a[k] else (pos_b, b)
+            assert all(int(x) in seen for x in lane[: lane_pos[r]])
+            seen.add(r)
+    assert oracle.stride_interleave(a, b, 1.0).tolist() == a.tolist()
+    assert oracle.stride_interleave(a, b, 0.0).tolist() == b.tolist()
+    assert oracle.stride_interleave(a, a, 0.7).tolist() == a.tolist()
+    # A ascending, B descending, alpha = 1/2: B, A, B, A ... from the two ends
+    up = np.arange(10, dtype=np.int32)
+    assert oracle.stride_interleave(up, up[::-1].copy(), 0.5).tolist() == [9, 0, 8, 1, 7, 2, 6, 3, 5, 4]
