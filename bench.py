@@ -278,13 +278,16 @@ def next_rows_timing(inp, out):
     ms_sig, (sec, sc, ev) = timed(lambda: B.peek_clpm_signals(h, bo, tree, hit=hit, tau=0, arrival=inp.arrival,
                                                               t_keys=inp.keys))
     ms_ord, lane = timed(lambda: B.peek_clpm_order_full(sec, hit, sc, tree.cluster_size, inp.arrival))
-    ms_gm, _ = timed(lambda: B.peek_clpm_group_major(lane, tree.cluster_id))
+    ms_gm, gm = timed(lambda: B.peek_clpm_group_major(lane, tree.cluster_id))
+    ms_lb, lane_b = timed(lambda: B.peek_clpm_lane_b(sec, hit, inp.arrival))
+    ms_si, _ = timed(lambda: B.peek_stride_interleave(gm, lane_b, 0.7), n=1)
     ms_off, (_, guards) = timed(lambda: B.peek_offline_phase1(h, bo, 8))
     ms_nd = None
     if inp.radix is not None and out["hit_radix"] is not None:
         ms_nd, _ = timed(lambda: B.peek_radix_demand(inp.tok, inp.off, inp.radix, out["hit_radix"]))
     return {"peek_clpm_signals_ms": ms_sig, "peek_clpm_order_full_ms": ms_ord,
-            "peek_clpm_group_major_ms": ms_gm, "peek_offline_phase1_ms": ms_off, "peek_radix_demand_ms": ms_nd,
+            "peek_clpm_group_major_ms": ms_gm, "peek_clpm_lane_b_ms": ms_lb, "peek_stride_interleave_ms": ms_si,
+            "peek_offline_phase1_ms": ms_off, "peek_radix_demand_ms": ms_nd,
             "offline_guards_dup_cov_depth_fired": guards.cpu().tolist(),
             "sections_warm_pioneer_sibling": torch.bincount(sec, minlength=3).tolist()[:3]}
 

@@ -235,8 +235,7 @@ peek_status peek_clpm_lane_b(const int32_t* section, const int32_t* hit, const i
  *          + 0.7 * prev_fair_share     (the new fairness share 1 - alpha, double, every product and
  *          sum rounded once), out[1] = singleton_frac = fraction of requests with cluster_size == 1.
  * out double[2] device; age_pressure = min(1, oldest singleton wait / 2 s) is the engine's to supply.
- * Workspace: >= 256 bytes.  The stride interleave of Alg. 2 line 22 is not part of this library: the
- * paper does not define it beyond its name. */
+ * Workspace: >= 256 bytes. */
 peek_status peek_dynamic_lane(const int32_t* cluster_size, int64_t N, double age_pressure,
                               double prev_fair_share, double* out, void* ws, int64_t ws_bytes, void* stream);
 
@@ -255,6 +254,17 @@ peek_status peek_pending_tree_update(const uint64_t* hashes, const int64_t* blk_
                                      int32_t* group_size, int32_t* cluster_depth, int32_t* cluster_size,
                                      int64_t* cluster_id, int32_t* n_groups, void* ws, int64_t ws_bytes,
                                      void* stream);
+
+/* a11d: the stride interleave of Alg. 2 line 22, which the paper names but does
+ * not define; R28: admission slot k = 0, 1, .. belongs to Lane A iff
+ * floor((k+1) * alpha) > floor(k * alpha) (double products rounded once), else to Lane B, and the lane
+ * admits its first request not admitted yet.
+ * lane_a, lane_b int32[N] permutations of the requests (peek_clpm_order_full / _group_major, _lane_b)
+ * alpha in [0, 1]: the share of Lane A (1 - out[0] of peek_dynamic_lane; default 0.7)
+ * out    int32[N] the admission order.  Workspace: (N + 31) / 32 * 4 bytes when that exceeds 200 KB
+ * (N > 1.6 M), none otherwise.  A sequential walk: one warp, 32 slots per step. */
+peek_status peek_stride_interleave(const int32_t* lane_a, const int32_t* lane_b, int64_t N, double alpha,
+                                   int32_t* out, void* ws, int64_t ws_bytes, void* stream);
 
 /* a12: PEEK-offline phase 1 (R25).
  * depth_blocks the trie covers the first depth_blocks blocks of every chain (the paper's D = 128

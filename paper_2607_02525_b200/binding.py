@@ -25,7 +25,8 @@ EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_worksp
            "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
            "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1", "peek_radix_demand",
-           "peek_clpm_lane_b", "peek_dynamic_lane", "peek_pending_tree_update"]
+           "peek_clpm_lane_b", "peek_dynamic_lane", "peek_pending_tree_update",
+           "peek_stride_interleave"]
 
 
 class PeekError(RuntimeError):
@@ -84,6 +85,8 @@ def lib():
         L.peek_clpm_group_major.argtypes = [vp, vp, i64, vp, vp, i64, vp]
         L.peek_pending_tree_update.restype = i32
         L.peek_pending_tree_update.argtypes = [vp, vp, i64, i64, vp, vp, i64, vp] + [vp] * 8 + [vp, i64, vp]
+        L.peek_stride_interleave.restype = i32
+        L.peek_stride_interleave.argtypes = [vp, vp, i64, ctypes.c_double, vp, vp, i64, vp]
         L.peek_clpm_lane_b.restype = i32
         L.peek_clpm_lane_b.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp]
         L.peek_dynamic_lane.restype = i32
@@ -332,6 +335,18 @@ def peek_pending_tree_update(hashes, blk_off, M: int, old: PendingTree, remap, s
                                     _ptr(ws), int(nb.value), _stream())
     _check(st, "peek_pending_tree_update")
     return t
+
+
+def peek_stride_interleave(lane_a, lane_b, alpha: float = 0.7):
+    """a11d: stride interleave of the two lanes (Alg. 2 line 22; R28).  int32[N]."""
+    N = int(lane_a.shape[0])
+    dev = lane_a.device
+    out = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N]
+    nbytes = max(256, (N + 31) // 32 * 4)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    st = lib().peek_stride_interleave(_ptr(lane_a), _ptr(lane_b), N, float(alpha), _ptr(out), _ptr(ws), nbytes, _stream())
+    _check(st, "peek_stride_interleave")
+    return out
 
 
 def peek_clpm_lane_b(section, hit, arrival=None):

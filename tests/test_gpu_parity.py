@@ -125,6 +125,9 @@ def check_next_rows(b, g_h, g_bo, gt, o_h, o_bo, ot, hit_np, arrival, t_keys, d_
             "full cLPM order tau=%d" % tau
         g_lb = b.peek_clpm_lane_b(g_sec, d_hit, d_arr)
         assert np.array_equal(_np(g_lb), oracle.lane_b(o_sec, hit_np, arrival)), "lane B order"
+        for alpha in (0.7, 0.4):
+            g_adm = b.peek_stride_interleave(g_full, g_lb, alpha)
+            assert np.array_equal(_np(g_adm), oracle.stride_interleave(_np(g_full), _np(g_lb), alpha)), "interleave"
         g_gm = b.peek_clpm_group_major(g_full, gt.cluster_id)
         assert np.array_equal(_np(g_gm), oracle.group_major(_np(g_full), ot.cluster_id)), "group-major order"
     for age, prev in ((0.0, 0.15), (0.37, 0.3), (1.0, 0.6)):
@@ -428,3 +431,20 @@ def test_pending_tree_update_matches_rebuild():
         want = oracle.pending_tree(h, bo)
         assert np.array_equal(_np(tree.order), want.order) and np.array_equal(_np(tree.lcp), want.lcp), cycle
         assert np.array_equal(_np(tree.cluster_size), want.cluster_size), cycle
+
+
+def test_stride_interleave_cases():
+    """Identical lanes (every step clashes and is replayed), reversed lanes, alpha 0 and 1, a queue
+    shorter than one step, and sizes around the 32-slot step and the 128-entry scan."""
+    b = _b()
+    rng = np.random.default_rng(8)
+    for n in (1, 5, 31, 32, 33, 127, 128, 129, 1000, 50000):
+        a = rng.permutation(n).astype(np.int32)
+        for lane_b in (a.copy(), a[::-1].copy(), rng.permutation(n).astype(np.int32)):
+            for alpha in (0.0, 0.3, 0.7, 1.0):
+                got = b.peek_stride_interleave(_dev(a), _dev(lane_b), alpha)
+                assert np.array_equal(_np(got), oracle.stride_interleave(a, lane_b, alpha)), (n, alpha)
+    n = 1_700_000  # the admitted-bitmap no longer fits shared memory: global-memory bitmap
+    a, lane_b = rng.permutation(n).astype(np.int32), rng.permutation(n).astype(np.int32)
+    got = b.peek_stride_interleave(_dev(a), _dev(lane_b), 0.7)
+    assert np.array_equal(_np(got), oracle.stride_interleave(a, lane_b, 0.7))
