@@ -120,16 +120,18 @@ def check_next_rows(b, g_h, g_bo, gt, o_h, o_bo, ot, hit_np, arrival, t_keys, d_
         assert np.array_equal(_np(g_score), o_score), "score"
         if t_keys is not None:
             assert np.array_equal(_np(g_ev), oracle.evict_score(o_h, o_bo, t_keys, 16)), "evict_score"
+        # every oracle input below is the oracle's own (never a CUDA output)
+        o_full = oracle.clpm_order_full(o_sec, hit_np, o_score, ot.cluster_size, arrival)
+        o_lb = oracle.lane_b(o_sec, hit_np, arrival)
         g_full = b.peek_clpm_order_full(g_sec, d_hit, g_score, gt.cluster_size, d_arr)
-        assert np.array_equal(_np(g_full), oracle.clpm_order_full(o_sec, hit_np, o_score, ot.cluster_size, arrival)), \
-            "full cLPM order tau=%d" % tau
+        assert np.array_equal(_np(g_full), o_full), "full cLPM order tau=%d" % tau
         g_lb = b.peek_clpm_lane_b(g_sec, d_hit, d_arr)
-        assert np.array_equal(_np(g_lb), oracle.lane_b(o_sec, hit_np, arrival)), "lane B order"
+        assert np.array_equal(_np(g_lb), o_lb), "lane B order"
         for alpha in (0.7, 0.4):
             g_adm = b.peek_stride_interleave(g_full, g_lb, alpha)
-            assert np.array_equal(_np(g_adm), oracle.stride_interleave(_np(g_full), _np(g_lb), alpha)), "interleave"
+            assert np.array_equal(_np(g_adm), oracle.stride_interleave(o_full, o_lb, alpha)), "interleave"
         g_gm = b.peek_clpm_group_major(g_full, gt.cluster_id)
-        assert np.array_equal(_np(g_gm), oracle.group_major(_np(g_full), ot.cluster_id)), "group-major order"
+        assert np.array_equal(_np(g_gm), oracle.group_major(o_full, ot.cluster_id)), "group-major order"
     for age, prev in ((0.0, 0.15), (0.37, 0.3), (1.0, 0.6)):
         g_dl = b.peek_dynamic_lane(gt.cluster_size, age, prev).cpu().numpy()
         assert g_dl.tolist() == list(oracle.dynamic_lane(ot.cluster_size, age, prev)), "dynamic lane"
