@@ -84,3 +84,41 @@ def test_binding_refuses_cpu_tensors():
     from paper_2607_02525_b200 import binding
     with pytest.raises(binding.PeekError):
         binding.peek_block_hash(torch.zeros(16, dtype=torch.int32), torch.tensor([0, 16]), 1)
+
+
+def test_next_row_calls_argument_errors(lib):
+    """Host-side checks of the SURVEY 8(f) calls answer before any CUDA call."""
+    vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
+    dbl = ctypes.c_double
+    lib.peek_clpm_signals.argtypes = [vp, vp, i64, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, i64, vp]
+    assert lib.peek_clpm_signals(None, None, -1, None, None, None, 0, None, None, None, None, None, None, 0, None) == -1
+    assert lib.peek_clpm_signals(None, None, 0, None, None, None, 0, None, None, None, None, None, None, 0, None) == 0
+    lib.peek_clpm_order_full.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp, i64, vp]
+    assert lib.peek_clpm_order_full(None, None, None, None, None, 0, None, None, 0, None) == 0
+    assert lib.peek_clpm_order_full(None, None, None, None, None, 3, None, None, 0, None) == -1
+    lib.peek_clpm_group_major.argtypes = [vp, vp, i64, vp, vp, i64, vp]
+    assert lib.peek_clpm_group_major(None, None, 3, None, None, 0, None) == -1
+    lib.peek_clpm_lane_b.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp]
+    assert lib.peek_clpm_lane_b(None, None, None, 3, None, None, 0, None) == -1
+    lib.peek_stride_interleave.argtypes = [vp, vp, i64, dbl, vp, vp, i64, vp]
+    assert lib.peek_stride_interleave(None, None, 0, 0.7, None, None, 0, None) == 0
+    assert lib.peek_stride_interleave(None, None, 4, 1.5, None, None, 0, None) == -1      # alpha outside [0, 1]
+    assert lib.peek_stride_interleave(None, None, 4, float("nan"), None, None, 0, None) == -1
+    lib.peek_dynamic_lane.argtypes = [vp, i64, dbl, dbl, vp, vp, i64, vp]
+    assert lib.peek_dynamic_lane(None, 4, 0.0, 0.15, None, None, 0, None) == -1
+    lib.peek_offline_phase1.argtypes = [vp, vp, i64, i32, vp, vp, vp, i64, vp]
+    assert lib.peek_offline_phase1(None, None, 4, 0, None, None, None, 0, None) == -1     # depth_blocks 1..16
+    assert lib.peek_offline_phase1(None, None, 4, 17, None, None, None, 0, None) == -1
+    assert lib.peek_offline_phase1(None, None, 0, 8, None, None, None, 0, None) == 0
+    lib.peek_radix_demand.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+    assert lib.peek_radix_demand(None, None, 4, None, None, None, None) == -1
+    lib.peek_pending_tree_update.argtypes = [vp, vp, i64, i64, vp, vp, i64, vp] + [vp] * 8 + [vp, i64, vp]
+    assert lib.peek_pending_tree_update(None, None, 4, 5, None, None, 0, None, *([None] * 8), None, 0, None) == -1  # M > N_new
+    assert lib.peek_pending_tree_update(None, None, 0, 0, None, None, 0, None, *([None] * 8), None, 0, None) == 0
+    out = ctypes.c_int64(0)
+    f = lib.peek_workspace_bytes
+    f.argtypes = [ctypes.c_int32] + [ctypes.c_int64] * 5 + [ctypes.POINTER(ctypes.c_int64)]
+    for call in (4, 5, 6, 7):
+        assert f(call, 1 << 16, 0, 0, 1 << 18, 0, ctypes.byref(out)) == 0 and out.value % 256 == 0
+    assert f(8, 1 << 16, 1 << 16, 100, 0, 0, ctypes.byref(out)) == 0 and out.value >= 256
+    assert f(8, 1 << 16, -1, 100, 0, 0, ctypes.byref(out)) == -1
