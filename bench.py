@@ -322,9 +322,12 @@ def oracle_pass(wl, cache, n_sample: int):
     """The oracle as it stands, on the first n_sample requests of the workload against the same
     cache.  Returns seconds for one pass of the whole path."""
     import oracle
-    sub = wl.queue.select(np.arange(n_sample))
-    toks, off = sub.materialize_np()
-    arrival = np.ascontiguousarray(wl.arrival[:n_sample])
+    memo = getattr(oracle_pass, "_memo", None)  # the same prefix is timed several times
+    if memo is None or memo[0] is not wl or memo[1] != n_sample:
+        sub = wl.queue.select(np.arange(n_sample))
+        toks, off = sub.materialize_np()
+        oracle_pass._memo = memo = (wl, n_sample, toks, off, np.ascontiguousarray(wl.arrival[:n_sample]))
+    _, _, toks, off, arrival = memo
     radix = None
     if cache.radix is not None:
         r = cache.radix
@@ -339,11 +342,10 @@ def oracle_pass(wl, cache, n_sample: int):
     return time.perf_counter() - t0
 
 
-def cpu_baseline(wl, cache, budget_s: float):
-    """The oracle as it stands on a bounded prefix of the workload sized for about budget_s seconds
-    of CPU work.  The pass has a fixed part (the demand map over the whole table) and a part
-    linear in the requests; the sample is grown from the measured marginal cost."""
-    import oracle
+def size_sample(wl, cache, budget_s: float):
+    """Requests (a prefix of the workload) the oracle gets through in about budget_s seconds.  The
+    pass has a fixed part (the demand map over the whole table) and a part linear in the requests;
+    the sample is grown from the measured marginal cost.  Returns (n, seconds of the last pass)."""
     n1 = min(wl.N, 2048)
     t1 = oracle_pass(wl, cache, n1)
     n, dt = n1, t1
@@ -355,6 +357,14 @@ def cpu_baseline(wl, cache, budget_s: float):
         n3 = int(min(wl.N, n2 + max(0.0, budget_s - t2) / marginal * 0.8))
         if n3 > n2 * 1.5 and t2 < 0.5 * budget_s:
             n, dt = n3, oracle_pass(wl, cache, n3)
+    return n, dt
+
+
+def cpu_baseline(wl, cache, budget_s: float):
+    """The oracle as it stands on a bounded prefix of the workload sized for about budget_s seconds
+    of CPU work."""
+    import oracle
+    n, dt = size_sample(wl, cache, budget_s)
     return {"value": n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
             "sample": "first %d of %d requests of the same workload, same cache, one pass of "
                       "hash+tree+lpm(radix,hash)+demand+rank in %.2f s" % (n, wl.N, dt)}
@@ -374,9 +384,10 @@ def run_reference(args):
         return
     import oracle
     wl, cache = cpu_inputs(args.config, args.seed, args.small)
-    n = min(wl.N, 2048)
-    dt = oracle_pass(wl, cache, n)
-    n = int(min(wl.N, max(n, n * 4.0 / max(dt, 1e-3) * 0.5)))  # ~4 s per step
+    # each step = the oracle on a prefix of the workload sized so that warm-up + timed steps take
+    # about a minute (at most 15 s a step)
+    budget = max(1.0, min(15.0, 60.0 / max(args.steps + args.warmup, 1)))
+    n, _ = size_sample(wl, cache, budget)
     for _ in range(args.warmup):
         oracle_pass(wl, cache, n)
     t = 0.0
