@@ -654,18 +654,21 @@ __device__ __forceinline__ bool si_bit(const u32* bits, i32 r) {
     return (((const volatile u32*)bits)[r >> 5] >> (r & 31)) & 1u;
 }
 
-// first <= 32 not-admitted entries of list[m .. N): c[] = request, ci[] = its list position
+// first <= 32 not-admitted entries of list[m .. N): c[] = request, ci[] = its list position.
+// v0[] = the first SI_SCAN x 32 entries from m, loaded by the caller (both lanes' loads are issued
+// together, one memory round trip per step in the common case)
+__device__ __forceinline__ void si_load(const i32* __restrict__ list, i64 m, i64 N, int lane, i32 (&v)[SI_SCAN]) {
+#pragma unroll
+    for (int u = 0; u < SI_SCAN; ++u) {
+        const i64 p = m + u * 32 + lane;
+        v[u] = p < N ? __ldg(list + p) : -1;
+    }
+}
 __device__ __forceinline__ int si_gather(const i32* __restrict__ list, i64 m, i64 N, const u32* bits, i32* c,
-                                         i64* ci, int lane) {
+                                         i64* ci, int lane, i32 (&v)[SI_SCAN]) {
     const unsigned FULL = 0xffffffffu, lt = (1u << lane) - 1u;
     int found = 0;
-    while (found < 32 && m < N) {
-        i32 v[SI_SCAN];
-#pragma unroll
-        for (int u = 0; u < SI_SCAN; ++u) {
-            const i64 p = m + u * 32 + lane;
-            v[u] = p < N ? __ldg(list + p) : -1;
-        }
+    for (;;) {
 #pragma unroll
         for (int u = 0; u < SI_SCAN; ++u) {
             const bool ne = v[u] >= 0 && !si_bit(bits, v[u]);
@@ -675,6 +678,8 @@ __device__ __forceinline__ int si_gather(const i32* __restrict__ list, i64 m, i6
             found += __popc(bal);
         }
         m += 32 * SI_SCAN;
+        if (found >= 32 || m >= N) break;
+        si_load(list, m, N, lane, v);
     }
     __syncwarp();
     return found < 32 ? found : 32;
@@ -701,8 +706,11 @@ __global__ void __launch_bounds__(32) k_stride_interleave(const i32* __restrict_
         const unsigned balA = __ballot_sync(FULL, from_a);
         const unsigned balB = ~balA & (cnt == 32 ? FULL : ((1u << cnt) - 1u));
         const int nA = __popc(balA), nB = __popc(balB);
-        const int gA = nA ? si_gather(lane_a, mA, N, bits, cA, iA, lane) : 0;
-        const int gB = nB ? si_gather(lane_b, mB, N, bits, cB, iB, lane) : 0;
+        i32 vA[SI_SCAN], vB[SI_SCAN];
+        si_load(lane_a, mA, N, lane, vA);
+        si_load(lane_b, mB, N, lane, vB);
+        const int gA = nA ? si_gather(lane_a, mA, N, bits, cA, iA, lane, vA) : 0;
+        const int gB = nB ? si_gather(lane_b, mB, N, bits, cB, iB, lane, vB) : 0;
         (void)gA; (void)gB;  // 32 not-admitted candidates per lane always suffice for 32 slots
         // every slot takes its lane's next candidate; a test-and-set exposes a request wanted twice
         i32 pick = -1;
