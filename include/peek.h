@@ -11,11 +11,14 @@
  *   peek_lpm           per-request hit length against the engine's prefix cache: a radix cache
  *                      (Alg. 1) and/or a flat block-hash table
  *                      ("per-request find_longest_cache_hit")
- *   (next rows: peek_clpm_signals - sections, ancestor score, Eq. 2 eviction
- *    score - and peek_clpm_order_full, the five-part key of Eq. 1; declared further down)
  *   peek_demand_rank   per-cached-block pending demand for the eviction hook (PAPER.md:115-119
  *                      Eq. 2 pending_count; :281 inverted index block_hash -> demand) and the cLPM
  *                      admission order, sub-key (-h, -|cluster|, arrival) of Eq. 1
+ * and the next rows of SURVEY.md 8(f), declared further down: peek_clpm_signals (sections, ancestor
+ * score, Eq. 2 eviction score), peek_radix_demand, peek_clpm_order_full (the five-part key of Eq. 1),
+ * peek_clpm_group_major, peek_clpm_lane_b, peek_dynamic_lane, peek_stride_interleave (Alg. 2 of
+ * PAPER.md:325 end to end), peek_pending_tree_update (incremental maintenance) and
+ * peek_offline_phase1 (PEEK-offline's reordering and guards).
  *
  * Conventions (the paper is silent on all of them):
  *   Pointers   every array pointer is caller-owned DEVICE memory unless marked [host]; it must
