@@ -77,12 +77,17 @@ __device__ __forceinline__ void gs_rank_tile(u32 (&meta)[K], GsSmem& sm) {
     const unsigned lt = (1u << lane) - 1u;
     for (int d = threadIdx.x; d < GS_WARPS * 256 / 2; d += GS_THREADS) ((u32*)&sm.wcnt[0][0])[d] = 0;
     unsigned peers[K];
+    unsigned live = 0;  // rows of this warp that hold any pair (small inputs fill only the first)
 #pragma unroll
-    for (int k = 0; k < K; ++k) peers[k] = gs_peers(meta[k]);
+    for (int k = 0; k < K; ++k) {
+        peers[k] = 0;
+        if (__any_sync(0xffffffffu, meta[k] < 256u)) { peers[k] = gs_peers(meta[k]); live |= 1u << k; }
+    }
     __syncthreads();
     PEEK_MARK(110);
 #pragma unroll
     for (int k = 0; k < K; ++k) {
+        if (!((live >> k) & 1u)) continue;  // warp-uniform
         const u32 dg = meta[k];
         const bool valid = dg < 256u;
         const u32 old = valid ? sm.wcnt[w][dg] : 0;
