@@ -264,8 +264,8 @@ peek_status peek_pending_tree_update(const uint64_t* hashes, const int64_t* blk_
  * admits its first request not admitted yet.
  * lane_a, lane_b int32[N] permutations of the requests (peek_clpm_order_full / _group_major, _lane_b)
  * alpha in [0, 1]: the share of Lane A (1 - out[0] of peek_dynamic_lane; default 0.7)
- * out    int32[N] the admission order.  Workspace: (N + 31) / 32 * 4 bytes when that exceeds 200 KB
- * (N > 1.6 M), none otherwise.  A sequential walk: one warp, 32 slots per step. */
+ * out    int32[N] the admission order.  Workspace: (N + 31) / 32 * 4 bytes when that exceeds 160 KB
+ * (N > 1.3 M), none otherwise.  Sequential across slots: one CTA, 1024 slots per step. */
 peek_status peek_stride_interleave(const int32_t* lane_a, const int32_t* lane_b, int64_t N, double alpha,
                                    int32_t* out, void* ws, int64_t ws_bytes, void* stream);
 

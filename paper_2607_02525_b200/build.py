@@ -12,7 +12,8 @@ from concurrent.futures import ThreadPoolExecutor
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpeek.so")
-SOURCES = ["peek_api.cu", "peek_hash.cu", "peek_lpm.cu", "peek_tree.cu", "peek_demand.cu", "peek_signals.cu", "peek_offline.cu"]
+SOURCES = ["peek_api.cu", "peek_hash.cu", "peek_lpm.cu", "peek_tree.cu", "peek_demand.cu", "peek_signals.cu", "peek_offline.cu",
+           "peek_interleave.cu"]
 HEADERS = ["peek_common.cuh", "peek_grid.cuh", "peek_sort.cuh", os.path.join("..", "..", "include", "peek.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-diag-suppress", "177"]

@@ -639,136 +639,5 @@ extern "C" peek_status peek_clpm_group_major(const int32_t* lane_order, const in
 
 PEEK_TRACE_EXPORT(peek_trace_read_rank)
 
-// ---- a11d: stride interleave of the two lanes (Alg. 2 line 22; R28) ----
-// Slot k belongs to Lane A iff floor((k+1) alpha) > floor(k alpha); the lane admits its first
-// request not admitted yet.  The walk is sequential by nature (a lane skips what the other one
-// admitted), so ONE warp does it, 32 slots per step: each lane list is scanned from its cursor for
-// the next not-admitted requests (coalesced reads, a bitmap of admitted requests in shared memory
-// when it fits), the 32 slots take them in order, and a test-and-set on the bitmap tells whether
-// two slots of the step wanted the same request - only then lane 0 replays the step one by one.
-namespace peek {
-static constexpr int SI_SCAN = 4;  // list entries per lane per scan: 128 per list and step
-
-// volatile: the bitmap changes under the warp's own atomics (and may live in global memory)
-__device__ __forceinline__ bool si_bit(const u32* bits, i32 r) {
-    return (((const volatile u32*)bits)[r >> 5] >> (r & 31)) & 1u;
-}
-
-// first <= 32 not-admitted entries of list[m .. N): c[] = request, ci[] = its list position.
-// v0[] = the first SI_SCAN x 32 entries from m, loaded by the caller (both lanes' loads are issued
-// together, one memory round trip per step in the common case)
-__device__ __forceinline__ void si_load(const i32* __restrict__ list, i64 m, i64 N, int lane, i32 (&v)[SI_SCAN]) {
-#pragma unroll
-    for (int u = 0; u < SI_SCAN; ++u) {
-        const i64 p = m + u * 32 + lane;
-        v[u] = p < N ? __ldg(list + p) : -1;
-    }
-}
-__device__ __forceinline__ int si_gather(const i32* __restrict__ list, i64 m, i64 N, const u32* bits, i32* c,
-                                         i64* ci, int lane, i32 (&v)[SI_SCAN]) {
-    const unsigned FULL = 0xffffffffu, lt = (1u << lane) - 1u;
-    int found = 0;
-    for (;;) {
-#pragma unroll
-        for (int u = 0; u < SI_SCAN; ++u) {
-            const bool ne = v[u] >= 0 && !si_bit(bits, v[u]);
-            const unsigned bal = __ballot_sync(FULL, ne);
-            const int rk = found + __popc(bal & lt);
-            if (ne && rk < 32) { c[rk] = v[u]; ci[rk] = m + u * 32 + lane; }
-            found += __popc(bal);
-        }
-        m += 32 * SI_SCAN;
-        if (found >= 32 || m >= N) break;
-        si_load(list, m, N, lane, v);
-    }
-    __syncwarp();
-    return found < 32 ? found : 32;
-}
-
-__global__ void __launch_bounds__(32) k_stride_interleave(const i32* __restrict__ lane_a,
-                                                         const i32* __restrict__ lane_b, i64 N, double alpha,
-                                                         i32* __restrict__ out, u32* gbits, int use_smem) {
-    extern __shared__ u32 si_smem[];
-    __shared__ i32 cA[32], cB[32];
-    __shared__ i64 iA[32], iB[32];
-    const unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x;
-    const unsigned lt = (1u << lane) - 1u;
-    u32* bits = use_smem ? si_smem : gbits;
-    const i64 words = (N + 31) >> 5;
-    for (i64 x = lane; x < words; x += 32) bits[x] = 0;
-    __syncwarp();
-    i64 mA = 0, mB = 0;
-    for (i64 k = 0; k < N; k += 32) {
-        const int cnt = (int)(N - k < 32 ? N - k : 32);
-        const i64 s = k + lane;
-        const bool from_a = lane < cnt && (i64)__dmul_rn((double)(s + 1), alpha) > (i64)__dmul_rn((double)s, alpha);
-        const unsigned balA = __ballot_sync(FULL, from_a);
-        const unsigned balB = ~balA & (cnt == 32 ? FULL : ((1u << cnt) - 1u));
-        const int nA = __popc(balA), nB = __popc(balB);
-        i32 vA[SI_SCAN], vB[SI_SCAN];
-        si_load(lane_a, mA, N, lane, vA);
-        si_load(lane_b, mB, N, lane, vB);
-        const int gA = nA ? si_gather(lane_a, mA, N, bits, cA, iA, lane, vA) : 0;
-        const int gB = nB ? si_gather(lane_b, mB, N, bits, cB, iB, lane, vB) : 0;
-        (void)gA; (void)gB;  // 32 not-admitted candidates per lane always suffice for 32 slots
-        // every slot takes its lane's next candidate; a test-and-set exposes a request wanted twice
-        i32 pick = -1;
-        if (lane < cnt) pick = from_a ? cA[__popc(balA & lt)] : cB[__popc(balB & lt)];
-        bool clash = false;
-        if (pick >= 0) clash = (atomicOr(&bits[pick >> 5], 1u << (pick & 31)) >> (pick & 31)) & 1u;
-        int ia = nA, ib = nB;
-        if (__any_sync(FULL, clash)) {
-            if (pick >= 0) atomicAnd(&bits[pick >> 5], ~(1u << (pick & 31)));
-            __syncwarp();
-            ia = ib = 0;
-            if (lane == 0) {  // replay the step slot by slot
-                for (int q = 0; q < cnt; ++q) {
-                    i32 r;
-                    if ((balA >> q) & 1u) { while (si_bit(bits, cA[ia])) ++ia; r = cA[ia++]; }
-                    else { while (si_bit(bits, cB[ib])) ++ib; r = cB[ib++]; }
-                    bits[r >> 5] |= 1u << (r & 31);
-                    out[k + q] = r;
-                }
-            }
-            ia = __shfl_sync(FULL, ia, 0);
-            ib = __shfl_sync(FULL, ib, 0);
-        } else if (lane < cnt) {
-            out[s] = pick;
-        }
-        __syncwarp();
-        if (ia > 0) mA = iA[ia - 1] + 1;  // everything up to the last candidate looked at is admitted
-        if (ib > 0) mB = iB[ib - 1] + 1;
-        __syncwarp();
-    }
-}
-}  // namespace peek
-
 using namespace peek;
 
-extern "C" peek_status peek_stride_interleave(const int32_t* lane_a, const int32_t* lane_b, int64_t N,
-                                              double alpha, int32_t* out, void* ws, int64_t ws_bytes,
-                                              void* stream) {
-    if (N < 0 || N >= 0x7fffffffLL || !(alpha >= 0.0 && alpha <= 1.0)) {
-        set_error("peek_stride_interleave: N out of range or alpha outside [0, 1]");
-        return PEEK_ERR_INVALID_ARG;
-    }
-    if (N == 0) return PEEK_OK;
-    if (!lane_a || !lane_b || !out) { set_error("peek_stride_interleave: NULL argument"); return PEEK_ERR_INVALID_ARG; }
-    const i64 bytes = ((N + 31) / 32) * 4;
-    const int use_smem = bytes <= 200 * 1024;
-    if (!use_smem && (!ws || ((uintptr_t)ws & 255) || ws_bytes < bytes)) {
-        set_error("peek_stride_interleave: workspace NULL, misaligned or too small");
-        return PEEK_ERR_WORKSPACE;
-    }
-    static bool attr_set = false;
-    if (!attr_set) {
-        PEEK_CUDA(cudaFuncSetAttribute(k_stride_interleave, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
-    }
-    cudaStream_t st = (cudaStream_t)stream;
-    Prof pr(PROF_RANK_FULL, st, 1);
-    k_stride_interleave<<<1, 32, use_smem ? (size_t)bytes : 0, st>>>(lane_a, lane_b, N, alpha, out, (u32*)ws, use_smem);
-    PEEK_CUDA(cudaGetLastError());
-    return PEEK_OK;
-}

@@ -436,14 +436,16 @@ def test_pending_tree_update_matches_rebuild():
 
 
 def test_stride_interleave_cases():
-    """Identical lanes (every step clashes and is replayed), reversed lanes, alpha 0 and 1, a queue
-    shorter than one step, and sizes around the 32-slot step and the 128-entry scan."""
+    """Identical lanes (every candidate clashes), reversed lanes, locally shuffled lanes (clashes in
+    most steps, resolved in time order), alpha 0, 1 and next to 1, a queue shorter than one step,
+    and sizes around the 1024-slot step and the 2048-entry window."""
     b = _b()
     rng = np.random.default_rng(8)
-    for n in (1, 5, 31, 32, 33, 127, 128, 129, 1000, 50000):
+    for n in (1, 5, 31, 32, 33, 1000, 1023, 1024, 1025, 2047, 2049, 4096, 5000, 50000):
         a = rng.permutation(n).astype(np.int32)
-        for lane_b in (a.copy(), a[::-1].copy(), rng.permutation(n).astype(np.int32)):
-            for alpha in (0.0, 0.3, 0.7, 1.0):
+        near = a[np.argsort(np.arange(n) + rng.uniform(0, 300, n), kind="stable")].copy()
+        for lane_b in (a.copy(), a[::-1].copy(), near, rng.permutation(n).astype(np.int32)):
+            for alpha in (0.0, 0.3, 0.5, 0.7, 0.999, 1.0 - 2.0 ** -40, 1.0):
                 got = b.peek_stride_interleave(_dev(a), _dev(lane_b), alpha)
                 assert np.array_equal(_np(got), oracle.stride_interleave(a, lane_b, alpha)), (n, alpha)
     n = 1_700_000  # the admitted-bitmap no longer fits shared memory: global-memory bitmap
