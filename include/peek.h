@@ -34,7 +34,11 @@
  *              anything is enqueued.  Contents of device arrays are trusted (monotone offsets,
  *              valid child indices, >= 1 EMPTY table slot) and not validated.
  *   Sizes      N = 0 is PEEK_OK and touches nothing.  N < 2^31 - 1.  block_size must be 16
- *              (every config) else PEEK_ERR_UNSUPPORTED.
+ *              (every config) else PEEK_ERR_UNSUPPORTED.  The element counts of
+ *              `tokens` and `hashes` live on the device (tok_off[N], blk_off[N]), so the host
+ *              checks cannot see them: an array that a requested output needs must be non-NULL
+ *              even when it holds no element (a queue without a full block has NB = 0); it is
+ *              then never read.
  *   Aliasing   inputs and outputs never alias each other or `ws`.
  *   Determinism outputs are a pure function of the inputs (no dependence on atomics order).
  *   There is no CPU fallback anywhere in this library.

@@ -120,6 +120,23 @@ def _ptr(t: Optional[torch.Tensor], dtype=None):
     return ctypes.c_void_p(t.data_ptr())
 
 
+_dummies = {}
+
+
+def _hptr(t: Optional[torch.Tensor]):
+    """Pointer to a hash array.  A queue without a single full block has NB = 0 and an empty tensor,
+    whose data pointer is NULL; the library wants a non-NULL `hashes` whenever an output needs the
+    chains, so such a tensor is passed as a one-element dummy that is never read."""
+    if t is None:
+        return None
+    if t.numel() == 0:
+        key = (t.device.type, t.device.index)
+        if key not in _dummies:
+            _dummies[key] = torch.zeros(1, dtype=U64, device=t.device)
+        return _ptr(_dummies[key])
+    return _ptr(t, U64)
+
+
 def _stream():
     return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
 
@@ -207,7 +224,7 @@ def peek_pending_tree(hashes: torch.Tensor, blk_off: torch.Tensor, signals: bool
                     torch.zeros(1, dtype=torch.int32, device=dev))
     ws, nbytes = _ws(CALL_PENDING_TREE, dev, N=N)
     sig = (lambda x: _ptr(x)) if signals else (lambda x: None)
-    st = lib().peek_pending_tree(_ptr(hashes, U64) if hashes.numel() else None, _ptr(blk_off, torch.int64),
+    st = lib().peek_pending_tree(_hptr(hashes), _ptr(blk_off, torch.int64),
                                  N, _ptr(t.order), _ptr(t.lcp), sig(t.group_id), sig(t.group_size),
                                  sig(t.cluster_depth), sig(t.cluster_size), sig(t.cluster_id),
                                  sig(t.n_groups), _ptr(ws), nbytes, _stream())
@@ -233,7 +250,7 @@ def peek_lpm(tokens=None, tok_off=None, hashes=None, blk_off=None, radix: Option
     if tokens is not None and tokens.numel() == 0:  # all requests empty: still a valid pointer
         tokens = torch.zeros(4, dtype=torch.int32, device=dev)
     st = lib().peek_lpm(_ptr(tokens), _ptr(tok_off),
-                        _ptr(hashes) if hashes is not None and hashes.numel() else None, _ptr(blk_off), N,
+                        _hptr(hashes), _ptr(blk_off), N,
                         block_size, ctypes.byref(cr) if cr is not None else None,
                         ctypes.byref(ct) if ct is not None else None,
                         ctypes.byref(cv) if cv is not None else None, _ptr(hr), _ptr(hh), _ptr(ws), nbytes,
@@ -257,7 +274,7 @@ def peek_demand_rank(hashes=None, blk_off=None, tree: Optional[PendingTree] = No
     out = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N] if want_order else None
     ct = _Table(_ptr(t_keys, U64), S) if t_keys is not None else None
     ws, nbytes = _ws(CALL_DEMAND_RANK, dev, N=N, S=S)
-    st = lib().peek_demand_rank(_ptr(hashes) if hashes is not None and hashes.numel() else None,
+    st = lib().peek_demand_rank(_hptr(hashes),
                                 _ptr(blk_off), N, _ptr(tree.order) if tree is not None else None,
                                 _ptr(tree.lcp) if tree is not None else None,
                                 ctypes.byref(ct) if ct is not None else None, _ptr(hit), _ptr(cluster_size),
@@ -282,7 +299,7 @@ def peek_clpm_signals(hashes, blk_off, tree: PendingTree, hit: Optional[torch.Te
     evict = torch.empty(S, dtype=torch.int64, device=dev) if want_evict else None
     ct = _Table(_ptr(t_keys, U64), S) if t_keys is not None else None
     ws, nbytes = _ws(CALL_CLPM_SIGNALS, dev, N=N, S=S)
-    st = lib().peek_clpm_signals(_ptr(hashes) if hashes is not None and hashes.numel() else None, _ptr(blk_off), N,
+    st = lib().peek_clpm_signals(_hptr(hashes), _ptr(blk_off), N,
                                  _ptr(tree.order), _ptr(tree.lcp), _ptr(hit), int(tau), _ptr(arrival),
                                  ctypes.byref(ct) if ct is not None else None, _ptr(section), _ptr(score),
                                  _ptr(evict), _ptr(ws), nbytes, _stream())
@@ -328,7 +345,7 @@ def peek_pending_tree_update(hashes, blk_off, M: int, old: PendingTree, remap, s
     nb = ctypes.c_int64(0)
     _check(L.peek_workspace_bytes(CALL_PENDING_TREE_UPDATE, N, N_old, int(M), 0, 0, ctypes.byref(nb)), "peek_workspace_bytes")
     ws = torch.empty(max(int(nb.value), 256), dtype=torch.uint8, device=dev)
-    st = L.peek_pending_tree_update(_ptr(hashes) if hashes is not None and hashes.numel() else None, _ptr(blk_off),
+    st = L.peek_pending_tree_update(_hptr(hashes), _ptr(blk_off),
                                     N, int(M), _ptr(old.order), _ptr(old.lcp), N_old, _ptr(remap),
                                     _ptr(t.order), _ptr(t.lcp), _ptr(t.group_id), _ptr(t.group_size),
                                     _ptr(t.cluster_depth), _ptr(t.cluster_size), _ptr(t.cluster_id), _ptr(t.n_groups),
@@ -379,7 +396,9 @@ def peek_radix_demand(tokens, tok_off, radix: Radix, hit_radix):
     V = int(radix.n_tok_len.shape[0])
     out = torch.empty(V, dtype=torch.int32, device=tok_off.device)
     cr = radix._c()
-    st = lib().peek_radix_demand(_ptr(tokens) if tokens is not None and tokens.numel() else None, _ptr(tok_off), N,
+    if tokens is not None and tokens.numel() == 0:  # all requests empty: still a valid pointer
+        tokens = torch.zeros(4, dtype=torch.int32, device=tok_off.device)
+    st = lib().peek_radix_demand(_ptr(tokens), _ptr(tok_off), N,
                                  ctypes.byref(cr), _ptr(hit_radix), _ptr(out), _stream())
     _check(st, "peek_radix_demand")
     return out
@@ -393,7 +412,7 @@ def peek_offline_phase1(hashes, blk_off, depth_blocks: int = 8):
     order = torch.empty(max(N, 1), dtype=torch.int32, device=dev)[:N]
     guards = torch.zeros(4, dtype=torch.float64, device=dev)
     ws, nbytes = _ws(CALL_OFFLINE_PHASE1, dev, N=N)
-    st = lib().peek_offline_phase1(_ptr(hashes) if hashes is not None and hashes.numel() else None, _ptr(blk_off),
+    st = lib().peek_offline_phase1(_hptr(hashes), _ptr(blk_off),
                                    N, int(depth_blocks), _ptr(order), _ptr(guards), _ptr(ws), nbytes, _stream())
     _check(st, "peek_offline_phase1")
     return order, guards

@@ -435,6 +435,59 @@ def test_pending_tree_update_matches_rebuild():
         assert np.array_equal(_np(tree.cluster_size), want.cluster_size), cycle
 
 
+def _random_case(seed):
+    """A random prefix forest of token segments and a queue drawn from it: exact nodes, prefixes of
+    nodes, nodes with random tails; vocab 2 .. 128256 (tiny vocab = collisions at every depth),
+    queue sizes around the one-CTA limit (1024) and the tile size (8192), a cache of random nodes
+    and requests (possibly empty), arrival a permutation or NULL."""
+    rng = np.random.default_rng(seed)
+    vocab = int(rng.choice([2, 3, 5, 50, 128256]))
+    n = int(rng.choice([1, 2, 7, 33, 200, 1023, 1024, 1025, 3000, 8191, 8193, 20000]))
+    levels, fan = int(rng.integers(1, 6)), int(rng.integers(1, 9))
+    seg = int(rng.choice([1, 5, 16, 17, 40, 200]))
+    nodes, frontier = [np.zeros(0, np.int32)], [0]
+    for _ in range(levels):
+        nxt = []
+        for p in frontier:
+            for _ in range(int(rng.integers(1, fan + 1))):
+                s = rng.integers(0, vocab, size=int(rng.integers(1, seg + 1))).astype(np.int32)
+                nodes.append(np.concatenate([nodes[p], s]))
+                nxt.append(len(nodes) - 1)
+        frontier = nxt[:4000]
+    reqs = []
+    for _ in range(n):
+        base = nodes[int(rng.integers(0, len(nodes)))]
+        mode = int(rng.integers(0, 4))
+        if mode == 0:
+            r = base
+        elif mode == 1:
+            r = base[: int(rng.integers(0, len(base) + 1))]
+        else:
+            r = np.concatenate([base, rng.integers(0, vocab, size=int(rng.integers(0, 3 * seg))).astype(np.int32)])
+        reqs.append(r.astype(np.int32))
+    toks, off = _csr(reqs)
+    ncache = int(rng.integers(0, min(len(nodes), 300) + 1))
+    cached = [nodes[int(i)] for i in rng.integers(0, len(nodes), size=ncache) if len(nodes[int(i)])]
+    cached += [reqs[int(i)] for i in rng.integers(0, n, size=int(rng.integers(0, 20))) if len(reqs[int(i)])]
+    if cached:
+        nblk = sum(len(c) // 16 for c in cached) + 8
+        radix, t_keys = _cache_from(cached, 1 << int(np.ceil(np.log2(2 * nblk + 2))))
+    else:
+        radix, _ = W.build_radix(None, 16, 0)
+        t_keys = np.full(64, W.EMPTY, dtype=np.uint64)
+    arrival = rng.permutation(n).astype(np.int32) if rng.integers(0, 2) else None
+    return toks, off, radix, t_keys, arrival
+
+
+@pytest.mark.parametrize("seed0", [0, 40, 80])
+def test_random_forests(seed0):
+    """40 random cases per parameter through the whole pipeline (every call, every LPM strategy),
+    bit-exact against the oracle.  Seeds 1 and 34 are queues without a single full block / without a
+    single token (NB = 0, T = 0: empty hash and token arrays)."""
+    for seed in range(seed0, seed0 + 40):
+        run_pipeline(*_random_case(seed))
+
+
 def test_stride_interleave_cases():
     """Identical lanes (every candidate clashes), reversed lanes, locally shuffled lanes (clashes in
     most steps, resolved in time order), alpha 0, 1 and next to 1, a queue shorter than one step,
