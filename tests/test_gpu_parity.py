@@ -488,6 +488,32 @@ def test_random_forests(seed0):
         run_pipeline(*_random_case(seed))
 
 
+def test_random_forest_updates():
+    """peek_pending_tree_update on 60 random forests: a random share of the queue removed (none,
+    2 %, half, 98 %, all) and 0 .. N + 3 arrivals (copies, prefixes, extensions, unrelated chains)."""
+    b = _b()
+    for seed in range(60):
+        rng = np.random.default_rng(10_000 + seed)
+        toks, off, _, _, _ = _random_case(seed)
+        reqs = [toks[off[i]:off[i + 1]].copy() for i in range(len(off) - 1)]
+        n = len(reqs)
+        keep = rng.random(n) >= float(rng.choice([0.0, 0.02, 0.5, 0.98, 1.0]))
+        m = min(int(rng.choice([0, 1, 5, 100, max(1, n // 2), n + 3])), 6000)
+        arr = []
+        for _ in range(m):
+            base = reqs[int(rng.integers(0, n))]
+            kind = int(rng.integers(0, 4))
+            if kind == 0:
+                arr.append(base.copy())
+            elif kind == 1:
+                arr.append(base[: int(rng.integers(0, len(base) + 1))].copy())
+            elif kind == 2:
+                arr.append(np.concatenate([base, rng.integers(0, 3, size=int(rng.integers(1, 40)))]).astype(np.int32))
+            else:
+                arr.append(rng.integers(0, 3, size=int(rng.integers(0, 100))).astype(np.int32))
+        _update_case(b, reqs, keep, arr)
+
+
 def test_stride_interleave_cases():
     """Identical lanes (every candidate clashes), reversed lanes, locally shuffled lanes (clashes in
     most steps, resolved in time order), alpha 0, 1 and next to 1, a queue shorter than one step,
