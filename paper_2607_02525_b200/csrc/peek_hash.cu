@@ -111,7 +111,11 @@ static constexpr int HF_THREADS = HF_WARPS * 32;
 static constexpr int HF_STAGES = PEEK_HF_STAGES;
 static constexpr int HF_STAGE_BYTES = 2176;          // 2048 + 16 rounded up to a multiple of 128
 static constexpr int HF_CROW = 33;                   // c-buffer row pitch in u64 (32 + 1: no conflicts)
-static constexpr int HF_WARP_BYTES = HF_STAGES * HF_STAGE_BYTES + 32 * HF_CROW * 8 + 64;
+#ifndef PEEK_HF_LANES
+#define PEEK_HF_LANES 32
+#endif
+static constexpr int HF_LANES = PEEK_HF_LANES;       // owning lanes (requests) per warp = c-buffer rows
+static constexpr int HF_WARP_BYTES = HF_STAGES * HF_STAGE_BYTES + HF_LANES * HF_CROW * 8 + 64;
 static constexpr int HF_SMEM_BYTES = HF_WARPS * HF_WARP_BYTES + 128;
 
 __device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
@@ -216,7 +220,7 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
     unsigned char* wbase = hf_smem + (size_t)wid * HF_WARP_BYTES;
     const u32 stage0 = smem_u32(wbase);
     u64* cbuf = (u64*)(wbase + HF_STAGES * HF_STAGE_BYTES);
-    const u32 bar0 = smem_u32(wbase + HF_STAGES * HF_STAGE_BYTES + 32 * HF_CROW * 8);
+    const u32 bar0 = smem_u32(wbase + HF_STAGES * HF_STAGE_BYTES + HF_LANES * HF_CROW * 8);
     if (lane == 0) {
 #pragma unroll
         for (int s = 0; s < HF_STAGES; ++s) mbar_init(bar0 + 8 * s, 1);
@@ -444,7 +448,7 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
         }
         i64 per_warp = (N + warps - 1) / warps;
         HashArgs A{tokens, tok_off, blk_off, N, seed, hashes, hashes_capacity, counter,
-                   (int)(per_warp < 1 ? 1 : (per_warp > 32 ? 32 : per_warp))};
+                   (int)(per_warp < 1 ? 1 : (per_warp > HF_LANES ? HF_LANES : per_warp))};
         Prof pr(PROF_HASH_CONTENT, st, 1);
         k_block_hash_fused<<<grid, HF_THREADS, HF_SMEM_BYTES, st>>>(A);
     }
