@@ -298,8 +298,13 @@ peek_status peek_offline_phase1(const uint64_t* hashes, const int64_t* blk_off, 
  * PEEK_OPT_GRID_LIMIT    cap on the CTAs of the persistent (cooperative) kernels of
  *                        peek_pending_tree and peek_demand_rank; 0 = one per SM (default).  A test
  *                        hook: a small cap makes every CTA loop over several tiles at small N.
+ * PEEK_OPT_TREE_LOCAL_CAP  peek_pending_tree: the largest unresolved segment (in sorted positions) that
+ *                        one CTA finishes out of shared memory; larger ones go through another
+ *                        grid-wide refinement round first.  0 = the built-in capacity (default);
+ *                        values 128 .. capacity lower it (a test hook: the grid-wide rounds and the
+ *                        work-item queues then run at small N).
  * Unknown key or bad value -> PEEK_ERR_INVALID_ARG. */
-enum { PEEK_OPT_LPM_STRATEGY = 1, PEEK_OPT_LPM_WINDOW = 2, PEEK_OPT_GRID_LIMIT = 3 };
+enum { PEEK_OPT_LPM_STRATEGY = 1, PEEK_OPT_LPM_WINDOW = 2, PEEK_OPT_GRID_LIMIT = 3, PEEK_OPT_TREE_LOCAL_CAP = 4 };
 enum { PEEK_LPM_AUTO = 0, PEEK_LPM_DUAL_WALK = 1, PEEK_LPM_SPECULATIVE = 2 };
 peek_status peek_set_option(int32_t key, int64_t value);
 

@@ -14,7 +14,8 @@ from typing import Optional
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpeek.so")
+# PEEK_LIB selects another build of the same library (the checked build, a traced build)
+LIB_PATH = os.environ.get("PEEK_LIB") or os.path.join(_HERE, "libpeek.so")
 _lib = None
 
 CALL_BLOCK_HASH, CALL_LPM, CALL_PENDING_TREE, CALL_DEMAND_RANK = 0, 1, 2, 3
@@ -418,7 +419,7 @@ def peek_offline_phase1(hashes, blk_off, depth_blocks: int = 8):
     return order, guards
 
 
-OPT_LPM_STRATEGY, OPT_LPM_WINDOW, OPT_GRID_LIMIT = 1, 2, 3
+OPT_LPM_STRATEGY, OPT_LPM_WINDOW, OPT_GRID_LIMIT, OPT_TREE_LOCAL_CAP = 1, 2, 3, 4
 LPM_AUTO, LPM_DUAL_WALK, LPM_SPECULATIVE = 0, 1, 2
 
 

@@ -2,6 +2,9 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <mutex>
+#include <vector>
+
 #include "peek_common.cuh"
 
 namespace peek {
@@ -24,6 +27,21 @@ static int g_grid_limit = 0;  // PEEK_OPT_GRID_LIMIT
 int persistent_ctas() {       // CTAs of a persistent cooperative kernel: one per SM unless capped
     int n = sm_count();
     return (g_grid_limit > 0 && g_grid_limit < n) ? g_grid_limit : n;
+}
+
+cudaError_t func_smem_optin(const void* func, int bytes) {
+    struct Done { int dev; const void* func; int bytes; };
+    static std::mutex mu;
+    static std::vector<Done> done;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    for (const Done& d : done)
+        if (d.dev == dev && d.func == func && d.bytes >= bytes) return cudaSuccess;
+    e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) done.push_back(Done{dev, func, bytes});
+    return e;
 }
 
 int sm_count() {
@@ -77,6 +95,7 @@ i64 group_major_ws_bytes(i64 N);
 i64 offline_phase1_ws_bytes(i64 N);
 i64 pending_tree_update_ws_bytes(i64 N_old, i64 N_new, i64 M);
 void lpm_set_option(int key, i64 v);
+void tree_set_option(int key, i64 v);
 
 }  // namespace peek
 
@@ -129,6 +148,10 @@ extern "C" peek_status peek_set_option(int32_t key, int64_t value) {
     if ((key == PEEK_OPT_LPM_STRATEGY && value >= 0 && value <= 2) ||
         (key == PEEK_OPT_LPM_WINDOW && value >= 0 && value <= (1 << 20))) {
         peek::lpm_set_option(key, value);
+        return PEEK_OK;
+    }
+    if (key == PEEK_OPT_TREE_LOCAL_CAP && value >= 0 && value <= (1 << 20)) {
+        peek::tree_set_option(key, value);
         return PEEK_OK;
     }
     if (key == PEEK_OPT_GRID_LIMIT && value >= 0 && value <= 65536) {

@@ -20,6 +20,9 @@ void set_error(const char* fmt, ...);
 peek_status cuda_fail(cudaError_t e, const char* what);
 int sm_count();  // SMs of the current device (148 on B200)
 int persistent_ctas();  // grid of the persistent cooperative kernels (PEEK_OPT_GRID_LIMIT)
+// opt `func` in to `bytes` of dynamic shared memory on the CURRENT device (the attribute belongs to the
+// device's context, so it is remembered per device; thread-safe)
+cudaError_t func_smem_optin(const void* func, int bytes);
 
 // tracing slots (peek_profile_*)
 enum ProfSlot {

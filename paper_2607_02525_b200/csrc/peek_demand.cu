@@ -496,11 +496,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
         PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(RANK_MAX_GRID)) - (char*)A.ctl), st));
         void* params[] = {&A};
         Prof pr(PROF_RANK, st, 1);
-        static bool attr_set = false;
-        if (!attr_set) {
-            PEEK_CUDA(cudaFuncSetAttribute(k_clpm_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
-            attr_set = true;
-        }
+        PEEK_CUDA(func_smem_optin((const void*)k_clpm_sort, GS_STAGE_BYTES));
         PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort, dim3(grid), dim3(GS_THREADS), params,
                                               GS_STAGE_BYTES, st));
     }
@@ -516,11 +512,7 @@ static peek_status launch_sort_full(FullArgs& A, i64 N, void* ws, cudaStream_t s
     i64 want = (N + GS_THREADS - 1) / GS_THREADS;
     if (want < grid) grid = (int)(want < 1 ? 1 : want);
     PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(1024)) - (char*)A.ctl), st));
-    static bool attr_set = false;
-    if (!attr_set) {
-        PEEK_CUDA(cudaFuncSetAttribute(k_clpm_sort_full, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
-        attr_set = true;
-    }
+    PEEK_CUDA(func_smem_optin((const void*)k_clpm_sort_full, GS_STAGE_BYTES));
     void* params[] = {&A};
     Prof pr(PROF_RANK_FULL, st, 1);
     PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort_full, dim3(grid), dim3(GS_THREADS), params,
@@ -625,11 +617,7 @@ extern "C" peek_status peek_clpm_group_major(const int32_t* lane_order, const in
     if (want < grid) grid = (int)(want < 1 ? 1 : want);
     PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(1024)) - (char*)A.ctl), st));
     PEEK_CUDA(cudaMemsetAsync(A.tkeys, 0xff, (size_t)((char*)(A.tfirst + (A.hmask + 1)) - (char*)A.tkeys), st));
-    static bool attr_set = false;
-    if (!attr_set) {
-        PEEK_CUDA(cudaFuncSetAttribute(k_group_major, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
-        attr_set = true;
-    }
+    PEEK_CUDA(func_smem_optin((const void*)k_group_major, GS_STAGE_BYTES));
     void* params[] = {&A};
     Prof pr(PROF_RANK_FULL, st, 1);
     PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_group_major, dim3(grid), dim3(GS_THREADS), params,

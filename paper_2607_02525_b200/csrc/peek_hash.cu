@@ -434,12 +434,7 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
         k_nb_apply<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial, blk_off);
     }
     if (hashes_capacity > 0) {
-        static bool attr_set = false;
-        if (!attr_set) {
-            PEEK_CUDA(cudaFuncSetAttribute(k_block_hash_fused, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           HF_SMEM_BYTES));
-            attr_set = true;
-        }
+        PEEK_CUDA(func_smem_optin((const void*)k_block_hash_fused, HF_SMEM_BYTES));
         int grid = sm_count();
         i64 warps = (i64)grid * HF_WARPS;
         if (N < warps) {  // fewer requests than warps: no point in idle CTAs

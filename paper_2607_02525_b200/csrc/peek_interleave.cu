@@ -346,12 +346,7 @@ extern "C" peek_status peek_stride_interleave(const int32_t* lane_a, const int32
         set_error("peek_stride_interleave: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        PEEK_CUDA(cudaFuncSetAttribute(k_stride_interleave, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)(sizeof(SiSmem) + SI_SMEM_BITS)));
-        attr_set = true;
-    }
+    PEEK_CUDA(func_smem_optin((const void*)k_stride_interleave, (int)(sizeof(SiSmem) + SI_SMEM_BITS)));
     cudaStream_t st = (cudaStream_t)stream;
     Prof pr(PROF_RANK_FULL, st, 1);
     k_stride_interleave<<<1, SI_T, sizeof(SiSmem) + (use_smem ? (size_t)bytes : 0), st>>>(lane_a, lane_b, N, alpha, out, (u32*)ws,

@@ -214,11 +214,7 @@ extern "C" peek_status peek_offline_phase1(const uint64_t* hashes, const int64_t
     if (cgrid > 1024) cgrid = 1024;
     i64 want = (N + GS_THREADS - 1) / GS_THREADS;
     if (want < cgrid) cgrid = (int)(want < 1 ? 1 : want);
-    static bool attr_set = false;
-    if (!attr_set) {
-        PEEK_CUDA(cudaFuncSetAttribute(k_offline_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
-        attr_set = true;
-    }
+    PEEK_CUDA(func_smem_optin((const void*)k_offline_sort, GS_STAGE_BYTES));
     void* params[] = {&A};
     PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_offline_sort, dim3(cgrid), dim3(GS_THREADS), params,
                                           GS_STAGE_BYTES, st));

@@ -2,14 +2,23 @@
 // a batch: lexicographic order of the requests' hash chains (= DFS order of the compressed trie),
 // adjacent LCP (= its branching depths), flat groups and per-request clusters.
 //
-// ONE persistent cooperative kernel (one CTA of GS_THREADS per SM, grid barriers between phases),
-// because the number of refinement rounds is data dependent and the call may not synchronise with
-// the host.  The pairs (sort key, request) are kept BY POSITION and go through peek_sort.cuh's
-// key/value sort; every phase walks the CTA's own chunk of positions in register tiles.
+// ONE persistent cooperative kernel (one CTA of GS_THREADS per SM), in two stages:
+//   GLOBAL stage - grid-wide partition.  Round 0 sorts the requests by the leading bits of their
+//     first hash word (stable LSD pair sort of peek_sort.cuh); further grid-wide rounds of the
+//     refinement below run only while some unresolved segment is larger than what one CTA can
+//     finish alone (cap_seg positions).
+//   LOCAL stage - every unresolved segment (a run of sorted positions whose chains share a prefix
+//     and are not ordered yet) is finished by ONE CTA out of shared memory: all further refinement
+//     rounds, their sorts and their scans cost CTA barriers instead of grid barriers, and
+//     segments are independent, so the tail of one does not hold up the others.  Work items are
+//     handed out through two atomic queues (big segments first, then fixed quanta of positions
+//     holding the small ones); which CTA takes which item never changes a result.
+//   Queues of at most LOC_CAP requests (the paper's hold 60-200) run in one CTA from
+//   the first step on and see no grid barrier at all.
 //
-// Sort = path-peeling refinement.  Every unresolved segment (a run of sorted positions whose
-// chains share a prefix) picks its LONGEST chain as head h.  A member r is classified by its
-// LCP with h in units of w-bit digits (a 64-bit hash word = D digits, most significant first):
+// Refinement = path peeling.  Every unresolved segment picks its LONGEST chain as head h.  A member
+// r is classified by its LCP with h in units of w-bit digits (a 64-bit hash word = D digits, most
+// significant first):
 //     r proper prefix of h            -> before h, by ascending LCP, "ended" (identical chains)
 //     r's digit < h's at the LCP      -> before h, by ascending LCP, then digit
 //     r identical to h                -> with h
@@ -17,24 +26,61 @@
 // One stable LSD radix sort by key = [segment rank | class+LCP | digit] splits the segment along
 // the whole root-to-leaf path of h at once, so rounds ~ 3 on the paper's workloads (shared
 // prompt / conversation / turn) instead of one per trie level; only the key bits that vary are
-// sorted on.  LCPs with the head use the chain property (k_i equal => all earlier words equal,
-// DESIGN.md R15) to bisect for the first differing word; the probes are random 32-byte sectors of
-// the hash array (the phase is HBM-transaction bound), so a warp row lets one lane bisect and the
-// others verify its answer with one probe pair (lcp_lockstep).
+// sorted on.  Round 0 is the same thing against a virtual head that is smaller than every chain
+// (class "after, LCP 0", digit = leading bits of the first word): no head, no probes.
+// LCPs with the head use the chain property (k_i equal => all earlier words equal, R15)
+// to bisect for the first differing word; the probes are random 32-byte sectors of the hash
+// array, so a lane first tries the answer of its previous element, then one lane per warp row
+// bisects and the others verify its answer with one probe pair (lcp_lockstep).
 // The ADJACENT LCP (output `lcp`) costs no chain reads at all: when a sort splits two neighbours
 // that came from one segment, they leave the old head's path at known digit depths, and
-// min(depths) / D is exactly their LCP (R1a); neighbours never split have identical chains.
+// min(depths) / D is exactly their LCP; neighbours never split have identical chains.
 #include "peek_sort.cuh"
 
 namespace peek {
+
+#ifndef PEEK_LOC_K
+#define PEEK_LOC_K 11
+#endif
+static constexpr int LOC_K = PEEK_LOC_K;              // positions per thread of a local work item
+static constexpr int LOC_CAP = GS_THREADS * LOC_K;    // positions one CTA refines out of shared memory
+static constexpr int TREE_DYN_SMEM = LOC_CAP * 18;    // u64 key + u32 request + 3 x u16 per position
+static_assert(TREE_DYN_SMEM >= GS_STAGE_BYTES, "the grid sort stages its tiles in the same buffer");
+static_assert(LOC_CAP <= 32768, "local positions are kept in 15 bits of a u16");
+static constexpr int W0_BITS = 16;                    // round 0: leading bits of the first hash word
+static constexpr int LOC_W = 16;                      // digit width of the local stage's keys
 
 struct TreeCtl {      // device control block (zeroed by the host before launch)
     u32 bar;          // grid barrier word
     u32 unres[3];     // unresolved-position counters, rotating
     u32 maxnb;        // max chain length in blocks
-    u32 pad[3];
+    u32 flags;        // bit 0: some chain is empty (no full block)
+    u32 maxseg[3];    // size of the largest unresolved segment, rotating
+    u32 nbig[3];      // entries of the big-segment list, rotating
+    u32 next_big, next_q;  // work queues of the local stage
+    u32 bar2;              // grid barrier word of the signals kernel
+    u32 fin_cb, fin_round; // where the grid-wide stage stopped: pair buffer, round (counter index)
+    u32 pad[2];
     unsigned long long kor[2], kand[2];  // OR / AND of the round's keys (rotating): varying bits
 };
+
+// per-request record, one 32-byte sector: everything a refinement round wants to know about a chain
+// without touching the hash array (gathered by request id, so it is packed to cost ONE sector)
+struct __align__(32) ReqRec {
+    i64 ao;     // blk_off[r]
+    u32 na;     // chain length in blocks
+    u32 pad;
+    u64 lasth;  // last word of the chain (0 for an empty chain): "does one chain prefix the other"
+    u64 k0;     // first word (0 for an empty chain): the first unknown word of a segment at depth 0
+};
+__device__ __forceinline__ void rec_head(const ReqRec* __restrict__ rec, u32 r, i64& ao, i32& na) {
+    const ulonglong2 v = __ldg((const ulonglong2*)(rec + r));
+    ao = (i64)v.x; na = (i32)(u32)v.y;
+}
+__device__ __forceinline__ void rec_tail(const ReqRec* __restrict__ rec, u32 r, u64& lasth, u64& k0) {
+    const ulonglong2 v = __ldg((const ulonglong2*)(rec + r) + 1);
+    lasth = v.x; k0 = v.y;
+}
 
 struct TreeArgs {
     const u64* hashes;
@@ -44,16 +90,19 @@ struct TreeArgs {
     i64* cluster_id;
     i32* n_groups;
     int signals_only;  // order and lcp are given: only groups and clusters are computed
+    int cap_seg;       // an unresolved segment of at most this many positions goes to the local stage
+    int quantum;       // positions per small-segment work item; segments above it are items of their own
     // workspace
     TreeCtl* ctl;
     GsBufs bufs;      // (sort key, request) by position, ping-pong
     u32* seg;         // N   by position: segment start | unresolved << 31
-    u32* srank;       // N   by position: dense rank of the segment (the sort key's leading field)
-    u64* lasth;       // N   by request: last word of its chain (read once; every round's first probe)
+    u32* srank;       // N   by position (global rounds) / by segment start (local): dense segment rank
+    ReqRec* rec;      // N   by request (phase 0)
     u64* seghead;     // N   by segment start: (nb << 32) | ~position of the longest chain
     i32* segdepth;    // N   by segment start: blocks all members are known to share
     i64* agg;         // gridDim scratch for grid scans
-    i32* gsz;         // N   group size by group id
+    i32* gsz;         // N   unresolved segment size by segment start; later group size by group id
+    u64* biglist;     // segments above the quantum: start | size << 32
     i32* mt_buf;      // min hierarchy
 };
 
@@ -95,10 +144,11 @@ struct KeyLayout {
     }
 };
 
-__device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb) {
+// wmax caps the digit width (the local stage sorts on narrower digits)
+__device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb, int wmax) {
     KeyLayout kl;
     kl.sbits = bits_for((u64)(N > 1 ? N - 1 : 1));
-    for (int w = 32; w >= 1; --w) {
+    for (int w = wmax; w >= 1; --w) {
         int D = (64 + w - 1) / w;
         u64 LDmax = (u64)D * maxnb + D;
         int lbits = bits_for(3 * LDmax + 4);
@@ -108,9 +158,26 @@ __device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb) {
     kl.total = kl.sbits + kl.lbits + kl.w;
     return kl;
 }
+// The narrowest layout (w = 1: D = 64, LDmax = 64 maxnb + 64, lbits <= bits(192 maxnb + 196)) needs
+// sbits + lbits + 1 <= 64; with N < 2^31 (sbits <= 31) that holds for every maxnb < 2^24, i.e.
+// chains of up to 2.6e8 tokens.  The entry point rejects longer chains (PEEK_ERR_UNSUPPORTED is
+// reported through the status word; see tree_launch).
+
+// round-0 key of a request: d0 = (leading W0_BITS of its first word) | 1 << 31, or 0 for an empty chain
+__device__ __forceinline__ u64 round0_key(const KeyLayout& kl, u32 d0) {
+    const int w0 = kl.w < W0_BITS ? kl.w : W0_BITS;
+    return (d0 >> 31) ? kl.pack(0, kl.f_after(0), (u64)((d0 & 0xffffu) >> (W0_BITS - w0)))
+                      : kl.pack(0, kl.f_before(0, true), 0);
+}
+__device__ __forceinline__ u64 round0_vary(const KeyLayout& kl, u32 flags) {
+    const int w0 = kl.w < W0_BITS ? kl.w : W0_BITS;
+    u64 v = (1ull << w0) - 1;
+    if (flags & 1u) v |= (kl.f_after(0) ^ kl.f_before(0, true)) << kl.w;
+    return v;
+}
 
 // ---- staged tile processing ---------------------------------------------------------------------
-// Every phase walks the CTA's chunk of positions (the sort engine's ownership: CTA c owns
+// Every grid-wide phase walks the CTA's chunk of positions (the sort engine's ownership: CTA c owns
 // [c0, c1), element (t, k) of thread (w, lane) is c0 + t*GS_TILE + w*32*GS_KPT + k*32 + lane) with
 // GS_KPT elements per thread held in registers, and is written stage by stage: all loads of a
 // stage are issued for the GS_KPT elements before any is used, so a phase costs (dependent stages)
@@ -122,29 +189,43 @@ __device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb) {
 #endif
 static constexpr int SB = PEEK_SB;
 #define SUBS(k) _Pragma("unroll") for (int k = 0; k < SB; ++k)
+#ifndef PEEK_LSB
+#define PEEK_LSB 1
+#endif
+static constexpr int LSB = PEEK_LSB;  // sub-batch of the local stage's classification
+static_assert(LOC_K % LSB == 0, "LOC_K must be a multiple of LSB");
+#define LSUBS(k) _Pragma("unroll") for (int k = 0; k < LSB; ++k)
 
 struct TreeSmem {
     i32 wv[GS_WARPS + 1];   // per-warp values of the carry chains
     i64 wv64[GS_WARPS + 1];
     i64 carry64;
     i32 carry;
-    i32 lvl_hi[2048 + 64 + 8];  // per-CTA copy of the min-hierarchy levels >= 3
+    u32 cnt, item, red;
+    unsigned long long orv, andv;
 };
+static constexpr int LVL_HI_WORDS = 2048 + 64 + 8;  // per-CTA copy of the min-hierarchy levels >= 3
 
 // LCP of K pairs of chains in lock step: chains H[ao..ao+na), H[bo..bo+nb), first lo words known
 // equal (chain property R15: equal at a depth => equal above it, so the first difference is found
 // by bisection).  act[k] selects the pairs to do; others keep res[k].
-// Probes are random 32-byte sectors of a multi-GB array (the phase is bound by HBM transactions,
-// not latency), so the search is organised to need few of them: (1) the last common word (one chain
-// prefixes the other: done); (2) per warp row, ONE lane bisects and its answer g is the guess of
-// the others (neighbours in sorted order mostly branch off their head at the same depth), who
-// probe words g-1 and g - usually one sector - and (3) bisect on only if that did not settle it.
-// HINT = false skips (2).  Must be called by full warps (uses warp collectives).
-template <int K, bool HINT>
+// Probes are random 32-byte sectors of a multi-GB array and the phase is bound by how many of them
+// the memory system serves, so the search spends as few as it can:
+//   (1) the last common word - one chain prefixes the other: done (the member's side comes from
+//       its record, the head's chain is shared by the segment);
+//   (2) the first unknown word (at depth 0 both first words are in the records: no read) together
+//       with `hint`, the answer of this lane's previous element - neighbours in sorted order mostly
+//       branch off their head at the same depth: one probe pair settles them;
+//   (3) per warp row, ONE lane bisects and its answer g is the guess of the others, who probe
+//       words g-1 and g; (4) whoever is still open bisects on.
+// Must be called by full warps.
+template <int K>
 __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i64 (&ao)[K], const i32 (&na)[K],
                                              const i64 (&bo)[K], const i32 (&nb)[K], const i32 (&lo)[K],
-                                             const bool (&act)[K], i32 (&res)[K], bool probe_lo,
-                                             const u64 (&alast)[K]) {  // alast[k] = H[ao[k] + na[k] - 1]
+                                             const bool (&act)[K], i32 (&res)[K],
+                                             const u64 (&alast)[K],  // alast[k] = H[ao[k] + na[k] - 1]
+                                             const u64 (&k0a)[K], const u64 (&k0b)[K],  // first words
+                                             i32& hint) {            // in/out, < 0: none
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     i32 L[K], R[K];  // while go: equal below/at L (L = lo - 1: nothing known), differ at R
@@ -158,29 +239,46 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
         L[k] = lo[k] - 1;
         R[k] = m - 1;
     }
-    {   // first round trip: the last common word and - if the caller expects branches right at
-        // lo (first round) - the first unknown word with it
-        u64 x2[K], y2[K];
+    // (1) the last common word
 #pragma unroll
-        for (int k = 0; k < K; ++k) {
-            if (go[k]) {
-                x[k] = R[k] == na[k] - 1 ? alast[k] : __ldg(H + ao[k] + R[k]);
-                y[k] = __ldg(H + bo[k] + R[k]);
-                if (probe_lo) { x2[k] = __ldg(H + ao[k] + lo[k]); y2[k] = __ldg(H + bo[k] + lo[k]); }
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            if (go[k]) {
-                if (x[k] == y[k]) { res[k] = R[k] + 1; go[k] = false; }
-                else if (probe_lo) {
-                    if (x2[k] != y2[k]) { res[k] = lo[k]; go[k] = false; }
-                    else L[k] = lo[k];
-                }
-                if (go[k] && R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
-            }
+    for (int k = 0; k < K; ++k) {
+        if (go[k]) {
+            x[k] = R[k] == na[k] - 1 ? alast[k] : __ldg(H + ao[k] + R[k]);
+            y[k] = __ldg(H + bo[k] + R[k]);
         }
     }
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+        if (go[k] && x[k] == y[k]) { res[k] = R[k] + 1; go[k] = false; }
+    // probe words g - 1 and g of the pairs selected by pr[k] (one round trip): settles the pair when
+    // g is the answer.  first = also probe word lo (the first unknown word) in the same round trip.
+    auto probe_around = [&](const i32 (&gk)[K], const bool (&pr)[K], bool first) {
+        u64 x2[K], y2[K], x3[K], y3[K];
+        bool p0[K], p1[K], p2[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            p0[k] = first && go[k];
+            p1[k] = pr[k] && gk[k] - 1 > L[k] + (first ? 1 : 0) && gk[k] - 1 < R[k];
+            p2[k] = pr[k] && gk[k] > L[k] + (first ? 1 : 0) && gk[k] < R[k];
+            x3[k] = y3[k] = 0;
+            if (p0[k]) {
+                if (lo[k] == 0) { x3[k] = k0a[k]; y3[k] = k0b[k]; }
+                else { x3[k] = __ldg(H + ao[k] + lo[k]); y3[k] = __ldg(H + bo[k] + lo[k]); }
+            }
+            if (p1[k]) { x[k] = __ldg(H + ao[k] + gk[k] - 1); y[k] = __ldg(H + bo[k] + gk[k] - 1); }
+            if (p2[k]) { x2[k] = __ldg(H + ao[k] + gk[k]); y2[k] = __ldg(H + bo[k] + gk[k]); }
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            if (p0[k]) {
+                if (x3[k] != y3[k]) { res[k] = lo[k]; go[k] = false; p1[k] = p2[k] = false; }
+                else L[k] = lo[k];
+            }
+            if (p1[k]) { if (x[k] == y[k]) L[k] = gk[k] - 1; else R[k] = gk[k] - 1; }
+            if (p2[k] && gk[k] < R[k]) { if (x2[k] == y2[k]) L[k] = gk[k]; else R[k] = gk[k]; }
+            if (go[k] && (p0[k] || pr[k]) && R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
+        }
+    };
     // one bisection step for the elements selected by sel[k]; returns whether any is still going
     auto step = [&](const bool (&sel)[K]) -> bool {
 #pragma unroll
@@ -202,93 +300,442 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
         }
         return any;
     };
-    bool all_sel[K];
-#pragma unroll
-    for (int k = 0; k < K; ++k) all_sel[k] = true;
     bool pending = false;
 #pragma unroll
     for (int k = 0; k < K; ++k) pending |= go[k];
-    if (HINT && __any_sync(FULL, pending)) {
-        bool lead[K];
-        int leader[K];
+    if (__any_sync(FULL, pending)) {
+        {   // (2) the first unknown word and this lane's previous answer
+            i32 gk[K];
+            bool pr[K];
 #pragma unroll
-        for (int k = 0; k < K; ++k) {
-            const unsigned bal = __ballot_sync(FULL, go[k]);
-            leader[k] = bal ? __ffs(bal) - 1 : -1;
-            lead[k] = lane == leader[k];
+            for (int k = 0; k < K; ++k) { gk[k] = hint; pr[k] = go[k] && hint >= 0; }
+            probe_around(gk, pr, true);
+            pending = false;
+#pragma unroll
+            for (int k = 0; k < K; ++k) pending |= go[k];
         }
-        bool any = true;
-        while (__any_sync(FULL, any)) any = step(lead);
-        // the others probe around the leader's answer
+        if (__any_sync(FULL, pending)) {  // (3) one lane per row bisects, the others verify
+            bool lead[K];
+            int leader[K];
 #pragma unroll
-        for (int k = 0; k < K; ++k) {
-            const i32 gk = __shfl_sync(FULL, res[k], leader[k] < 0 ? 0 : leader[k]);
-            const bool pr = go[k] && leader[k] >= 0;
-            const bool p1 = pr && gk - 1 > L[k] && gk - 1 < R[k], p2 = pr && gk > L[k] && gk < R[k];
-            if (p1) { x[k] = __ldg(H + ao[k] + gk - 1); y[k] = __ldg(H + bo[k] + gk - 1); }
-            u64 x2 = 0, y2 = 0;
-            if (p2) { x2 = __ldg(H + ao[k] + gk); y2 = __ldg(H + bo[k] + gk); }
-            if (p1) { if (x[k] == y[k]) L[k] = gk - 1; else R[k] = gk - 1; }
-            if (p2 && gk < R[k]) { if (x2 == y2) L[k] = gk; else R[k] = gk; }
-            if (go[k] && R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
+            for (int k = 0; k < K; ++k) {
+                const unsigned bal = __ballot_sync(FULL, go[k]);
+                leader[k] = bal ? __ffs(bal) - 1 : -1;
+                lead[k] = lane == leader[k];
+            }
+            bool any = true;
+            while (__any_sync(FULL, any)) any = step(lead);
+            i32 gk[K];
+            bool pr[K];
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                gk[k] = __shfl_sync(FULL, res[k], leader[k] < 0 ? 0 : leader[k]);
+                pr[k] = go[k] && leader[k] >= 0;
+            }
+            probe_around(gk, pr, false);
         }
     }
+    bool all_sel[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) all_sel[k] = true;
     bool any = true;
-    while (any) any = step(all_sel);
+    while (any) any = step(all_sel);  // (4)
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+        if (act[k]) hint = res[k];
 }
 
-__global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
-    extern __shared__ __align__(16) unsigned char dyn_smem[];
-    __shared__ GsSmem ssm;
-    __shared__ TreeSmem tsm;
-    const GsStage stg = gs_stage(dyn_smem);
+// new sort key of a classified member (l = LCP with the head in words; wa / wb = the two words at l)
+__device__ __forceinline__ u64 class_key(const KeyLayout& kl, u32 rank, i32 l, i32 na, i32 nb, u64 wa, u64 wb) {
+    u64 F, dig = 0;
+    if (l == na && l == nb) F = kl.f_head();
+    else if (l == na) F = kl.f_before((u64)kl.D * l, true);
+    else {  // l < na <= nb: the words at l differ
+        const int jd = __clzll((long long)(wa ^ wb)) / kl.w;
+        const u64 ld = (u64)kl.D * l + jd;
+        const u64 da = (wa << (jd * kl.w)) >> (64 - kl.w), db = (wb << (jd * kl.w)) >> (64 - kl.w);
+        dig = da;
+        F = da < db ? kl.f_before(ld, false) : kl.f_after(ld);
+    }
+    return kl.pack(rank, F, dig);
+}
+
+// ---- local stage ----------------------------------------------------------------------------------
+// A work item lives in shared memory.  Its elements (sort key, request, chain length saturated to
+// 16 bits - the head of a segment is its longest chain, found without a gather) never move: the
+// sorted order is a permutation `idx` of element numbers (u16), so a sort pass moves two bytes per
+// element and nothing is held in registers across a barrier.  The second index buffer doubles as
+// the per-position scratch between sorts (segment start + unresolved flag).
+struct LocalBufs {
+    u64* key;             // by element
+    u32* val;             // by element: request
+    unsigned short* na;   // by element: chain length, 0xffff = look it up in the record
+    unsigned short* idx;  // by position: element (current order)
+    unsigned short* aux;  // by position: the other index buffer / segment start | unresolved << 15
+};
+__device__ __forceinline__ LocalBufs local_bufs(unsigned char* dyn_smem) {
+    return LocalBufs{(u64*)dyn_smem, (u32*)(dyn_smem + (size_t)LOC_CAP * 8),
+                     (unsigned short*)(dyn_smem + (size_t)LOC_CAP * 12),
+                     (unsigned short*)(dyn_smem + (size_t)LOC_CAP * 14),
+                     (unsigned short*)(dyn_smem + (size_t)LOC_CAP * 16)};
+}
+
+// Stable LSD sort of the item's n <= LOC_CAP positions by the key bits set in `vary` (8-bit
+// digits): permutes lb.idx (ping-pong with lb.aux; the roles are swapped in place).  Warp w owns
+// positions [w*32*Kp, (w+1)*32*Kp), Kp = ceil(n / GS_THREADS) rows.
+__device__ __forceinline__ void local_sort(LocalBufs& lb, int n, u64 vary, GsSmem& sm) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int Kp = (n + GS_THREADS - 1) / GS_THREADS;
+    const int wbase = w * 32 * Kp;
+    while (vary) {
+        const int sh = __ffsll((long long)vary) - 1;
+        vary &= ~(0xffull << sh);
+        u32 meta[LOC_K];
+        unsigned short el[LOC_K];
+#pragma unroll
+        for (int k = 0; k < LOC_K; ++k) {
+            const int i = wbase + k * 32 + lane;
+            const bool valid = k < Kp && i < n;
+            el[k] = valid ? lb.idx[i] : (unsigned short)0;
+            meta[k] = valid ? (u32)(lb.key[el[k]] >> sh) & 255u : (0x100u | lane);
+        }
+        gs_rank_tile<LOC_K>(meta, sm);
+#pragma unroll
+        for (int k = 0; k < LOC_K; ++k) {
+            const int i = wbase + k * 32 + lane;
+            if (k < Kp && i < n) {
+                const u32 d = meta[k] & 0xffffu;
+                lb.aux[sm.dstart[d] + sm.wcnt[w][d] + (meta[k] >> 16)] = el[k];
+            }
+        }
+        __syncthreads();
+        unsigned short* t = lb.idx; lb.idx = lb.aux; lb.aux = t;
+    }
+}
+
+enum { LOCAL_FROM_GLOBAL = 0, LOCAL_WHOLE_QUEUE = 1 };
+
+// One CTA finishes positions [p0, p0 + n), n <= LOC_CAP, which hold whole segments: all remaining
+// refinement rounds, then the final order and the adjacent LCPs of the range.
+//   LOCAL_FROM_GLOBAL  the pairs are Kg / Vg as the global stage left them (keys in layout kg); the
+//                      LCP at every boundary of the range as it stands is already written
+//   LOCAL_WHOLE_QUEUE  p0 = 0, n = N: round 0 runs here too (A.srank holds the round-0 digits)
+// Keys made here use the layout kl (narrower digits than the grid-wide rounds: fewer sort passes;
+// a digit collision only keeps two branches together for one more round).
+__device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& kg, const KeyLayout& kl,
+                                           const u64* __restrict__ Kg, const u32* __restrict__ Vg, i64 p0, int n,
+                                           int mode, GsSmem& ssm, TreeSmem& tsm, LocalBufs lb) {
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned le_mask = 0xffffffffu >> (31 - lane);
+    const u64* __restrict__ H = A.hashes;
+    const ReqRec* __restrict__ rec = A.rec;
+    const int Kp = (n + GS_THREADS - 1) / GS_THREADS;
+    const int wbase = w * 32 * Kp;
+    PEEK_MARK(30);
+    for (int i = threadIdx.x; i < n; i += GS_THREADS) {
+        u32 r;
+        if (mode == LOCAL_FROM_GLOBAL) { lb.key[i] = __ldcg(Kg + p0 + i); r = __ldcg(Vg + p0 + i); }
+        else { lb.key[i] = round0_key(kl, __ldcg(A.srank + i)); r = (u32)i; }
+        lb.val[i] = r;
+        lb.idx[i] = (unsigned short)i;
+        const u32 na = __ldg(&rec[r].na);
+        lb.na[i] = (unsigned short)(na < 0xffffu ? na : 0xffffu);
+    }
+    __syncthreads();
+    i32 hint = -1;
+    u64 vary = mode == LOCAL_WHOLE_QUEUE ? round0_vary(kl, __ldcg(&A.ctl->flags)) : 0;
+    for (int lr = mode == LOCAL_WHOLE_QUEUE ? 1 : 0;; ++lr) {
+        // stable sort of the range by the keys of the last classification (round 0: the first words)
+        PEEK_MARK(31);
+        if (lr > 0) local_sort(lb, n, vary, ssm);
+        PEEK_MARK(32);
+        const KeyLayout& kc = lr == 0 ? kg : kl;  // layout of the keys as they stand
+        // key of position i, of its left and of its right neighbour (shuffles inside the row)
+        auto keys3 = [&](int i, bool valid, u64& key, u64& prev, u64& next) {
+            key = valid ? lb.key[lb.idx[i]] : 0;
+            prev = __shfl_up_sync(FULL, key, 1);
+            next = __shfl_down_sync(FULL, key, 1);
+            if (lane == 0) prev = (valid && i > 0) ? lb.key[lb.idx[i - 1]] : 0;
+            if (lane == 31 || !(i + 1 < n)) next = (valid && i + 1 < n) ? lb.key[lb.idx[i + 1]] : 0;
+        };
+        // ---- L1a: segment starts per warp ----
+        {
+            u32 wc = 0, wl = 0;
+#pragma unroll
+            for (int k = 0; k < LOC_K; ++k) {
+                if (k < Kp) {
+                    const int i = wbase + k * 32 + lane;
+                    const bool valid = i < n;
+                    u64 key, prev, next;
+                    keys3(i, valid, key, prev, next);
+                    const bool start = valid && (i == 0 || prev != key);
+                    if (start) A.seghead[p0 + i] = 0;  // reset before L1b's maxima (a CTA barrier apart)
+                    const unsigned bal = __ballot_sync(FULL, start);
+                    wc += __popc(bal);
+                    if (bal) wl = (u32)((i - lane) + 31 - __clz(bal)) + 1u;
+                }
+            }
+            if (lane == 0) tsm.wv64[w] = ((i64)wc << 32) | wl;
+            if (threadIdx.x == 0) { tsm.cnt = 0; tsm.orv = 0; tsm.andv = ~0ull; }
+            __syncthreads();
+            if (w == 0) {  // exclusive (sum, max) scan over the warps
+                const i64 own = lane < GS_WARPS ? tsm.wv64[lane] : 0;
+                u32 ic = (u32)(own >> 32), il = (u32)own;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const u32 xc = __shfl_up_sync(FULL, ic, o), xl = __shfl_up_sync(FULL, il, o);
+                    if (lane >= o) { ic += xc; il = max(il, xl); }
+                }
+                u32 ec = __shfl_up_sync(FULL, ic, 1), el = __shfl_up_sync(FULL, il, 1);
+                if (lane == 0) { ec = 0; el = 0; }
+                if (lane < GS_WARPS) tsm.wv64[lane] = ((i64)ec << 32) | el;
+            }
+            __syncthreads();
+        }
+        // ---- L1b: segment start and rank of every position, adjacent LCP of the boundaries the
+        // last sort made, unresolved flag, head = longest chain of every unresolved segment ----
+        {
+            i32 c = (i32)(u32)tsm.wv64[w] - 1;  // last segment start before this warp's rows
+            u32 cc = (u32)(tsm.wv64[w] >> 32);  // segment starts before this warp's rows
+            u32 n_unres = 0;
+#pragma unroll
+            for (int k = 0; k < LOC_K; ++k) {
+                if (k < Kp) {
+                    const int i = wbase + k * 32 + lane;
+                    const bool valid = i < n;
+                    u64 key, prev, next;
+                    keys3(i, valid, key, prev, next);
+                    const bool start = valid && (i == 0 || prev != key);
+                    const bool last = valid && (i == n - 1 || next != key);
+                    const u64 F = kc.F_of(key);
+                    const bool br = valid && kc.is_branch(F);
+                    const unsigned bal = __ballot_sync(FULL, start);
+                    const unsigned m = bal & le_mask;
+                    const i32 s = m ? (i32)(i - lane) + 31 - __clz(m) : c;
+                    if (bal) c = (i32)(i - lane) + 31 - __clz(bal);
+                    const u32 rank = cc + __popc(m) - 1u;
+                    cc += __popc(bal);
+                    const bool un = br && !(start && last);
+                    if (valid) lb.aux[i] = (unsigned short)(s | (un ? 0x8000 : 0));
+                    if (start) {
+                        A.srank[p0 + i] = rank;
+                        A.segdepth[p0 + i] = br ? (i32)(kc.ld_of(F) / kc.D) : 0;
+                        if (p0 + i == 0) A.lcp[0] = 0;
+                        else if (i > 0 && lr > 0 && kc.seg_of(prev) == kc.seg_of(key)) {
+                            const u64 la = kc.ldv(kc.F_of(prev)), lb2 = kc.ldv(F);
+                            A.lcp[p0 + i] = (i32)((la < lb2 ? la : lb2) / kc.D);
+                        }
+                    }
+                    const unsigned ub = __ballot_sync(FULL, un);
+                    n_unres += __popc(ub);
+                    if (ub) {  // warp-uniform
+                        const int e = valid ? lb.idx[i] : 0;
+                        u32 nbv = un ? (u32)lb.na[e] : 0u;
+                        if (nbv == 0xffffu) nbv = __ldg(&rec[lb.val[e]].na);  // saturated: the record has it
+                        u64 v = un ? (((u64)nbv << 32) | (u64)(0xffffffffu - (u32)i)) : 0ull;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const u64 x = __shfl_up_sync(FULL, v, o);
+                            const i32 sx = __shfl_up_sync(FULL, s, o);
+                            if (lane >= o && sx == s && x > v) v = x;
+                        }
+                        const i32 sn = __shfl_down_sync(FULL, s, 1);
+                        if (v && (lane == 31 || sn != s)) atomicMax((unsigned long long*)&A.seghead[p0 + s], v);
+                    }
+                }
+            }
+            if (lane == 0 && n_unres) atomicAdd(&tsm.cnt, n_unres);
+            __syncthreads();
+        }
+        PEEK_MARK(33);
+        if (tsm.cnt == 0) break;
+        // ---- L2: classify every unresolved position against its segment head.  The new key
+        // replaces the element's old one in place: this phase reads no neighbour's key ----
+        {
+            u64 orv = 0, andv = ~0ull;
+            for (int hb = 0; hb * LSB < Kp; ++hb) {
+                u32 sg[LSB], r[LSB], rk[LSB], h[LSB], el[LSB];
+                bool val_[LSB], un[LSB], cmp[LSB];
+                u64 hv[LSB], al[LSB], k0a[LSB], k0b[LSB];
+                i64 ao[LSB], bo[LSB];
+                i32 na[LSB], nb[LSB], lo[LSB], l[LSB];
+                LSUBS(k) {
+                    const int kk = hb * LSB + k;
+                    const int i = wbase + kk * 32 + lane;
+                    val_[k] = kk < Kp && i < n;
+                    sg[k] = 0; r[k] = 0; un[k] = false; el[k] = 0;
+                    if (val_[k]) {
+                        const u32 a = lb.aux[i];
+                        sg[k] = a & 0x7fffu;
+                        un[k] = (a >> 15) != 0;
+                        el[k] = lb.idx[i];
+                        r[k] = lb.val[el[k]];
+                    }
+                }
+                LSUBS(k) {
+                    rk[k] = 0; hv[k] = 0; ao[k] = 0; na[k] = 0; lo[k] = 0; al[k] = 0; k0a[k] = 0;
+                    if (val_[k]) rk[k] = __ldcg(A.srank + p0 + sg[k]);
+                    if (un[k]) {
+                        hv[k] = __ldcg(A.seghead + p0 + sg[k]);
+                        lo[k] = __ldcg(A.segdepth + p0 + sg[k]);
+                        rec_head(rec, r[k], ao[k], na[k]);
+                        rec_tail(rec, r[k], al[k], k0a[k]);
+                    }
+                }
+                LSUBS(k) { h[k] = un[k] ? lb.val[lb.idx[0xffffffffu - (u32)hv[k]]] : 0u; nb[k] = (i32)(hv[k] >> 32); }
+                LSUBS(k) {
+                    bo[k] = 0; k0b[k] = 0;
+                    if (un[k]) { i32 nh; u64 lh; rec_head(rec, h[k], bo[k], nh); rec_tail(rec, h[k], lh, k0b[k]); }
+                    cmp[k] = un[k] && r[k] != h[k];
+                    l[k] = na[k];  // r == h: the head itself
+                }
+                PEEK_MARK(40 + hb);
+                lcp_lockstep<LSB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, hint);
+                PEEK_MARK(60 + hb);
+                u64 wa[LSB], wb[LSB];
+                LSUBS(k) {
+                    wa[k] = wb[k] = 0;
+                    if (un[k] && l[k] < na[k]) { wa[k] = __ldg(H + ao[k] + l[k]); wb[k] = __ldg(H + bo[k] + l[k]); }
+                }
+                LSUBS(k) {
+                    if (val_[k]) {
+                        const u64 nk = un[k] ? class_key(kl, rk[k], l[k], na[k], nb[k], wa[k], wb[k])
+                                             : kl.pack(rk[k], 0, 0);
+                        lb.key[el[k]] = nk;
+                        orv |= nk;
+                        andv &= nk;
+                    }
+                }
+            }
+            const u32 olo = __reduce_or_sync(FULL, (u32)orv), ohi = __reduce_or_sync(FULL, (u32)(orv >> 32));
+            const u32 alo = __reduce_and_sync(FULL, (u32)andv), ahi = __reduce_and_sync(FULL, (u32)(andv >> 32));
+            if (lane == 0) {
+                atomicOr(&tsm.orv, ((unsigned long long)ohi << 32) | olo);
+                atomicAnd(&tsm.andv, ((unsigned long long)ahi << 32) | alo);
+            }
+            __syncthreads();
+        }
+        vary = tsm.orv & ~tsm.andv;  // sorted on at the top of the next round
+        __syncthreads();             // tsm.orv is reset by the next round's L1a
+    }
+    // ---- final order of the range; positions inside a final segment repeat their neighbour's
+    // chain (the LCP of every boundary was written when the boundary appeared) ----
+    PEEK_MARK(35);
+#pragma unroll
+    for (int k = 0; k < LOC_K; ++k) {
+        if (k < Kp) {
+            const int i = wbase + k * 32 + lane;
+            if (i < n) {
+                const int e = lb.idx[i];
+                const u32 r = lb.val[e];
+                A.order[p0 + i] = (i32)r;
+                if (i > 0 && lb.key[e] == lb.key[lb.idx[i - 1]]) {
+                    u32 nbv = lb.na[e];
+                    if (nbv == 0xffffu) nbv = __ldg(&rec[r].na);
+                    A.lcp[p0 + i] = (i32)nbv;
+                }
+            }
+        }
+    }
+    __syncthreads();  // the shared buffers are reused by the next work item
+}
+
+// final order and LCP of positions [x, y) that the global stage left resolved: written straight
+// from the global pairs (a non-start position of a resolved segment repeats its neighbour's chain)
+__device__ __forceinline__ void tree_direct_output(const TreeArgs& A, const u32* __restrict__ Vg, i64 x, i64 y) {
+    for (i64 j = x + threadIdx.x; j < y; j += GS_THREADS) {
+        const u32 r = __ldcg(Vg + j);
+        A.order[j] = (i32)r;
+        if ((i64)(__ldcg(A.seg + j) & 0x7fffffffu) != j) A.lcp[j] = (i32)__ldg(&A.rec[r].na);
+    }
+}
+
+// ---- the stages as device functions; the kernels below string them together ---------------------
+
+// phase 0: chain lengths, last words, round-0 digits.  Ends with a grid barrier.
+__device__ __forceinline__ void tree_phase0(const TreeArgs& A, Grid& g) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const unsigned le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
     const i64 N = A.N;
     const int G = gridDim.x, me = blockIdx.x;
     const i64 gtid = (i64)me * GS_THREADS + threadIdx.x;
-    Grid g{&A.ctl->bar, 0};
     const u64* __restrict__ H = A.hashes;
     const i64* __restrict__ BO = A.blk_off;
     const i64 C = (N + G - 1) / G;
     const i64 c0 = min((i64)me * C, N), c1 = min(c0 + C, N);
     const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
     auto IDX = [&](int t, int k) -> i64 { return c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane; };
-    PEEK_MARK(1);
-
-    if (!A.signals_only) {  // build order + lcp; otherwise they are inputs (peek_pending_tree_update)
-    // ---- phase 0: max chain length, identity order ----
+    (void)FULL; (void)le_mask; (void)gtid; (void)H; (void)BO; (void)ntiles; (void)c1;
+    // ---- phase 0: chain lengths, last words, round-0 digits (leading bits of the first word) ----
     {
-        u32 mx = 0;
+        u32 mx = 0, empty = 0;
         for (int t = 0; t < ntiles; ++t) {
             i64 b0[GS_KPT], b1[GS_KPT];
             ELEMS(k) {
                 const i64 i = IDX(t, k);
                 b0[k] = b1[k] = 0;
-                if (i < c1) { b0[k] = __ldg(BO + i); b1[k] = __ldg(BO + i + 1); A.bufs.val[0][i] = (u32)i; }
+                if (i < c1) { b0[k] = __ldg(BO + i); b1[k] = __ldg(BO + i + 1); }
             }
-            ELEMS(k) mx = max(mx, (u32)(b1[k] - b0[k]));
-            // the last word of every chain, gathered once: a member's chain is never longer than
-            // its head's, so the "does one chain prefix the other" probe of every round reads it
-            u64 lw[GS_KPT];
-            ELEMS(k) lw[k] = b1[k] > b0[k] ? __ldg(H + b1[k] - 1) : 0ull;
-            ELEMS(k) { const i64 i = IDX(t, k); if (i < c1) A.lasth[i] = lw[k]; }
+            // the first and the last word of every chain, gathered once into the request's record: a
+            // member's chain is never longer than its head's, so the "does one chain prefix the
+            // other" probe of every round reads the member's side from the record
+            u64 lw[GS_KPT], fw[GS_KPT];
+            ELEMS(k) {
+                lw[k] = fw[k] = 0;
+                if (b1[k] > b0[k]) { lw[k] = __ldg(H + b1[k] - 1); fw[k] = __ldg(H + b0[k]); }
+            }
+            ELEMS(k) {
+                const i64 i = IDX(t, k);
+                if (i < c1) {
+                    const bool has = b1[k] > b0[k];
+                    mx = max(mx, (u32)(b1[k] - b0[k]));
+                    empty |= has ? 0u : 1u;
+                    ulonglong2* rp = (ulonglong2*)(A.rec + i);
+                    rp[0] = make_ulonglong2((u64)b0[k], (u64)(u32)(b1[k] - b0[k]));
+                    rp[1] = make_ulonglong2(lw[k], fw[k]);
+                    A.srank[i] = has ? (0x80000000u | (u32)(fw[k] >> (64 - W0_BITS))) : 0u;
+                }
+            }
         }
         mx = __reduce_max_sync(FULL, mx);
+        empty = __reduce_or_sync(FULL, empty);
         if (lane == 0 && mx) atomicMax(&A.ctl->maxnb, mx);
+        if (lane == 0 && empty) atomicOr(&A.ctl->flags, 1u);
         if (gtid == 0) { A.ctl->kand[0] = ~0ull; A.ctl->kand[1] = ~0ull; }
     }
     g.sync();
-    const KeyLayout kl = make_layout(N, __ldcg(&A.ctl->maxnb));
-    {
-        const u64 k_init = kl.pack(0, kl.f_before(0, false), 0);
-        for (int t = 0; t < ntiles; ++t)
-            ELEMS(k) { const i64 i = IDX(t, k); if (i < c1) A.bufs.key[0][i] = k_init; }
-    }
-    int cb = 0;  // buffer that holds the current (key, request) pairs by position
+}
 
-    for (int round = 0;; ++round) {
+// grid-wide stage: round 0, then refinement rounds while some unresolved segment exceeds cap_seg.
+// Leaves the pairs in A.bufs.*[ctl->fin_cb] and the round's counters at index ctl->fin_round % 3.
+__device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& kl, Grid& g, GsSmem& ssm,
+                                            TreeSmem& tsm, const GsStage stg) {
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
+    const i64 N = A.N;
+    const int G = gridDim.x, me = blockIdx.x;
+    const i64 gtid = (i64)me * GS_THREADS + threadIdx.x;
+    const u64* __restrict__ H = A.hashes;
+    const i64* __restrict__ BO = A.blk_off;
+    const i64 C = (N + G - 1) / G;
+    const i64 c0 = min((i64)me * C, N), c1 = min(c0 + C, N);
+    const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
+    auto IDX = [&](int t, int k) -> i64 { return c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane; };
+    (void)FULL; (void)le_mask; (void)gtid; (void)H; (void)BO; (void)ntiles; (void)c1;
+    int cb = 0, round = 0;
+    // ---- round 0: stable sort by the round-0 key (generated on the fly from the digits) ----
+    {
+        const u32 flags = __ldcg(&A.ctl->flags);
+        const u32* __restrict__ d0 = A.srank;
+        cb = grid_sort_pairs_gen(A.bufs, N, round0_vary(kl, flags), g, ssm, stg,
+                                 [&](i64 i, u64& key, u32& val) { key = round0_key(kl, __ldcg(d0 + i)); val = (u32)i; });
+    }
+    PEEK_MARK(9);
+
+    for (round = 1;; ++round) {
         g.sync();  // keys / order of the previous phase visible
         PEEK_MARK(10);
         const u64* K = A.bufs.key[cb];
@@ -296,6 +743,8 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
         u32* cnt = &A.ctl->unres[round % 3];
         if (gtid == 0) {
             A.ctl->unres[(round + 1) % 3] = 0;
+            A.ctl->maxseg[(round + 1) % 3] = 0;
+            A.ctl->nbig[(round + 1) % 3] = 0;
             A.ctl->kor[(round + 1) & 1] = 0;
             A.ctl->kand[(round + 1) & 1] = ~0ull;
         }
@@ -325,7 +774,7 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                         // two chains leave their old head's path at ldv digits, so they share
                         // exactly min(ldv) digits - the final adjacent LCP, no chain reads needed
                         if (i == 0) A.lcp[0] = 0;
-                        else if (round > 0 && kl.seg_of(km[k]) == kl.seg_of(k0[k])) {
+                        else if (kl.seg_of(km[k]) == kl.seg_of(k0[k])) {
                             const u64 la = kl.ldv(kl.F_of(km[k])), lb = kl.ldv(F);
                             A.lcp[i] = (i32)((la < lb ? la : lb) / kl.D);
                         }
@@ -341,7 +790,8 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
             }
         }
         g.sync();
-        // ---- R1b: segment start of every position, unresolved flag, head = longest chain ----
+        // ---- R1b: segment start of every position, unresolved flag, head = longest chain; sizes
+        // of the unresolved segments (the largest decides whether the local stage can take over) ----
         {
             if (w == 0) {  // segment starts in the chunks before mine: how many, and the last one
                 u32 cs = 0, ls = 0;
@@ -357,7 +807,7 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                 if (lane == 0) tsm.carry64 = ((i64)cs << 32) | ls;
             }
             __syncthreads();
-            u32 n_unres = 0;
+            u32 n_unres = 0, max_size = 0;
             u64 carry_v = 0;  // head candidate of the segment the warp's last full rows lay in
             i32 carry_s = 0;
             for (int t = 0; t < ntiles; ++t) {
@@ -425,15 +875,24 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                         un[k] = valid && (fl[kk] & 4u) && (fl[kk] & 3u) != 3u;
                         sarr[k] = s;
                         if (valid) { A.seg[i] = (u32)s | (un[k] ? 0x80000000u : 0u); A.srank[i] = rank; }
+                        if (un[k] && (fl[kk] & 2u)) {  // last position of an unresolved segment: its size
+                            const u32 size = (u32)(i - (i64)s) + 1u;
+                            A.gsz[s] = (i32)size;
+                            max_size = max(max_size, size);
+                            if (size > (u32)A.quantum && size <= (u32)A.cap_seg) {
+                                const u32 slot = atomicAdd(&A.ctl->nbig[round % 3], 1u);
+                                A.biglist[slot] = (u64)(u32)s | ((u64)size << 32);
+                            }
+                        }
                         r[k] = un[k] ? __ldcg(cur + i) : 0u;
                     }
-                    i64 b0[SB], b1[SB];
-                    SUBS(k) { b0[k] = b1[k] = 0; if (un[k]) { b0[k] = __ldg(BO + r[k]); b1[k] = __ldg(BO + r[k] + 1); } }
+                    u32 nbr[SB];
+                    SUBS(k) nbr[k] = un[k] ? __ldg(&A.rec[r[k]].na) : 0u;
                     SUBS(k) {
                         // head = longest chain of the segment, lowest position on ties: segmented
                         // max over the row's runs of equal s, one atomic per run
                         const i64 i = IDX(t, hb * SB + k);
-                        u64 v = un[k] ? (((u64)(u32)(b1[k] - b0[k]) << 32) | (u64)(0xffffffffu - (u32)i)) : 0ull;
+                        u64 v = un[k] ? (((u64)nbr[k] << 32) | (u64)(0xffffffffu - (u32)i)) : 0ull;
                         const i32 s = sarr[k];
 #pragma unroll
                         for (int o = 1; o < 32; o <<= 1) {
@@ -466,15 +925,19 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
             }
             if (lane == 0 && carry_v) atomicMax((unsigned long long*)&A.seghead[carry_s], carry_v);
             if (lane == 0 && n_unres) atomicAdd(cnt, n_unres);
+            max_size = __reduce_max_sync(FULL, max_size);
+            if (lane == 0 && max_size) atomicMax(&A.ctl->maxseg[round % 3], max_size);
         }
         g.sync();
         PEEK_MARK(11);
-        if (__ldcg(cnt) == 0) break;  // grid-uniform: read after the barrier
+        // grid-uniform (read after the barrier): every unresolved segment fits one CTA
+        if (__ldcg(&A.ctl->maxseg[round % 3]) <= (u32)A.cap_seg) break;  // the local stage takes over
 
         // ---- R2: classify every unresolved position against its segment head (keys in place) ----
         {
             u64* Kw = A.bufs.key[cb];
             u64 orv = 0, andv = ~0ull;
+            i32 hint = -1;
             for (int t = 0; t < ntiles; ++t)
             for (int hb = 0; hb < GS_KPT / SB; ++hb) {
                 u32 sg[SB], r[SB], h[SB], rk[SB];
@@ -485,28 +948,27 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                     if (i < c1) { sg[k] = A.seg[i]; r[k] = __ldcg(cur + i); rk[k] = A.srank[i]; }
                     un[k] = (sg[k] >> 31) != 0;
                 }
-                u64 hv[SB];
+                u64 hv[SB], al[SB], k0a[SB], k0b[SB];
                 i64 ao[SB], bo[SB];
                 i32 na[SB], nb[SB], lo[SB], l[SB];
                 SUBS(k) {
-                    hv[k] = 0; ao[k] = 0; na[k] = 0; lo[k] = 0;
+                    hv[k] = 0; ao[k] = 0; na[k] = 0; lo[k] = 0; al[k] = 0; k0a[k] = 0;
                     if (un[k]) {
                         const u32 s = sg[k] & 0x7fffffffu;
                         hv[k] = __ldcg(A.seghead + s);
                         lo[k] = __ldcg(A.segdepth + s);
-                        ao[k] = __ldg(BO + r[k]);
-                        na[k] = (i32)(__ldg(BO + r[k] + 1) - ao[k]);
+                        rec_head(A.rec, r[k], ao[k], na[k]);
+                        rec_tail(A.rec, r[k], al[k], k0a[k]);
                     }
                 }
                 SUBS(k) { h[k] = un[k] ? __ldcg(cur + (0xffffffffu - (u32)hv[k])) : 0u; nb[k] = (i32)(hv[k] >> 32); }
                 SUBS(k) {
-                    bo[k] = un[k] ? __ldg(BO + h[k]) : 0;
+                    bo[k] = 0; k0b[k] = 0;
+                    if (un[k]) { i32 nh; u64 lh; rec_head(A.rec, h[k], bo[k], nh); rec_tail(A.rec, h[k], lh, k0b[k]); }
                     cmp[k] = un[k] && r[k] != h[k];
                     l[k] = na[k];  // r == h: the head itself
                 }
-                u64 al[SB];
-                SUBS(k) al[k] = un[k] ? __ldcg(A.lasth + r[k]) : 0ull;
-                lcp_lockstep<SB, true>(H, ao, na, bo, nb, lo, cmp, l, round == 0, al);
+                lcp_lockstep<SB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, hint);
                 u64 wa[SB], wb[SB];
                 SUBS(k) {
                     wa[k] = wb[k] = 0;
@@ -515,24 +977,8 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
                 SUBS(k) {
                     const i64 i = IDX(t, hb * SB + k);
                     if (i < c1) {
-                        const u32 s = rk[k];  // dense segment rank: few leading key bits vary
-                        u64 nk;
-                        if (!un[k]) {
-                            nk = kl.pack(s, 0, 0);
-                        } else {
-                            u64 F, dig = 0;
-                            if (l[k] == na[k] && l[k] == nb[k]) F = kl.f_head();
-                            else if (l[k] == na[k]) F = kl.f_before((u64)kl.D * l[k], true);
-                            else {  // l < na <= nb: the words at l differ
-                                const u64 a = wa[k], b = wb[k];
-                                const int jd = __clzll((long long)(a ^ b)) / kl.w;
-                                const u64 ld = (u64)kl.D * l[k] + jd;
-                                const u64 da = (a << (jd * kl.w)) >> (64 - kl.w), db = (b << (jd * kl.w)) >> (64 - kl.w);
-                                dig = da;
-                                F = da < db ? kl.f_before(ld, false) : kl.f_after(ld);
-                            }
-                            nk = kl.pack(s, F, dig);
-                        }
+                        // dense segment rank: few leading key bits vary
+                        const u64 nk = un[k] ? class_key(kl, rk[k], l[k], na[k], nb[k], wa[k], wb[k]) : kl.pack(rk[k], 0, 0);
                         Kw[i] = nk;
                         orv |= nk;
                         andv &= nk;
@@ -554,38 +1000,103 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
         cb = grid_sort_pairs(A.bufs, N, vary, g, ssm, stg, cb);
         PEEK_MARK(13);
     }
-    const u32* cur = A.bufs.val[cb];
+    if (gtid == 0) { A.ctl->fin_cb = (u32)cb; A.ctl->fin_round = (u32)round; }
+}
 
-    // ---- F1: final order.  The adjacent LCP of every segment boundary was written when the
-    // boundary appeared (R1a); positions inside a final segment repeat their neighbour's chain ----
+// local stage: every work item is finished by one CTA (no CTA waits for another)
+__device__ __forceinline__ void tree_local_stage(const TreeArgs& A, const KeyLayout& kg, const KeyLayout& kl, bool whole, int cb, int round,
+                                                 GsSmem& ssm, TreeSmem& tsm, unsigned char* dyn_smem) {
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const i64 N = A.N;
+    const LocalBufs lb = local_bufs(dyn_smem);
+    // ---- local stage: every work item is finished by one CTA.  Items: the whole queue (small
+    // inputs), else the segments above the quantum (one item each), then the quanta of positions ----
     {
         const u64* K = A.bufs.key[cb];
-        for (int t = 0; t < ntiles; ++t) {
-            u32 r[GS_KPT];
-            bool same[GS_KPT];
-            ELEMS(k) {
-                const i64 i = IDX(t, k);
-                r[k] = 0; same[k] = false;
-                if (i < c1) {
-                    r[k] = __ldcg(cur + i);
-                    if (i > 0) same[k] = __ldcg(K + i) == __ldcg(K + i - 1);
+        const u32* cur = A.bufs.val[cb];
+        const u32 nbig = whole ? 0u : __ldcg(&A.ctl->nbig[round % 3]);
+        const bool any_unres = whole || __ldcg(&A.ctl->unres[round % 3]) != 0;
+        const i64 Q = A.quantum;
+        const u32 nq = (u32)((N + Q - 1) / Q);
+        int stage = whole ? 0 : 1;  // 0 whole queue, 1 big segments, 2 quanta, 3 done
+        while (stage < 3) {
+            i64 p0 = 0;
+            int n = 0;
+            if (stage == 0) {
+                n = (int)N;
+                stage = 3;
+            } else {
+                if (threadIdx.x == 0) tsm.item = atomicAdd(stage == 1 ? &A.ctl->next_big : &A.ctl->next_q, 1u);
+                __syncthreads();
+                const u32 it = tsm.item;
+                __syncthreads();
+                if (stage == 1) {
+                    if (it >= nbig) { stage = 2; continue; }
+                    const u64 e = __ldcg(A.biglist + it);
+                    p0 = (i64)(u32)e;
+                    n = (int)(e >> 32);
+                } else {
+                    if (it >= nq) break;
+                    const i64 a = (i64)it * Q, b = min(a + Q, N);
+                    if (!any_unres) { tree_direct_output(A, cur, a, b); continue; }
+                    // positions at the start of the quantum that belong to a segment begun before
+                    // it: resolved ones are written here, an unresolved segment is another item's
+                    p0 = a;
+                    const u32 sa = __ldcg(A.seg + a);
+                    if ((i64)(sa & 0x7fffffffu) < a) {
+                        if (threadIdx.x == 0) tsm.red = (u32)(b - a);
+                        __syncthreads();
+                        u32 first = (u32)(b - a);
+                        for (i64 j = a + threadIdx.x; j < b; j += GS_THREADS)
+                            if ((i64)(__ldcg(A.seg + j) & 0x7fffffffu) >= a) { first = (u32)(j - a); break; }
+                        first = __reduce_min_sync(FULL, first);
+                        if (lane == 0 && first < (u32)(b - a)) atomicMin(&tsm.red, first);
+                        __syncthreads();
+                        p0 = a + tsm.red;
+                        __syncthreads();
+                        if (!(sa >> 31)) tree_direct_output(A, cur, a, p0);
+                    }
+                    if (p0 >= b) continue;
+                    // the segment holding the quantum's last position started inside the range
+                    const u32 sb = __ldcg(A.seg + b - 1);
+                    const i64 sl = (i64)(sb & 0x7fffffffu);
+                    i64 e = b;
+                    if (sb >> 31) {
+                        const i64 size = __ldcg(A.gsz + sl);
+                        e = size > Q ? sl : sl + size;  // above the quantum: an item of the big list
+                    }
+                    if (e <= p0) continue;
+                    int un_any = 0;  // anything left to refine in [p0, e)?
+                    for (i64 j = p0 + threadIdx.x; j < e; j += GS_THREADS) un_any |= (int)(__ldcg(A.seg + j) >> 31);
+                    un_any = __syncthreads_or(un_any);
+                    if (!un_any) { tree_direct_output(A, cur, p0, e); continue; }
+                    n = (int)(e - p0);
                 }
             }
-            ELEMS(k) {
-                const i64 i = IDX(t, k);
-                if (i < c1) {
-                    A.order[i] = (i32)r[k];
-                    if (same[k]) A.lcp[i] = (i32)(__ldg(BO + r[k] + 1) - __ldg(BO + r[k]));
-                }
-            }
+            tree_local(A, kg, kl, K, cur, p0, n, whole ? LOCAL_WHOLE_QUEUE : LOCAL_FROM_GLOBAL, ssm, tsm, lb);
         }
     }
-    }  // !signals_only
-    PEEK_MARK(20);
+}
+
+// groups and clusters from (order, lcp): three grid-wide phases
+__device__ __forceinline__ void tree_signals(const TreeArgs& A, Grid& g, TreeSmem& tsm, i32* lvl_hi) {
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
+    const i64 N = A.N;
+    const int G = gridDim.x, me = blockIdx.x;
+    const i64 gtid = (i64)me * GS_THREADS + threadIdx.x;
+    const u64* __restrict__ H = A.hashes;
+    const i64* __restrict__ BO = A.blk_off;
+    const i64 C = (N + G - 1) / G;
+    const i64 c0 = min((i64)me * C, N), c1 = min(c0 + C, N);
+    const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
+    auto IDX = [&](int t, int k) -> i64 { return c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane; };
+    (void)FULL; (void)le_mask; (void)gtid; (void)H; (void)BO; (void)ntiles; (void)c1;
     const bool want_groups = A.group_id || A.group_size || A.n_groups;
     const bool want_clusters = A.cluster_depth || A.cluster_size || A.cluster_id;
     if (!want_groups && !want_clusters) return;
-    g.sync();
     MinTree mt;
     mintree_layout(mt, A.lcp, N, A.mt_buf);
     const i64 gwarp = gtid >> 5, nwarps = ((i64)G * GS_THREADS) >> 5;
@@ -688,7 +1199,7 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
         if (mt.n[3] <= 2048) {
             int off = 0;
             for (int k = 3; k < mt.levels; ++k) {
-                mt.lvl[k] = tsm.lvl_hi + off;
+                mt.lvl[k] = lvl_hi + off;
                 off += k == 3 ? 2048 : (k == 4 ? 64 : 2);
             }
             for (int k = 3; k < mt.levels; ++k) {
@@ -836,6 +1347,54 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_pending_tree(TreeArgs A) {
     PEEK_MARK(22);
 }
 
+// k_tree_global -> k_tree_local -> k_tree_signals on one stream; separate kernels because the three
+// stages want different resources (the sort stages tiles in shared memory, the local stage keeps a
+// whole work item there, the signals want the L1 instead) and none of them needs the others'
+// registers alive.  k_tree_small runs a whole small queue in one CTA, one launch.
+__global__ void __launch_bounds__(GS_THREADS, 1) k_tree_global(TreeArgs A) {
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    __shared__ GsSmem ssm;
+    __shared__ TreeSmem tsm;
+    Grid g{&A.ctl->bar, 0};
+    PEEK_MARK(1);
+    tree_phase0(A, g);
+    const KeyLayout kl = make_layout(A.N, __ldcg(&A.ctl->maxnb), 32);
+    tree_global(A, kl, g, ssm, tsm, gs_stage(dyn_smem));
+    PEEK_MARK(14);
+}
+
+__global__ void __launch_bounds__(GS_THREADS, 1) k_tree_local(TreeArgs A) {
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    __shared__ GsSmem ssm;
+    __shared__ TreeSmem tsm;
+    PEEK_MARK(15);
+    const KeyLayout kg = make_layout(A.N, __ldcg(&A.ctl->maxnb), 32), kl = make_layout(A.N, __ldcg(&A.ctl->maxnb), LOC_W);
+    tree_local_stage(A, kg, kl, false, (int)__ldcg(&A.ctl->fin_cb), (int)__ldcg(&A.ctl->fin_round), ssm, tsm, dyn_smem);
+    PEEK_MARK(20);
+}
+
+__global__ void __launch_bounds__(GS_THREADS, 1) k_tree_signals(TreeArgs A) {
+    __shared__ TreeSmem tsm;
+    __shared__ i32 lvl_hi[LVL_HI_WORDS];
+    Grid g{&A.ctl->bar2, 0};
+    PEEK_MARK(23);
+    tree_signals(A, g, tsm, lvl_hi);
+}
+
+__global__ void __launch_bounds__(GS_THREADS, 1) k_tree_small(TreeArgs A) {
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    __shared__ GsSmem ssm;
+    __shared__ TreeSmem tsm;
+    Grid g{&A.ctl->bar, 0};  // one CTA: every grid barrier is a CTA barrier
+    PEEK_MARK(1);
+    tree_phase0(A, g);
+    const KeyLayout kl = make_layout(A.N, __ldcg(&A.ctl->maxnb), LOC_W);
+    tree_local_stage(A, kl, kl, true, 0, 0, ssm, tsm, dyn_smem);
+    __syncthreads();
+    PEEK_MARK(23);
+    tree_signals(A, g, tsm, (i32*)dyn_smem);  // the work item's buffers are free now
+}
+
 static void tree_layout(Arena& a, i64 N, int grid, TreeArgs& A) {
     A.ctl = a.take<TreeCtl>(1);
     A.bufs.hist = a.take<u32>(gs_hist_words(grid));  // directly after ctl: one memset clears both
@@ -845,11 +1404,12 @@ static void tree_layout(Arena& a, i64 N, int grid, TreeArgs& A) {
     A.bufs.val[1] = a.take<u32>(N);
     A.seg = a.take<u32>(N);
     A.srank = a.take<u32>(N);
-    A.lasth = a.take<u64>(N);
+    A.rec = a.take<ReqRec>(N);
     A.seghead = a.take<u64>(N);
     A.segdepth = a.take<i32>(N);
     A.agg = a.take<i64>(grid);
     A.gsz = a.take<i32>(N);
+    A.biglist = a.take<u64>(N / 64 + 64);
     A.mt_buf = a.take<i32>(mintree_words(N));
 }
 
@@ -860,6 +1420,11 @@ i64 pending_tree_ws_bytes(i64 N) {
     TreeArgs A;
     tree_layout(a, N, MAX_GRID, A);
     return a.used;
+}
+
+static int g_tree_local_cap = 0;  // PEEK_OPT_TREE_LOCAL_CAP (0 = LOC_CAP)
+void tree_set_option(int key, i64 v) {
+    if (key == PEEK_OPT_TREE_LOCAL_CAP) g_tree_local_cap = (int)v;
 }
 
 }  // namespace peek
@@ -881,17 +1446,32 @@ static peek_status tree_launch(const u64* hashes, const i64* blk_off, i64 N, i32
     A.cluster_depth = cluster_depth; A.cluster_size = cluster_size; A.cluster_id = cluster_id;
     A.n_groups = n_groups;
     A.signals_only = signals_only;
+    // what one CTA finishes alone: segments of up to cap_seg positions; those above the quantum are
+    // work items of their own, the others are taken a quantum of positions at a time
+    A.cap_seg = (g_tree_local_cap >= 128 && g_tree_local_cap < LOC_CAP) ? g_tree_local_cap : LOC_CAP;
+    A.quantum = A.cap_seg / 2;
     tree_layout(a, N, MAX_GRID, A);
     PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(MAX_GRID)) - (char*)A.ctl), st));
     void* params[] = {&A};
-    Prof pr(PROF_TREE, st, 1);
-    static bool attr_set = false;
-    if (!attr_set) {
-        PEEK_CUDA(cudaFuncSetAttribute(k_pending_tree, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_STAGE_BYTES));
-        attr_set = true;
+    const bool want_signals = group_id || group_size || n_groups || cluster_depth || cluster_size || cluster_id;
+    if (!signals_only && N <= (i64)A.cap_seg) {  // the whole queue in one CTA, one launch, no grid barrier
+        Prof pr(PROF_TREE, st, 1);
+        PEEK_CUDA(func_smem_optin((const void*)k_tree_small, TREE_DYN_SMEM));
+        k_tree_small<<<1, GS_THREADS, TREE_DYN_SMEM, st>>>(A);
+        PEEK_CUDA(cudaGetLastError());
+        return PEEK_OK;
     }
-    PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_pending_tree, dim3(grid), dim3(GS_THREADS), params,
-                                          GS_STAGE_BYTES, st));
+    Prof pr(PROF_TREE, st, (signals_only ? 0 : 2) + (want_signals ? 1 : 0));
+    if (!signals_only) {
+        PEEK_CUDA(func_smem_optin((const void*)k_tree_global, GS_STAGE_BYTES));
+        PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_tree_global, dim3(grid), dim3(GS_THREADS), params,
+                                              GS_STAGE_BYTES, st));
+        PEEK_CUDA(func_smem_optin((const void*)k_tree_local, TREE_DYN_SMEM));
+        k_tree_local<<<grid, GS_THREADS, TREE_DYN_SMEM, st>>>(A);
+        PEEK_CUDA(cudaGetLastError());
+    }
+    if (want_signals)
+        PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_tree_signals, dim3(grid), dim3(GS_THREADS), params, 0, st));
     return PEEK_OK;
 }
 
@@ -902,7 +1482,7 @@ extern "C" peek_status peek_pending_tree(const uint64_t* hashes, const int64_t* 
                                          void* ws, int64_t ws_bytes, void* stream) {
     if (N < 0 || N >= 0x7fffffffLL) { set_error("peek_pending_tree: N out of range"); return PEEK_ERR_INVALID_ARG; }
     if (N == 0) return PEEK_OK;
-    if (!blk_off || !order || !lcp) { set_error("peek_pending_tree: NULL argument"); return PEEK_ERR_INVALID_ARG; }
+    if (!hashes || !blk_off || !order || !lcp) { set_error("peek_pending_tree: NULL argument"); return PEEK_ERR_INVALID_ARG; }
     if (!ws || ((uintptr_t)ws & 255) || ws_bytes < pending_tree_ws_bytes(N)) {
         set_error("peek_pending_tree: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;

@@ -264,6 +264,48 @@ def test_persistent_kernels_multi_tile(grid_limit):
         b.set_option(b.OPT_GRID_LIMIT, 0)
 
 
+def _tree_only(b, reqs):
+    """peek_pending_tree alone against the oracle, every output."""
+    toks, off = _csr(reqs)
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    d_h = _dev(o_h.view(np.int64), torch.uint64) if o_h.shape[0] else torch.zeros(0, dtype=torch.uint64, device=DEV)
+    gt = b.peek_pending_tree(d_h, _dev(o_bo))
+    ot = oracle.pending_tree(o_h, o_bo)
+    for name in ("order", "lcp", "group_id", "group_size", "cluster_depth", "cluster_size", "cluster_id"):
+        assert np.array_equal(_np(getattr(gt, name)), getattr(ot, name)), name
+    assert int(gt.n_groups.item()) == ot.n_groups
+
+
+@pytest.mark.parametrize("local_cap", [128, 700, 4096, 0])
+@pytest.mark.parametrize("grid_limit", [2, 0])
+def test_pending_tree_local_stage(local_cap, grid_limit):
+    """peek_pending_tree's two stages with the local capacity lowered (PEEK_OPT_TREE_LOCAL_CAP): segments
+    above the capacity go through more grid-wide rounds, those above the quantum are work items of
+    their own, the rest is taken a quantum of positions at a time - deeply nested queues (tiny
+    vocabulary), flat ones (big vocabulary), many duplicates, and sizes around the capacities."""
+    b = _b()
+    rng = np.random.default_rng(1234 + local_cap)
+    b.set_option(b.OPT_TREE_LOCAL_CAP, local_cap)
+    b.set_option(b.OPT_GRID_LIMIT, grid_limit)
+    try:
+        for n in (127, 129, 1500, 12288, 12289, 30011):
+            reqs, _ = _nested_queue(rng, n)
+            _tree_only(b, reqs)
+        flat = [rng.integers(0, 128256, size=int(rng.integers(0, 200))).astype(np.int32) for _ in range(20000)]
+        _tree_only(b, flat)
+        base = rng.integers(0, 9, size=4000).astype(np.int32)
+        nested = [base[: int(rng.integers(0, 4000))] for _ in range(9000)]  # every request a prefix of one chain
+        _tree_only(b, nested)
+        dup = [flat[int(rng.integers(0, 50))] for _ in range(14000)]        # 50 distinct chains
+        _tree_only(b, dup)
+        shared = [np.concatenate([base[:1600], rng.integers(0, 3, size=int(rng.integers(0, 90)))]).astype(np.int32)
+                  for _ in range(15000)]                                    # one long shared prefix
+        _tree_only(b, shared)
+    finally:
+        b.set_option(b.OPT_TREE_LOCAL_CAP, 0)
+        b.set_option(b.OPT_GRID_LIMIT, 0)
+
+
 def test_rank_two_phase_wide_keys():
     """cLPM keys too wide for one 64-bit packed key (full-range hit, cluster size and arrival):
     the arrival sort followed by the stable (hit, cluster size) sort."""
