@@ -48,7 +48,7 @@ static constexpr int TREE_DYN_SMEM = LOC_CAP * 18;    // u64 key + u32 request +
 static_assert(TREE_DYN_SMEM >= GS_STAGE_BYTES, "the grid sort stages its tiles in the same buffer");
 static_assert(LOC_CAP <= 32768, "local positions are kept in 15 bits of a u16");
 static constexpr int W0_BITS = 16;                    // round 0: leading bits of the first hash word
-static constexpr int LOC_W = 16;                      // digit width of the local stage's keys
+static constexpr int LOC_W = 24;                      // digit width of the local stage's keys
 
 struct TreeCtl {      // device control block (zeroed by the host before launch)
     u32 bar;          // grid barrier word
@@ -73,13 +73,20 @@ struct __align__(32) ReqRec {
     u64 lasth;  // last word of the chain (0 for an empty chain): "does one chain prefix the other"
     u64 k0;     // first word (0 for an empty chain): the first unknown word of a segment at depth 0
 };
-__device__ __forceinline__ void rec_head(const ReqRec* __restrict__ rec, u32 r, i64& ao, i32& na) {
-    const ulonglong2 v = __ldg((const ulonglong2*)(rec + r));
-    ao = (i64)v.x; na = (i32)(u32)v.y;
+// the whole record in one 256-bit load that asks L2 to keep the line (the records are gathered again
+// every round; the hash-array probes below are marked evict-first instead)
+__device__ __forceinline__ void rec_load(const ReqRec* __restrict__ rec, u32 r, i64& ao, i32& na, u64& lasth, u64& k0) {
+    u64 a, b;
+    asm volatile("ld.global.nc.L2::evict_last.v4.b64 {%0,%1,%2,%3}, [%4];"
+                 : "=l"(a), "=l"(b), "=l"(lasth), "=l"(k0) : "l"(rec + r));
+    ao = (i64)a; na = (i32)(u32)b;
 }
-__device__ __forceinline__ void rec_tail(const ReqRec* __restrict__ rec, u32 r, u64& lasth, u64& k0) {
-    const ulonglong2 v = __ldg((const ulonglong2*)(rec + r) + 1);
-    lasth = v.x; k0 = v.y;
+// a word of the hash array: read-once random sector, first in line for eviction from L2
+__device__ __forceinline__ u64 ldh(const u64* p) {
+    u64 pol, v;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("ld.global.nc.L2::cache_hint.u64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
+    return v;
 }
 
 struct TreeArgs {
@@ -103,6 +110,7 @@ struct TreeArgs {
     i64* agg;         // gridDim scratch for grid scans
     i32* gsz;         // N   unresolved segment size by segment start; later group size by group id
     u64* biglist;     // segments above the quantum: start | size << 32
+    unsigned short* posna;  // N by position: chain length of an unresolved position (0xffff: see the record)
     i32* mt_buf;      // min hierarchy
 };
 
@@ -225,11 +233,14 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
                                              const bool (&act)[K], i32 (&res)[K],
                                              const u64 (&alast)[K],  // alast[k] = H[ao[k] + na[k] - 1]
                                              const u64 (&k0a)[K], const u64 (&k0b)[K],  // first words
-                                             i32& hint) {            // in/out, < 0: none
+                                             i32& hint,              // in/out, < 0: none
+                                             int& mode) {            // in/out: 1 = try the hint before (1)
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    i32 L[K], R[K];  // while go: equal below/at L (L = lo - 1: nothing known), differ at R
-    bool go[K];
+    // while go: equal below/at L (L = lo - 1: nothing known); differ at R - known once R < Rm or the
+    // last common word has been compared (lastdone)
+    i32 L[K], R[K], Rm[K];
+    bool go[K], lastdone[K];
     u64 x[K], y[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) {
@@ -237,36 +248,44 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
         go[k] = act[k] && m > lo[k];
         if (act[k] && !go[k]) res[k] = m;
         L[k] = lo[k] - 1;
-        R[k] = m - 1;
+        R[k] = Rm[k] = m - 1;
+        lastdone[k] = false;
     }
-    // (1) the last common word
+    // (1) the last common word, for the pairs selected by sel[k] that can still be prefixes
+    auto probe_last = [&](const bool (&sel)[K]) {
 #pragma unroll
-    for (int k = 0; k < K; ++k) {
-        if (go[k]) {
-            x[k] = R[k] == na[k] - 1 ? alast[k] : __ldg(H + ao[k] + R[k]);
-            y[k] = __ldg(H + bo[k] + R[k]);
+        for (int k = 0; k < K; ++k) {
+            if (go[k] && sel[k] && R[k] == Rm[k]) {
+                x[k] = R[k] == na[k] - 1 ? alast[k] : ldh(H + ao[k] + R[k]);
+                y[k] = ldh(H + bo[k] + R[k]);
+            }
         }
-    }
 #pragma unroll
-    for (int k = 0; k < K; ++k)
-        if (go[k] && x[k] == y[k]) { res[k] = R[k] + 1; go[k] = false; }
+        for (int k = 0; k < K; ++k) {
+            if (go[k] && sel[k] && R[k] == Rm[k]) {
+                lastdone[k] = true;
+                if (x[k] == y[k]) { res[k] = R[k] + 1; go[k] = false; }
+                else if (R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
+            }
+        }
+    };
     // probe words g - 1 and g of the pairs selected by pr[k] (one round trip): settles the pair when
     // g is the answer.  first = also probe word lo (the first unknown word) in the same round trip.
-    auto probe_around = [&](const i32 (&gk)[K], const bool (&pr)[K], bool first) {
+    auto probe_around = [&](const i32 (&gk)[K], const bool (&pr)[K], bool first, const bool (&fsel)[K]) {
         u64 x2[K], y2[K], x3[K], y3[K];
         bool p0[K], p1[K], p2[K];
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            p0[k] = first && go[k];
+            p0[k] = first && go[k] && fsel[k];
             p1[k] = pr[k] && gk[k] - 1 > L[k] + (first ? 1 : 0) && gk[k] - 1 < R[k];
             p2[k] = pr[k] && gk[k] > L[k] + (first ? 1 : 0) && gk[k] < R[k];
             x3[k] = y3[k] = 0;
             if (p0[k]) {
                 if (lo[k] == 0) { x3[k] = k0a[k]; y3[k] = k0b[k]; }
-                else { x3[k] = __ldg(H + ao[k] + lo[k]); y3[k] = __ldg(H + bo[k] + lo[k]); }
+                else { x3[k] = ldh(H + ao[k] + lo[k]); y3[k] = ldh(H + bo[k] + lo[k]); }
             }
-            if (p1[k]) { x[k] = __ldg(H + ao[k] + gk[k] - 1); y[k] = __ldg(H + bo[k] + gk[k] - 1); }
-            if (p2[k]) { x2[k] = __ldg(H + ao[k] + gk[k]); y2[k] = __ldg(H + bo[k] + gk[k]); }
+            if (p1[k]) { x[k] = ldh(H + ao[k] + gk[k] - 1); y[k] = ldh(H + bo[k] + gk[k] - 1); }
+            if (p2[k]) { x2[k] = ldh(H + ao[k] + gk[k]); y2[k] = ldh(H + bo[k] + gk[k]); }
         }
 #pragma unroll
         for (int k = 0; k < K; ++k) {
@@ -276,7 +295,7 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
             }
             if (p1[k]) { if (x[k] == y[k]) L[k] = gk[k] - 1; else R[k] = gk[k] - 1; }
             if (p2[k] && gk[k] < R[k]) { if (x2[k] == y2[k]) L[k] = gk[k]; else R[k] = gk[k]; }
-            if (go[k] && (p0[k] || pr[k]) && R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
+            if (go[k] && (p0[k] || pr[k]) && R[k] - L[k] <= 1 && (R[k] < Rm[k] || lastdone[k])) { res[k] = R[k]; go[k] = false; }
         }
     };
     // one bisection step for the elements selected by sel[k]; returns whether any is still going
@@ -285,7 +304,7 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
         for (int k = 0; k < K; ++k) {
             if (go[k] && sel[k]) {
                 const i32 p = (L[k] + R[k]) >> 1;
-                x[k] = __ldg(H + ao[k] + p); y[k] = __ldg(H + bo[k] + p);
+                x[k] = ldh(H + ao[k] + p); y[k] = ldh(H + bo[k] + p);
             }
         }
         bool any = false;
@@ -300,16 +319,41 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
         }
         return any;
     };
+    bool all_sel[K], doneB[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) { all_sel[k] = true; doneB[k] = false; }
+    // (2) the first unknown word and this lane's previous answer
+    auto probe_hint = [&](const bool (&sel)[K]) {
+        i32 gk[K];
+        bool pr[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) { gk[k] = hint; pr[k] = go[k] && sel[k] && hint >= 0; }
+        probe_around(gk, pr, true, sel);
+#pragma unroll
+        for (int k = 0; k < K; ++k) doneB[k] |= sel[k];
+    };
+    {   // lanes whose previous element branched try that depth first: it usually settles the pair
+        // and then the last common word is never read
+        bool early[K];
+        bool e = false;
+#pragma unroll
+        for (int k = 0; k < K; ++k) { early[k] = go[k] && mode == 1 && hint >= 0; e |= early[k]; }
+        if (__any_sync(FULL, e)) probe_hint(early);
+    }
     bool pending = false;
 #pragma unroll
     for (int k = 0; k < K; ++k) pending |= go[k];
-    if (__any_sync(FULL, pending)) {
-        {   // (2) the first unknown word and this lane's previous answer
-            i32 gk[K];
-            bool pr[K];
+    if (__any_sync(FULL, pending)) probe_last(all_sel);
+    pending = false;
 #pragma unroll
-            for (int k = 0; k < K; ++k) { gk[k] = hint; pr[k] = go[k] && hint >= 0; }
-            probe_around(gk, pr, true);
+    for (int k = 0; k < K; ++k) pending |= go[k];
+    if (__any_sync(FULL, pending)) {
+        {
+            bool late[K];
+            bool e = false;
+#pragma unroll
+            for (int k = 0; k < K; ++k) { late[k] = go[k] && !doneB[k]; e |= late[k]; }
+            if (__any_sync(FULL, e)) probe_hint(late);
             pending = false;
 #pragma unroll
             for (int k = 0; k < K; ++k) pending |= go[k];
@@ -332,17 +376,19 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
                 gk[k] = __shfl_sync(FULL, res[k], leader[k] < 0 ? 0 : leader[k]);
                 pr[k] = go[k] && leader[k] >= 0;
             }
-            probe_around(gk, pr, false);
+            probe_around(gk, pr, false, all_sel);
         }
     }
-    bool all_sel[K];
-#pragma unroll
-    for (int k = 0; k < K; ++k) all_sel[k] = true;
     bool any = true;
     while (any) any = step(all_sel);  // (4)
 #pragma unroll
-    for (int k = 0; k < K; ++k)
-        if (act[k]) hint = res[k];
+    for (int k = 0; k < K; ++k) {
+        if (act[k]) {
+            const bool branched = res[k] <= Rm[k];  // not a prefix relation
+            mode = branched ? 1 : 0;
+            if (branched) hint = res[k];
+        }
+    }
 }
 
 // new sort key of a classified member (l = LCP with the head in words; wa / wb = the two words at l)
@@ -439,11 +485,12 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
         else { lb.key[i] = round0_key(kl, __ldcg(A.srank + i)); r = (u32)i; }
         lb.val[i] = r;
         lb.idx[i] = (unsigned short)i;
-        const u32 na = __ldg(&rec[r].na);
-        lb.na[i] = (unsigned short)(na < 0xffffu ? na : 0xffffu);
+        if (mode == LOCAL_FROM_GLOBAL) lb.na[i] = __ldcg(A.posna + p0 + i);
+        else { const u32 na = __ldg(&rec[r].na); lb.na[i] = (unsigned short)(na < 0xffffu ? na : 0xffffu); }
     }
     __syncthreads();
     i32 hint = -1;
+    int hmode = 0;
     u64 vary = mode == LOCAL_WHOLE_QUEUE ? round0_vary(kl, __ldcg(&A.ctl->flags)) : 0;
     for (int lr = mode == LOCAL_WHOLE_QUEUE ? 1 : 0;; ++lr) {
         // stable sort of the range by the keys of the last classification (round 0: the first words)
@@ -579,24 +626,23 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
                     if (un[k]) {
                         hv[k] = __ldcg(A.seghead + p0 + sg[k]);
                         lo[k] = __ldcg(A.segdepth + p0 + sg[k]);
-                        rec_head(rec, r[k], ao[k], na[k]);
-                        rec_tail(rec, r[k], al[k], k0a[k]);
+                        rec_load(rec, r[k], ao[k], na[k], al[k], k0a[k]);
                     }
                 }
                 LSUBS(k) { h[k] = un[k] ? lb.val[lb.idx[0xffffffffu - (u32)hv[k]]] : 0u; nb[k] = (i32)(hv[k] >> 32); }
                 LSUBS(k) {
                     bo[k] = 0; k0b[k] = 0;
-                    if (un[k]) { i32 nh; u64 lh; rec_head(rec, h[k], bo[k], nh); rec_tail(rec, h[k], lh, k0b[k]); }
+                    if (un[k]) { i32 nh; u64 lh; rec_load(rec, h[k], bo[k], nh, lh, k0b[k]); }
                     cmp[k] = un[k] && r[k] != h[k];
                     l[k] = na[k];  // r == h: the head itself
                 }
                 PEEK_MARK(40 + hb);
-                lcp_lockstep<LSB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, hint);
+                lcp_lockstep<LSB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, hint, hmode);
                 PEEK_MARK(60 + hb);
                 u64 wa[LSB], wb[LSB];
                 LSUBS(k) {
                     wa[k] = wb[k] = 0;
-                    if (un[k] && l[k] < na[k]) { wa[k] = __ldg(H + ao[k] + l[k]); wb[k] = __ldg(H + bo[k] + l[k]); }
+                    if (un[k] && l[k] < na[k]) { wa[k] = ldh(H + ao[k] + l[k]); wb[k] = ldh(H + bo[k] + l[k]); }
                 }
                 LSUBS(k) {
                     if (val_[k]) {
@@ -888,6 +934,10 @@ __device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& 
                     }
                     u32 nbr[SB];
                     SUBS(k) nbr[k] = un[k] ? __ldg(&A.rec[r[k]].na) : 0u;
+                    SUBS(k) {  // kept by position for the local stage (its head search needs no gather then)
+                        const i64 i = IDX(t, hb * SB + k);
+                        if (i < c1) A.posna[i] = (unsigned short)(un[k] && nbr[k] < 0xffffu ? nbr[k] : 0xffffu);
+                    }
                     SUBS(k) {
                         // head = longest chain of the segment, lowest position on ties: segmented
                         // max over the row's runs of equal s, one atomic per run
@@ -938,6 +988,7 @@ __device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& 
             u64* Kw = A.bufs.key[cb];
             u64 orv = 0, andv = ~0ull;
             i32 hint = -1;
+            int hmode = 0;
             for (int t = 0; t < ntiles; ++t)
             for (int hb = 0; hb < GS_KPT / SB; ++hb) {
                 u32 sg[SB], r[SB], h[SB], rk[SB];
@@ -957,22 +1008,21 @@ __device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& 
                         const u32 s = sg[k] & 0x7fffffffu;
                         hv[k] = __ldcg(A.seghead + s);
                         lo[k] = __ldcg(A.segdepth + s);
-                        rec_head(A.rec, r[k], ao[k], na[k]);
-                        rec_tail(A.rec, r[k], al[k], k0a[k]);
+                        rec_load(A.rec, r[k], ao[k], na[k], al[k], k0a[k]);
                     }
                 }
                 SUBS(k) { h[k] = un[k] ? __ldcg(cur + (0xffffffffu - (u32)hv[k])) : 0u; nb[k] = (i32)(hv[k] >> 32); }
                 SUBS(k) {
                     bo[k] = 0; k0b[k] = 0;
-                    if (un[k]) { i32 nh; u64 lh; rec_head(A.rec, h[k], bo[k], nh); rec_tail(A.rec, h[k], lh, k0b[k]); }
+                    if (un[k]) { i32 nh; u64 lh; rec_load(A.rec, h[k], bo[k], nh, lh, k0b[k]); }
                     cmp[k] = un[k] && r[k] != h[k];
                     l[k] = na[k];  // r == h: the head itself
                 }
-                lcp_lockstep<SB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, hint);
+                lcp_lockstep<SB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, hint, hmode);
                 u64 wa[SB], wb[SB];
                 SUBS(k) {
                     wa[k] = wb[k] = 0;
-                    if (un[k] && l[k] < na[k]) { wa[k] = __ldg(H + ao[k] + l[k]); wb[k] = __ldg(H + bo[k] + l[k]); }
+                    if (un[k] && l[k] < na[k]) { wa[k] = ldh(H + ao[k] + l[k]); wb[k] = ldh(H + bo[k] + l[k]); }
                 }
                 SUBS(k) {
                     const i64 i = IDX(t, hb * SB + k);
@@ -1410,6 +1460,7 @@ static void tree_layout(Arena& a, i64 N, int grid, TreeArgs& A) {
     A.agg = a.take<i64>(grid);
     A.gsz = a.take<i32>(N);
     A.biglist = a.take<u64>(N / 64 + 64);
+    A.posna = a.take<unsigned short>(N);
     A.mt_buf = a.take<i32>(mintree_words(N));
 }
 
