@@ -89,6 +89,16 @@ __device__ __forceinline__ u64 ldh(const u64* p) {
     return v;
 }
 
+// per-segment record of the local stage, by segment start: what every member needs for its
+// classification, in one sector
+struct __align__(32) SegRec {
+    unsigned long long head;  // (nb << 32) | ~position of the longest chain (atomicMax)
+    u64 bo;                   // the head's blk_off
+    u64 k0b;                  // the head's first word
+    u32 depth;                // blocks all members are known to share
+    u32 rank;                 // dense rank of the segment inside the work item
+};
+
 struct TreeArgs {
     const u64* hashes;
     const i64* blk_off;
@@ -110,6 +120,7 @@ struct TreeArgs {
     i64* agg;         // gridDim scratch for grid scans
     i32* gsz;         // N   unresolved segment size by segment start; later group size by group id
     u64* biglist;     // segments above the quantum: start | size << 32
+    SegRec* segrec;   // N   by segment start (local stage)
     unsigned short* posna;  // N by position: chain length of an unresolved position (0xffff: see the record)
     i32* mt_buf;      // min hierarchy
 };
@@ -233,6 +244,7 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
                                              const bool (&act)[K], i32 (&res)[K],
                                              const u64 (&alast)[K],  // alast[k] = H[ao[k] + na[k] - 1]
                                              const u64 (&k0a)[K], const u64 (&k0b)[K],  // first words
+                                             u64 (&wx)[K], u64 (&wy)[K],  // out: the two words at res when the chains branch
                                              i32& hint,              // in/out, < 0: none
                                              int& mode) {            // in/out: 1 = try the hint before (1)
     const unsigned FULL = 0xffffffffu;
@@ -250,6 +262,7 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
         L[k] = lo[k] - 1;
         R[k] = Rm[k] = m - 1;
         lastdone[k] = false;
+        wx[k] = wy[k] = 0;
     }
     // (1) the last common word, for the pairs selected by sel[k] that can still be prefixes
     auto probe_last = [&](const bool (&sel)[K]) {
@@ -265,7 +278,8 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
             if (go[k] && sel[k] && R[k] == Rm[k]) {
                 lastdone[k] = true;
                 if (x[k] == y[k]) { res[k] = R[k] + 1; go[k] = false; }
-                else if (R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
+                else { wx[k] = x[k]; wy[k] = y[k]; }
+                if (go[k] && R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
             }
         }
     };
@@ -290,11 +304,11 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             if (p0[k]) {
-                if (x3[k] != y3[k]) { res[k] = lo[k]; go[k] = false; p1[k] = p2[k] = false; }
+                if (x3[k] != y3[k]) { res[k] = lo[k]; go[k] = false; p1[k] = p2[k] = false; wx[k] = x3[k]; wy[k] = y3[k]; }
                 else L[k] = lo[k];
             }
-            if (p1[k]) { if (x[k] == y[k]) L[k] = gk[k] - 1; else R[k] = gk[k] - 1; }
-            if (p2[k] && gk[k] < R[k]) { if (x2[k] == y2[k]) L[k] = gk[k]; else R[k] = gk[k]; }
+            if (p1[k]) { if (x[k] == y[k]) L[k] = gk[k] - 1; else { R[k] = gk[k] - 1; wx[k] = x[k]; wy[k] = y[k]; } }
+            if (p2[k] && gk[k] < R[k]) { if (x2[k] == y2[k]) L[k] = gk[k]; else { R[k] = gk[k]; wx[k] = x2[k]; wy[k] = y2[k]; } }
             if (go[k] && (p0[k] || pr[k]) && R[k] - L[k] <= 1 && (R[k] < Rm[k] || lastdone[k])) { res[k] = R[k]; go[k] = false; }
         }
     };
@@ -312,7 +326,7 @@ __device__ __forceinline__ void lcp_lockstep(const u64* __restrict__ H, const i6
         for (int k = 0; k < K; ++k) {
             if (go[k] && sel[k]) {
                 const i32 p = (L[k] + R[k]) >> 1;
-                if (x[k] == y[k]) L[k] = p; else R[k] = p;
+                if (x[k] == y[k]) L[k] = p; else { R[k] = p; wx[k] = x[k]; wy[k] = y[k]; }
                 if (R[k] - L[k] <= 1) { res[k] = R[k]; go[k] = false; }
                 any |= go[k];
             }
@@ -517,7 +531,7 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
                     u64 key, prev, next;
                     keys3(i, valid, key, prev, next);
                     const bool start = valid && (i == 0 || prev != key);
-                    if (start) A.seghead[p0 + i] = 0;  // reset before L1b's maxima (a CTA barrier apart)
+                    if (start) A.segrec[p0 + i].head = 0;  // reset before L1b's maxima (a CTA barrier apart)
                     const unsigned bal = __ballot_sync(FULL, start);
                     wc += __popc(bal);
                     if (bal) wl = (u32)((i - lane) + 31 - __clz(bal)) + 1u;
@@ -566,8 +580,8 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
                     const bool un = br && !(start && last);
                     if (valid) lb.aux[i] = (unsigned short)(s | (un ? 0x8000 : 0));
                     if (start) {
-                        A.srank[p0 + i] = rank;
-                        A.segdepth[p0 + i] = br ? (i32)(kc.ld_of(F) / kc.D) : 0;
+                        A.segrec[p0 + i].rank = rank;
+                        A.segrec[p0 + i].depth = br ? (u32)(kc.ld_of(F) / kc.D) : 0u;
                         if (p0 + i == 0) A.lcp[0] = 0;
                         else if (i > 0 && lr > 0 && kc.seg_of(prev) == kc.seg_of(key)) {
                             const u64 la = kc.ldv(kc.F_of(prev)), lb2 = kc.ldv(F);
@@ -588,7 +602,7 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
                             if (lane >= o && sx == s && x > v) v = x;
                         }
                         const i32 sn = __shfl_down_sync(FULL, s, 1);
-                        if (v && (lane == 31 || sn != s)) atomicMax((unsigned long long*)&A.seghead[p0 + s], v);
+                        if (v && (lane == 31 || sn != s)) atomicMax(&A.segrec[p0 + s].head, v);
                     }
                 }
             }
@@ -597,6 +611,25 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
         }
         PEEK_MARK(33);
         if (tsm.cnt == 0) break;
+        // ---- L1c: the head's chain offset and first word into every unresolved segment's record ----
+#pragma unroll
+        for (int k = 0; k < LOC_K; ++k) {
+            if (k < Kp) {
+                const int i = wbase + k * 32 + lane;
+                if (i < n) {
+                    const u32 a = lb.aux[i];
+                    if (a == (0x8000u | (u32)i)) {  // an unresolved segment starts here
+                        const unsigned long long hv = __ldcg(&A.segrec[p0 + i].head);
+                        const u32 h = lb.val[lb.idx[0xffffffffu - (u32)hv]];
+                        i64 bo; i32 nh; u64 lh, k0b;
+                        rec_load(rec, h, bo, nh, lh, k0b);
+                        A.segrec[p0 + i].bo = (u64)bo;
+                        A.segrec[p0 + i].k0b = k0b;
+                    }
+                }
+            }
+        }
+        __syncthreads();
         // ---- L2: classify every unresolved position against its segment head.  The new key
         // replaces the element's old one in place: this phase reads no neighbour's key ----
         {
@@ -621,29 +654,25 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
                     }
                 }
                 LSUBS(k) {
-                    rk[k] = 0; hv[k] = 0; ao[k] = 0; na[k] = 0; lo[k] = 0; al[k] = 0; k0a[k] = 0;
-                    if (val_[k]) rk[k] = __ldcg(A.srank + p0 + sg[k]);
-                    if (un[k]) {
-                        hv[k] = __ldcg(A.seghead + p0 + sg[k]);
-                        lo[k] = __ldcg(A.segdepth + p0 + sg[k]);
-                        rec_load(rec, r[k], ao[k], na[k], al[k], k0a[k]);
+                    rk[k] = 0; hv[k] = 0; ao[k] = 0; na[k] = 0; lo[k] = 0; al[k] = 0; k0a[k] = 0; bo[k] = 0; k0b[k] = 0;
+                    if (val_[k]) {
+                        const ulonglong2* sp = (const ulonglong2*)(A.segrec + p0 + sg[k]);
+                        const ulonglong2 s0 = __ldcg(sp), s1 = __ldcg(sp + 1);
+                        hv[k] = s0.x; bo[k] = (i64)s0.y; k0b[k] = s1.x;
+                        lo[k] = (i32)(u32)s1.y; rk[k] = (u32)(s1.y >> 32);
                     }
+                    if (un[k]) rec_load(rec, r[k], ao[k], na[k], al[k], k0a[k]);
                 }
-                LSUBS(k) { h[k] = un[k] ? lb.val[lb.idx[0xffffffffu - (u32)hv[k]]] : 0u; nb[k] = (i32)(hv[k] >> 32); }
                 LSUBS(k) {
-                    bo[k] = 0; k0b[k] = 0;
-                    if (un[k]) { i32 nh; u64 lh; rec_load(rec, h[k], bo[k], nh, lh, k0b[k]); }
-                    cmp[k] = un[k] && r[k] != h[k];
-                    l[k] = na[k];  // r == h: the head itself
+                    nb[k] = (i32)(hv[k] >> 32);
+                    const int kk = hb * LSB + k;
+                    cmp[k] = un[k] && (u32)(wbase + kk * 32 + lane) != 0xffffffffu - (u32)hv[k];  // not the head itself
+                    l[k] = na[k];
                 }
                 PEEK_MARK(40 + hb);
-                lcp_lockstep<LSB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, hint, hmode);
-                PEEK_MARK(60 + hb);
                 u64 wa[LSB], wb[LSB];
-                LSUBS(k) {
-                    wa[k] = wb[k] = 0;
-                    if (un[k] && l[k] < na[k]) { wa[k] = ldh(H + ao[k] + l[k]); wb[k] = ldh(H + bo[k] + l[k]); }
-                }
+                lcp_lockstep<LSB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, wa, wb, hint, hmode);
+                PEEK_MARK(60 + hb);
                 LSUBS(k) {
                     if (val_[k]) {
                         const u64 nk = un[k] ? class_key(kl, rk[k], l[k], na[k], nb[k], wa[k], wb[k])
@@ -1018,12 +1047,8 @@ __device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& 
                     cmp[k] = un[k] && r[k] != h[k];
                     l[k] = na[k];  // r == h: the head itself
                 }
-                lcp_lockstep<SB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, hint, hmode);
                 u64 wa[SB], wb[SB];
-                SUBS(k) {
-                    wa[k] = wb[k] = 0;
-                    if (un[k] && l[k] < na[k]) { wa[k] = ldh(H + ao[k] + l[k]); wb[k] = ldh(H + bo[k] + l[k]); }
-                }
+                lcp_lockstep<SB>(H, ao, na, bo, nb, lo, cmp, l, al, k0a, k0b, wa, wb, hint, hmode);
                 SUBS(k) {
                     const i64 i = IDX(t, hb * SB + k);
                     if (i < c1) {
@@ -1461,6 +1486,7 @@ static void tree_layout(Arena& a, i64 N, int grid, TreeArgs& A) {
     A.gsz = a.take<i32>(N);
     A.biglist = a.take<u64>(N / 64 + 64);
     A.posna = a.take<unsigned short>(N);
+    A.segrec = a.take<SegRec>(N);
     A.mt_buf = a.take<i32>(mintree_words(N));
 }
 
