@@ -308,6 +308,17 @@ enum { PEEK_OPT_LPM_STRATEGY = 1, PEEK_OPT_LPM_WINDOW = 2, PEEK_OPT_GRID_LIMIT =
 enum { PEEK_LPM_AUTO = 0, PEEK_LPM_DUAL_WALK = 1, PEEK_LPM_SPECULATIVE = 2 };
 peek_status peek_set_option(int32_t key, int64_t value);
 
+/* ---- work counters of peek_lpm (the amortisation claim) ---- */
+/* counters: NULL (default: off) or uint64[4] [device, caller-owned, zeroed by the caller], valid
+ * until switched off again.  While set, every peek_lpm call ADDS, per mode it runs:
+ * [0] walks started at the root of the cache (one per request without a tree view; one per run of
+ * sorted positions in the dual walk - every other position copies its predecessor's hit or resumes
+ * below their shared prefix), [1] child lookups (radix mode; a resumed walk costs lookups, no
+ * re-descent), [2] tokens compared against edge labels (matched tokens plus the mismatching one),
+ * [3] table slots' first probes (hash mode).  [2] and [3] are the work the dual walk amortises
+ * (PAPER.md:293 O(C x D) against O(N x D)).  Process-wide like the options; results never depend on it. */
+peek_status peek_lpm_counters(uint64_t* counters);
+
 /* ---- tracing (CUDA events per kernel group) --------------------------- */
 /* Off by default.  When on, every kernel group a call enqueues is bracketed by a pair of CUDA
  * events on the caller's stream (up to 512 pairs per slot between reads; later ones are dropped).

@@ -23,7 +23,7 @@ CALL_CLPM_SIGNALS, CALL_CLPM_ORDER_FULL, CALL_CLPM_GROUP_MAJOR, CALL_OFFLINE_PHA
 CALL_PENDING_TREE_UPDATE = 8
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
-           "peek_launch_count", "peek_set_option", "peek_bench_random_gather",
+           "peek_launch_count", "peek_set_option", "peek_bench_random_gather", "peek_lpm_counters",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
            "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1", "peek_radix_demand",
            "peek_clpm_lane_b", "peek_dynamic_lane", "peek_pending_tree_update",
@@ -247,7 +247,7 @@ def peek_lpm(tokens=None, tok_off=None, hashes=None, blk_off=None, radix: Option
     cr = radix._c() if radix is not None else None
     ct = _Table(_ptr(t_keys, U64), int(t_keys.shape[0])) if t_keys is not None else None
     cv = _TreeView(_ptr(tree.order, torch.int32), _ptr(tree.lcp, torch.int32)) if tree is not None else None
-    ws, nbytes = _ws(CALL_LPM, dev, N=N)
+    ws, nbytes = _ws(CALL_LPM, dev, N=N, V=max(int(radix.n_tok_len.shape[0]), int(radix.e_child.shape[0])) if radix is not None else 0)
     if tokens is not None and tokens.numel() == 0:  # all requests empty: still a valid pointer
         tokens = torch.zeros(4, dtype=torch.int32, device=dev)
     st = lib().peek_lpm(_ptr(tokens), _ptr(tok_off),
@@ -421,6 +421,14 @@ def peek_offline_phase1(hashes, blk_off, depth_blocks: int = 8):
 
 OPT_LPM_STRATEGY, OPT_LPM_WINDOW, OPT_GRID_LIMIT, OPT_TREE_LOCAL_CAP = 1, 2, 3, 4
 LPM_AUTO, LPM_DUAL_WALK, LPM_SPECULATIVE = 0, 1, 2
+
+
+def lpm_counters(buf: Optional[torch.Tensor]):
+    """peek_lpm_counters: uint64[4] device tensor that later peek_lpm calls add to, or None (off)."""
+    L = lib()
+    L.peek_lpm_counters.restype = ctypes.c_int32
+    L.peek_lpm_counters.argtypes = [ctypes.c_void_p]
+    _check(L.peek_lpm_counters(_ptr(buf) if buf is not None else None), "peek_lpm_counters")
 
 
 def set_option(key: int, value: int) -> None:

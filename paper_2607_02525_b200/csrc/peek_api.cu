@@ -54,7 +54,7 @@ int sm_count() {
 // ---- tracing ---------------------------------------------------------------------------
 static const char* const g_prof_names[PROF_NSLOTS] = {
     "hash.nb_scan", "hash.content", "hash.chain", "tree.persistent", "lpm.radix_walk", "lpm.hash_probe",
-    "lpm.resolve_scan", "demand.count", "rank.clpm_sort", "signals.clpm", "rank.full_key", "offline.phase1"};
+    "lpm.resolve_scan", "lpm.dual_walk", "demand.count", "rank.clpm_sort", "signals.clpm", "rank.full_key", "offline.phase1"};
 static constexpr int PROF_RING = 512;
 struct ProfSlotState {
     cudaEvent_t ev[PROF_RING][2];
@@ -86,7 +86,7 @@ void prof_end(int slot, cudaStream_t st, int launches) {
 }
 
 i64 block_hash_ws_bytes(i64 N);
-i64 lpm_ws_bytes(i64 N);
+i64 lpm_ws_bytes(i64 N, i64 V);
 i64 pending_tree_ws_bytes(i64 N);
 i64 demand_rank_ws_bytes(i64 N, i64 S);
 i64 clpm_signals_ws_bytes(i64 N);
@@ -118,14 +118,13 @@ extern "C" int32_t peek_version(void) { return 100; }
 
 extern "C" peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t T, int64_t NB,
                                             int64_t S, int64_t V, int64_t* out_bytes) {
-    (void)V;
     if (!out_bytes || N < 0 || S < 0) {
         peek::set_error("peek_workspace_bytes: bad argument");
         return PEEK_ERR_INVALID_ARG;
     }
     switch (call_id) {
         case PEEK_CALL_BLOCK_HASH: *out_bytes = peek::block_hash_ws_bytes(N); break;
-        case PEEK_CALL_LPM: *out_bytes = peek::lpm_ws_bytes(N); break;
+        case PEEK_CALL_LPM: *out_bytes = peek::lpm_ws_bytes(N, V > 0 ? V : 0); break;
         case PEEK_CALL_PENDING_TREE: *out_bytes = peek::pending_tree_ws_bytes(N); break;
         case PEEK_CALL_DEMAND_RANK: *out_bytes = peek::demand_rank_ws_bytes(N, S); break;
         case PEEK_CALL_CLPM_SIGNALS: *out_bytes = peek::clpm_signals_ws_bytes(N); break;

@@ -27,7 +27,7 @@ cudaError_t func_smem_optin(const void* func, int bytes);
 // tracing slots (peek_profile_*)
 enum ProfSlot {
     PROF_HASH_SCAN = 0, PROF_HASH_CONTENT, PROF_HASH_CHAIN, PROF_TREE, PROF_LPM_RADIX, PROF_LPM_HASH,
-    PROF_LPM_RESOLVE, PROF_DEMAND, PROF_RANK, PROF_SIGNALS, PROF_RANK_FULL, PROF_OFFLINE, PROF_NSLOTS
+    PROF_LPM_RESOLVE, PROF_LPM_DUAL, PROF_DEMAND, PROF_RANK, PROF_SIGNALS, PROF_RANK_FULL, PROF_OFFLINE, PROF_NSLOTS
 };
 void prof_begin(int slot, cudaStream_t st);
 void prof_end(int slot, cudaStream_t st, int launches);

@@ -83,15 +83,26 @@ __device__ __forceinline__ i64 match_len(const i32* __restrict__ a, const i32* _
     return limit;
 }
 
+// the dual walk's compare: every round trip looks at 32 x 10 tokens (a turn's new segment, the run of
+// tokens a resumed walk usually has to confirm, fits one trip; loads past `limit` are predicated off)
+__device__ __forceinline__ i64 match_len_wide(const i32* __restrict__ a, const i32* __restrict__ b, i64 limit,
+                                              int lane) {
+    i64 m = limit;
+    for (i64 base = 0; base < limit; base += 320)
+        if (match_step<10>(a, b, base, limit, lane, &m)) return m;
+    return limit > 0 ? limit : 0;
+}
+
 // Walk request tokens s[0..len) from the root.  start > 0: first re-descend to depth `start` by
 // child lookups only (valid when the first `start` tokens are known to be cached).
 __device__ __forceinline__ i32 radix_walk(const RadixDev& R, const i32* __restrict__ s, i64 len,
-                                          i64 start, int lane) {
+                                          i64 start, int lane, u32& c_look, u32& c_tok) {
     i32 v = 0;
     i64 d = 0;
     for (;;) {
         if (d >= len) break;
         i32 t = __ldg(s + d);
+        ++c_look;
         i32 e = find_child(R.e_first_tok, __ldg(R.n_child_off + v), __ldg(R.n_child_off + v + 1), t, lane);
         if (e < 0) break;
         i32 u = __ldg(R.e_child + e);
@@ -105,6 +116,7 @@ __device__ __forceinline__ i32 radix_walk(const RadixDev& R, const i32* __restri
         const i32* lab = R.c_tokens + __ldg(R.n_tok_off + u);
         i64 limit = min(L, len - d);
         i64 m = skip + match_len(lab + skip, s + d + skip, limit - skip, lane);
+        c_tok += (u32)(m - skip) + (m < limit ? 1u : 0u);
         d += m;
         if (m < L) break;
         v = u;
@@ -114,14 +126,21 @@ __device__ __forceinline__ i32 radix_walk(const RadixDev& R, const i32* __restri
 
 __global__ void __launch_bounds__(LPM_THREADS) k_lpm_radix(const i32* __restrict__ tokens,
                                                           const i64* __restrict__ tok_off, i64 N,
-                                                          RadixDev R, i32* __restrict__ out) {
+                                                          RadixDev R, i32* __restrict__ out,
+                                                          unsigned long long* counters) {
     const int lane = threadIdx.x & 31;
     i64 r = ((i64)blockIdx.x * LPM_THREADS + threadIdx.x) >> 5;
     if (r >= N) return;
     i64 o = tok_off[r];
     i64 len = tok_off[r + 1] - o;
-    i32 h = radix_walk(R, tokens + o, len, 0, lane);
+    u32 c_look = 0, c_tok = 0;
+    i32 h = radix_walk(R, tokens + o, len, 0, lane, c_look, c_tok);
     if (lane == 0) out[r] = h;
+    if (counters && lane == 0) {
+        atomicAdd(counters + 0, 1ull);
+        atomicAdd(counters + 1, (unsigned long long)c_look);
+        atomicAdd(counters + 2, (unsigned long long)c_tok);
+    }
 }
 
 __device__ __forceinline__ bool table_has(const u64* __restrict__ t_keys, u64 mask, u64 key) {
@@ -137,7 +156,7 @@ __device__ __forceinline__ bool table_has(const u64* __restrict__ t_keys, u64 ma
 __global__ void __launch_bounds__(LPM_THREADS) k_lpm_hash(const u64* __restrict__ hashes,
                                                          const i64* __restrict__ blk_off, i64 N,
                                                          const u64* __restrict__ t_keys, u64 mask,
-                                                         i32* __restrict__ out) {
+                                                         i32* __restrict__ out, unsigned long long* counters) {
     const int lane = threadIdx.x & 31;
     i64 r = ((i64)blockIdx.x * LPM_THREADS + threadIdx.x) >> 5;
     if (r >= N) return;
@@ -145,14 +164,17 @@ __global__ void __launch_bounds__(LPM_THREADS) k_lpm_hash(const u64* __restrict_
     i64 nb = blk_off[r + 1] - b0;
     i64 i0 = 0;
     i64 hit = nb;
+    u32 c_probe = 0;
     for (; i0 < nb; i0 += 32) {
         i64 i = i0 + lane;
         bool miss = false;
         if (i < nb) miss = !table_has(t_keys, mask, hashes[b0 + i]);
+        c_probe += (u32)__popc(__ballot_sync(0xffffffffu, i < nb));
         unsigned m = __ballot_sync(0xffffffffu, miss);
         if (m) { hit = i0 + (__ffs(m) - 1); break; }
     }
     if (lane == 0) out[r] = (i32)(hit * 16);
+    if (counters && lane == 0) { atomicAdd(counters + 0, 1ull); atomicAdd(counters + 3, (unsigned long long)c_probe); }
 }
 
 // ---- speculative co-descent (small N, long requests) -----------------------------------------
@@ -172,7 +194,8 @@ __global__ void __launch_bounds__(LPM_THREADS) k_lpm_radix_spec(const i32* __res
     i64 start = order ? (i64)lcp[j] * 16 : 0;
     i64 o = tok_off[r];
     i64 len = tok_off[r + 1] - o;
-    i32 h = radix_walk(R, tokens + o, len, start, lane);
+    u32 c_look = 0, c_tok = 0;
+    i32 h = radix_walk(R, tokens + o, len, start, lane, c_look, c_tok);
     if (lane == 0) out[j] = h;  // by sorted position when co-descending, by request otherwise
 }
 
@@ -344,19 +367,54 @@ __global__ void __launch_bounds__(1024) k_resolve_single(const i32* __restrict__
 // ---- dual-walk over the sorted order (PAPER.md:65-90 Alg. 1, :96) ------------------------------
 // A warp owns a RUN of consecutive sorted positions and processes it in order, carrying the
 // predecessor's hit and - in radix mode - the predecessor's path through the cache (the nodes it
-// entered and the depth it entered them at, one entry per lane, in registers).  For position j
-// with s = B*lcp[j] tokens shared with j-1:
+// entered and the depth it entered them at; a stack in shared memory).  For position j with
+// s = B*lcp[j] tokens shared with j-1:
 //     hit(j-1) <  s : hit(j) = hit(j-1), nothing is read from the cache
 //     hit(j-1) >= s : pop the path back to depth s and resume the walk inside the node that covers
 //                     s - no re-descent from the root, no compares below s
 // which is the co-descent of the pending trie (order + lcp) against the radix cache: one cache
 // walk per pending edge.  Runs are cut at the position of minimal lcp inside fixed windows of
 // `win` positions (cheap heads: a run head has no predecessor and does a full walk from the root).
-// Small CTAs: a CTA lives as long as its slowest warp and run lengths vary a lot, so fewer warps
-// per CTA keep more of the SM's warp slots busy (config 5: radix 0.335 -> 0.293 ms at 64 threads,
-// hash 0.184 -> 0.173 ms at 128).
-static constexpr int DW_THREADS = 64;    // k_lpm_radix_dual
-static constexpr int DWH_THREADS = 128;  // k_lpm_hash_dual
+//
+// ONE persistent kernel serves both modes: its warps draw work items from an atomic counter, the
+// radix windows first (they are the longer ones), then the hash windows, so the two modes overlap
+// and the tail of one is filled by the other.  What the radix walk reads per node is packed:
+//   * k_lpm_prep builds one 32-byte EdgeInfo per child edge (child, label length and offset, the
+//     child's own edge range), so a child lookup costs the search over first tokens + ONE sector
+//     instead of four dependent reads (e_child -> n_tok_len, n_tok_off -> n_child_off);
+//   * the first tokens of the root's edges (the hottest node: every run head searches it) are
+//     staged in shared memory by every CTA (north_star: "staging of the hot top levels").
+// Labels are compared 32 lanes x CMP_UNROLL tokens per round trip with coalesced 32-bit loads: the
+// kernel is bound by dependent round trips, one register holds one token in flight whatever the
+// load width, and the two streams are misaligned against each other by an arbitrary number of
+// tokens, so 128-bit loads would cost a second load on one stream for the same tokens in flight.
+struct __align__(32) EdgeInfo {
+    i32 child, tok_len;
+    i64 tok_off;
+    i32 ce0, ce1;  // the child's edge range
+    i32 pad[2];
+};
+
+__global__ void __launch_bounds__(256) k_lpm_prep(RadixDev R, i32 E, EdgeInfo* __restrict__ info) {
+    const i32 e = blockIdx.x * 256 + threadIdx.x;
+    if (e >= E) return;
+    const i32 u = R.e_child[e];
+    EdgeInfo x;
+    x.child = u; x.tok_len = R.n_tok_len[u]; x.tok_off = R.n_tok_off[u];
+    x.ce0 = R.n_child_off[u]; x.ce1 = R.n_child_off[u + 1];
+    x.pad[0] = x.pad[1] = 0;
+    info[e] = x;
+}
+
+#ifndef PEEK_DW_THREADS
+#define PEEK_DW_THREADS 256
+#endif
+#ifndef PEEK_DW_CAP
+#define PEEK_DW_CAP 8
+#endif
+static constexpr int DW_THREADS = PEEK_DW_THREADS;   // k_lpm_dual: several CTAs per SM
+static constexpr int DW_WARPS = DW_THREADS / 32;
+static constexpr int DW_ROOT_STAGE = 2048;  // first tokens of the root's edges kept in shared memory
 
 // first position of minimal lcp in [w0, w0 + win) (clipped to N); w0 = 0 gives 0 (lcp[0] = 0)
 __device__ __forceinline__ i64 window_head(const i32* __restrict__ lcp, i64 w0, int win, i64 N, int lane) {
@@ -372,139 +430,192 @@ __device__ __forceinline__ i64 window_head(const i32* __restrict__ lcp, i64 w0, 
     return w0 + bidx;
 }
 
-struct PathEntry { i32 u, ds, L; i64 lab; };  // node entered at token depth ds; label length, offset
+struct PathEntry { i32 ds, L, ce0, ce1; i64 lab; };  // node entered at token depth ds; label length, offset; its edges
 
-__global__ void __launch_bounds__(DW_THREADS) k_lpm_radix_dual(const i32* __restrict__ tokens,
-                                                               const i64* __restrict__ tok_off, i64 N,
-                                                               RadixDev R, const i32* __restrict__ order,
-                                                               const i32* __restrict__ lcp, int win,
-                                                               i32* __restrict__ out) {
-    const unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    const i64 w = ((i64)blockIdx.x * DW_THREADS + threadIdx.x) >> 5;
-    const i64 w0 = w * win;
-    if (w0 >= N) return;
-    const i64 head = window_head(lcp, w0, win, N, lane);
-    const i64 end = window_head(lcp, w0 + win, win, N, lane);
-    PathEntry pe{0, 0, 0, 0};  // this lane's stack entry (entry index = lane)
-    int top = 0;               // entries in use (<= 32; deeper nodes are not recorded)
-    i32 Hprev = 0;
-    for (i64 jb = head; jb < end; jb += 32) {
-        const i64 jl = jb + lane;
-        const bool valid = jl < end;
-        const i32 r_l = valid ? __ldg(order + jl) : 0;
-        const i32 s_l = valid ? 16 * __ldg(lcp + jl) : 0;
-        const i64 o_l = valid ? __ldg(tok_off + r_l) : 0;
-        const i32 len_l = valid ? (i32)(__ldg(tok_off + r_l + 1) - o_l) : 0;
-        i32 H_l = 0;
-        const int cnt = (int)min((i64)32, end - jb);
-        for (int i = 0; i < cnt; ++i) {
-            i32 s = __shfl_sync(FULL, s_l, i);
-            const bool first = (jb == head && i == 0);
-            if (first) s = 0;
-            i32 H;
-            if (!first && Hprev < s) {
-                H = Hprev;
-            } else {
-                const i64 o = __shfl_sync(FULL, o_l, i);
-                const i32 len = __shfl_sync(FULL, len_l, i);
-                const i32* __restrict__ q = tokens + o;
-                // deepest recorded entry entered strictly above depth s
-                const unsigned mk = __ballot_sync(FULL, lane < top && pe.ds < s);
-                i32 v = 0, d = 0;
-                bool stop = false;
-                if (mk) {
-                    const int k = 31 - __clz(mk);
-                    top = k + 1;
-                    const i32 u = __shfl_sync(FULL, pe.u, k), ds = __shfl_sync(FULL, pe.ds, k),
-                              L = __shfl_sync(FULL, pe.L, k);
-                    const i64 lab = __shfl_sync(FULL, pe.lab, k);
-                    const i32 off = s - ds;
-                    if (off >= L) {  // node fully inside the shared prefix: continue below it
-                        v = u; d = ds + L;
-                    } else {
-                        const i32 limit = min(L, len - ds);
-                        const i32 m = off + (i32)match_len(R.c_tokens + lab + off, q + ds + off, limit - off, lane);
-                        d = ds + m;
-                        if (m < L) stop = true; else v = u;
-                    }
-                } else {
-                    top = 0;
-                }
-                while (!stop && d < len) {
-                    const i32 t = __ldg(q + d);
-                    const i32 e = find_child(R.e_first_tok, __ldg(R.n_child_off + v), __ldg(R.n_child_off + v + 1), t, lane);
-                    if (e < 0) break;
-                    const i32 u = __ldg(R.e_child + e);
-                    const i32 L = __ldg(R.n_tok_len + u);
-                    const i64 lab = __ldg(R.n_tok_off + u);
-                    if (top < 32) {
-                        if (lane == top) { pe.u = u; pe.ds = d; pe.L = L; pe.lab = lab; }
-                        ++top;
-                    }
-                    if (d + L <= s) { d += L; v = u; continue; }  // still inside the shared prefix: no compares
-                    const i32 skip = s > d ? s - d : 0;
-                    const i32 limit = min(L, len - d);
-                    const i32 m = skip + (i32)match_len(R.c_tokens + lab + skip, q + d + skip, limit - skip, lane);
-                    d += m;
-                    if (m < L) break;
-                    v = u;
-                }
-                H = d;
-            }
-            Hprev = H;
-            if (lane == i) H_l = H;
-        }
-        if (valid) out[r_l] = H_l;
+struct DualArgs {
+    const i32* tokens; const i64* tok_off;
+    const u64* hashes; const i64* blk_off;
+    i64 N;
+    RadixDev R; const EdgeInfo* info;                // radix mode (hit_radix != NULL)
+    const u64* t_keys; u64 mask;                     // hash mode (hit_hash != NULL)
+    const i32* order; const i32* lcp;
+    int win;
+    i32 *hit_radix, *hit_hash;
+    u32* ctr;             // work-item counter (zero on entry)
+    unsigned long long* counters;  // NULL or [4]: walks, child lookups, tokens compared, table probes
+};
+
+// edge index in [e0, e1) whose first token equals t, or -1; `ft` = the first-token array the range
+// indexes (global, or the staged copy of the root's)
+__device__ __forceinline__ i32 find_child_in(const i32* ft, i32 e0, i32 e1, i32 t, int lane, bool smem) {
+    while (e1 - e0 > 32) {
+        i32 n = e1 - e0;
+        i32 step = (n + 31) >> 5;
+        i32 pos = e0 + lane * step;
+        bool le = pos < e1 && (smem ? ft[pos] : __ldg(ft + pos)) <= t;
+        unsigned m = __ballot_sync(0xffffffffu, le);
+        if (m == 0) return -1;
+        int k = 31 - __clz(m);
+        e0 = e0 + k * step;
+        e1 = min(e0 + step, e1);
     }
+    i32 f = (e0 + lane < e1) ? (smem ? ft[e0 + lane] : __ldg(ft + e0 + lane)) : 0;
+    unsigned m = __ballot_sync(0xffffffffu, (e0 + lane < e1) && f == t);
+    return m ? e0 + (__ffs(m) - 1) : -1;
 }
 
-__global__ void __launch_bounds__(DWH_THREADS) k_lpm_hash_dual(const u64* __restrict__ hashes,
-                                                              const i64* __restrict__ blk_off, i64 N,
-                                                              const u64* __restrict__ t_keys, u64 mask,
-                                                              const i32* __restrict__ order,
-                                                              const i32* __restrict__ lcp, int win,
-                                                              i32* __restrict__ out) {
+#ifndef PEEK_DW_MINB
+#define PEEK_DW_MINB 4
+#endif
+// RADIX selects the mode at compile time: the two instantiations get their own register budgets
+// (the hash probe loop is lean and wants every warp slot of the SM; the radix walk is not)
+template <bool RADIX>
+__global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_dual(DualArgs A) {
+    __shared__ i32 root_ft[DW_ROOT_STAGE];
+    __shared__ PathEntry stack[DW_WARPS][32];
     const unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    const i64 w = ((i64)blockIdx.x * DWH_THREADS + threadIdx.x) >> 5;
-    const i64 w0 = w * win;
-    if (w0 >= N) return;
-    const i64 head = window_head(lcp, w0, win, N, lane);
-    const i64 end = window_head(lcp, w0 + win, win, N, lane);
-    i32 Hprev = 0;  // in blocks
-    for (i64 jb = head; jb < end; jb += 32) {
-        const i64 jl = jb + lane;
-        const bool valid = jl < end;
-        const i32 r_l = valid ? __ldg(order + jl) : 0;
-        const i32 s_l = valid ? __ldg(lcp + jl) : 0;
-        const i64 b_l = valid ? __ldg(blk_off + r_l) : 0;
-        const i32 nb_l = valid ? (i32)(__ldg(blk_off + r_l + 1) - b_l) : 0;
-        i32 H_l = 0;
-        const int cnt = (int)min((i64)32, end - jb);
-        for (int i = 0; i < cnt; ++i) {
-            i32 s = __shfl_sync(FULL, s_l, i);
-            const bool first = (jb == head && i == 0);
-            if (first) s = 0;
-            i32 H;
-            if (!first && Hprev < s) {
-                H = Hprev;
-            } else {
-                const i64 b0 = __shfl_sync(FULL, b_l, i);
-                const i32 nb = __shfl_sync(FULL, nb_l, i);
-                H = nb;
-                for (i32 i0 = s; i0 < nb; i0 += 32) {
-                    const i32 x = i0 + lane;
-                    bool miss = false;
-                    if (x < nb) miss = !table_has(t_keys, mask, __ldg(hashes + b0 + x));
-                    const unsigned m = __ballot_sync(FULL, miss);
-                    if (m) { H = i0 + (__ffs(m) - 1); break; }
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const i64 N = A.N;
+    const int win = A.win;
+    const i64 nwin = (N + win - 1) / win;
+    const i64 n_items = nwin;
+    const i32 root_e0 = RADIX ? __ldg(A.R.n_child_off) : 0, root_e1 = RADIX ? __ldg(A.R.n_child_off + 1) : 0;
+    const i32 root_staged = root_e0 == 0 ? min(root_e1, (i32)DW_ROOT_STAGE) : 0;  // node 0 = root: edges [0, root_e1)
+    for (int i = threadIdx.x; i < root_staged; i += DW_THREADS) root_ft[i] = __ldg(A.R.e_first_tok + i);
+    __syncthreads();
+    PathEntry* st = stack[wi];
+    u32 c_walks = 0, c_look = 0, c_tok = 0, c_probe = 0;
+    for (;;) {
+        u32 item = 0;
+        if (lane == 0) item = atomicAdd(A.ctr, 1u);
+        item = __shfl_sync(FULL, item, 0);
+        if ((i64)item >= n_items) break;
+        const i64 w0 = (i64)item * win;
+        const i64 head = window_head(A.lcp, w0, win, N, lane);
+        const i64 end = window_head(A.lcp, w0 + win, win, N, lane);
+        if (RADIX) {
+            int top = 0;  // stack entries in use (<= 32; deeper nodes are not recorded)
+            i32 Hprev = 0;
+            for (i64 jb = head; jb < end; jb += 32) {
+                const i64 jl = jb + lane;
+                const bool valid = jl < end;
+                const i32 r_l = valid ? __ldg(A.order + jl) : 0;
+                const i32 s_l = valid ? 16 * __ldg(A.lcp + jl) : 0;
+                const i64 o_l = valid ? __ldg(A.tok_off + r_l) : 0;
+                const i32 len_l = valid ? (i32)(__ldg(A.tok_off + r_l + 1) - o_l) : 0;
+                i32 H_l = 0;
+                const int cnt = (int)min((i64)32, end - jb);
+                for (int i = 0; i < cnt; ++i) {
+                    i32 s = __shfl_sync(FULL, s_l, i);
+                    const bool first = (jb == head && i == 0);
+                    if (first) s = 0;
+                    i32 H;
+                    if (!first && Hprev < s) {
+                        H = Hprev;
+                    } else {
+                        const i64 o = __shfl_sync(FULL, o_l, i);
+                        const i32 len = __shfl_sync(FULL, len_l, i);
+                        const i32* __restrict__ q = A.tokens + o;
+                        if (first) ++c_walks;
+                        // deepest recorded entry entered strictly above depth s
+                        const unsigned mk = __ballot_sync(FULL, lane < top && st[lane].ds < s);
+                        i32 d = 0, ce0 = root_e0, ce1 = root_e1;  // position in the cache: depth, edges of the node below
+                        bool at_root = true, stop = false;
+                        if (mk) {
+                            const int k = 31 - __clz(mk);
+                            top = k + 1;
+                            const PathEntry pe = st[k];
+                            const i32 off = s - pe.ds;
+                            if (off >= pe.L) {  // node fully inside the shared prefix: continue below it
+                                d = pe.ds + pe.L;
+                            } else {
+                                const i32 limit = min(pe.L, len - pe.ds);
+                                const i32 m = off + (i32)match_len_wide(A.R.c_tokens + pe.lab + off, q + pe.ds + off, limit - off, lane);
+                                c_tok += (u32)(m - off) + (m < limit ? 1u : 0u);
+                                d = pe.ds + m;
+                                if (m < pe.L) stop = true;
+                            }
+                            ce0 = pe.ce0; ce1 = pe.ce1; at_root = false;
+                        } else {
+                            top = 0;
+                        }
+                        while (!stop && d < len) {
+                            const i32 t = __ldg(q + d);
+                            ++c_look;
+                            const bool sm = at_root && ce1 <= root_staged;
+                            const i32 e = find_child_in(sm ? root_ft : A.R.e_first_tok, ce0, ce1, t, lane, sm);
+                            if (e < 0) break;
+                            const EdgeInfo ei = A.info[e];
+                            if (top < 32) {
+                                if (lane == 0) st[top] = PathEntry{d, ei.tok_len, ei.ce0, ei.ce1, ei.tok_off};
+                                ++top;
+                            }
+                            __syncwarp();
+                            ce0 = ei.ce0; ce1 = ei.ce1; at_root = false;
+                            const i32 L = ei.tok_len;
+                            if (d + L <= s) { d += L; continue; }  // still inside the shared prefix: no compares
+                            const i32 skip = s > d ? s - d : 0;
+                            const i32 limit = min(L, len - d);
+                            const i32 m = skip + (i32)match_len_wide(A.R.c_tokens + ei.tok_off + skip, q + d + skip, limit - skip, lane);
+                            c_tok += (u32)(m - skip) + (m < limit ? 1u : 0u);
+                            d += m;
+                            if (m < L) break;
+                        }
+                        H = d;
+                    }
+                    Hprev = H;
+                    if (lane == i) H_l = H;
                 }
+                if (valid) A.hit_radix[r_l] = H_l;
             }
-            Hprev = H;
-            if (lane == i) H_l = H;
+        } else {
+            i32 Hprev = 0;  // in blocks
+            for (i64 jb = head; jb < end; jb += 32) {
+                const i64 jl = jb + lane;
+                const bool valid = jl < end;
+                const i32 r_l = valid ? __ldg(A.order + jl) : 0;
+                const i32 s_l = valid ? __ldg(A.lcp + jl) : 0;
+                const i64 b_l = valid ? __ldg(A.blk_off + r_l) : 0;
+                const i32 nb_l = valid ? (i32)(__ldg(A.blk_off + r_l + 1) - b_l) : 0;
+                i32 H_l = 0;
+                const int cnt = (int)min((i64)32, end - jb);
+                for (int i = 0; i < cnt; ++i) {
+                    i32 s = __shfl_sync(FULL, s_l, i);
+                    const bool first = (jb == head && i == 0);
+                    if (first) s = 0;
+                    i32 H;
+                    if (!first && Hprev < s) {
+                        H = Hprev;
+                    } else {
+                        const i64 b0 = __shfl_sync(FULL, b_l, i);
+                        const i32 nb = __shfl_sync(FULL, nb_l, i);
+                        if (first) ++c_walks;
+                        H = nb;
+                        // a resumed walk mostly misses at once (the branch below the shared prefix
+                        // is not cached): its first batch is 8 probes, later ones 32
+                        int batch = 32;
+                        for (i32 i0 = s; i0 < nb; i0 += batch, batch = 32) {
+                            const i32 x = i0 + lane;
+                            bool miss = false;
+                            const bool act = lane < batch && x < nb;
+                            if (act) miss = !table_has(A.t_keys, A.mask, __ldg(A.hashes + b0 + x));
+                            c_probe += (u32)__popc(__ballot_sync(FULL, act));
+                            const unsigned m = __ballot_sync(FULL, miss);
+                            if (m) { H = i0 + (__ffs(m) - 1); break; }
+                        }
+                    }
+                    Hprev = H;
+                    if (lane == i) H_l = H;
+                }
+                if (valid) A.hit_hash[r_l] = H_l * 16;
+            }
         }
-        if (valid) out[r_l] = H_l * 16;
+    }
+    if (A.counters && lane == 0) {
+        if (c_walks) atomicAdd(A.counters + 0, (unsigned long long)c_walks);
+        if (c_look) atomicAdd(A.counters + 1, (unsigned long long)c_look);
+        if (c_tok) atomicAdd(A.counters + 2, (unsigned long long)c_tok);
+        if (c_probe) atomicAdd(A.counters + 3, (unsigned long long)c_probe);
     }
 }
 
@@ -534,14 +645,17 @@ __global__ void __launch_bounds__(LPM_THREADS) k_radix_demand(const i32* __restr
 }
 __global__ void k_radix_demand_root(i32* node_demand, i32 n) { node_demand[0] = n; }
 
-i64 lpm_ws_bytes(i64 N) {  // speculative path: W per mode and the scan partials
+i64 lpm_ws_bytes(i64 N, i64 V) {  // speculative path: W per mode and the scan partials; dual walk: edge table + counter
     Arena a(nullptr);
     a.take<i32>(N);
     a.take<i32>(N);
     a.take<Fn>((N + RS_CHUNK - 1) / RS_CHUNK + 1);
+    a.take<EdgeInfo>(V);
+    a.take<u32>(64);
     return a.used;
 }
 
+static unsigned long long* g_lpm_counters = nullptr;  // peek_lpm_counters
 static int g_lpm_strategy = 0;  // PEEK_OPT_LPM_STRATEGY
 static int g_lpm_window = 0;    // PEEK_OPT_LPM_WINDOW
 void lpm_set_option(int key, i64 v) {
@@ -582,7 +696,8 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
         return PEEK_ERR_INVALID_ARG;
     }
     if (N == 0 || (!hit_radix && !hit_hash)) return PEEK_OK;
-    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < lpm_ws_bytes(N)) {
+    const i64 VE = hit_radix ? (radix->V > radix->E ? radix->V : radix->E) : 0;
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < lpm_ws_bytes(N, VE)) {
         set_error("peek_lpm: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;
     }
@@ -599,13 +714,13 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
     int win = 1;
     while (win < 32 && N / win > 8192) win *= 2;
     if (g_lpm_window > 0) win = g_lpm_window;
-    const unsigned dual_grid = (unsigned)((((N + win - 1) / win) * 32 + DW_THREADS - 1) / DW_THREADS);
-    const unsigned dualh_grid = (unsigned)((((N + win - 1) / win) * 32 + DWH_THREADS - 1) / DWH_THREADS);
     Arena a(ws);
     i32* Wr = a.take<i32>(N);
     i32* Wh = a.take<i32>(N);
     const i64 nchunks = (N + RS_CHUNK - 1) / RS_CHUNK;
     Fn* partial = a.take<Fn>(nchunks + 1);
+    EdgeInfo* info = a.take<EdgeInfo>(VE);
+    u32* ctr = a.take<u32>(64);
     auto resolve = [&](const i32* W, i32* hit) {
         if (N <= 65536) {
             Prof pr(PROF_LPM_RESOLVE, st, 1);
@@ -617,30 +732,59 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
             k_resolve_apply<<<(unsigned)nchunks, RS_THREADS, 0, st>>>(order, lcp, W, N, partial, hit);
         }
     };
-    if (hit_radix) {
-        RadixDev R{radix->c_tokens, radix->n_tok_off, radix->n_tok_len,
-                   radix->n_child_off, radix->e_first_tok, radix->e_child};
-        {
-            Prof pr(PROF_LPM_RADIX, st, 1);
-            if (dual) k_lpm_radix_dual<<<dual_grid, DW_THREADS, 0, st>>>(tokens, tok_off, N, R, order, lcp, win, hit_radix);
-            else if (spec) k_lpm_radix_spec<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, order, lcp, Wr);
-            else k_lpm_radix<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, hit_radix);
+    RadixDev R{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    if (hit_radix) R = RadixDev{radix->c_tokens, radix->n_tok_off, radix->n_tok_len,
+                                radix->n_child_off, radix->e_first_tok, radix->e_child};
+    if (dual) {  // persistent kernels, one per mode (plus the edge table of the radix cache)
+        PEEK_CUDA(cudaMemsetAsync(ctr, 0, 256, st));
+        DualArgs D;
+        D.tokens = tokens; D.tok_off = tok_off; D.hashes = hashes; D.blk_off = blk_off; D.N = N;
+        D.R = R; D.info = info;
+        D.t_keys = hit_hash ? table->t_keys : nullptr; D.mask = hit_hash ? (u64)(table->S - 1) : 0;
+        D.order = order; D.lcp = lcp; D.win = win; D.hit_radix = hit_radix; D.hit_hash = hit_hash;
+        D.counters = g_lpm_counters;
+        const i64 items = (N + win - 1) / win;
+        i64 ctas = (items + DW_WARPS - 1) / DW_WARPS;
+        const i64 cap = (i64)sm_count() * PEEK_DW_CAP;  // resident CTAs per SM - the warps loop over the items
+        if (ctas > cap) ctas = cap;
+        if (hit_radix) {
+            Prof pr(PROF_LPM_RADIX, st, radix->E > 0 ? 2 : 1);
+            if (radix->E > 0) k_lpm_prep<<<(unsigned)((radix->E + 255) / 256), 256, 0, st>>>(R, radix->E, info);
+            D.ctr = ctr;
+            k_lpm_dual<true><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
         }
-        if (spec) resolve(Wr, hit_radix);
-    }
-    if (hit_hash) {
-        {
+        if (hit_hash) {
             Prof pr(PROF_LPM_HASH, st, 1);
-            if (dual) k_lpm_hash_dual<<<dualh_grid, DWH_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), order, lcp, win, hit_hash);
-            else if (spec) k_lpm_hash_spec<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), order, lcp, Wh);
-            else k_lpm_hash<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), hit_hash);
+            D.ctr = ctr + 32;
+            k_lpm_dual<false><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
         }
-        if (spec) resolve(Wh, hit_hash);
+    } else {
+        if (hit_radix) {
+            {
+                Prof pr(PROF_LPM_RADIX, st, 1);
+                if (spec) k_lpm_radix_spec<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, order, lcp, Wr);
+                else k_lpm_radix<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, N, R, hit_radix, g_lpm_counters);
+            }
+            if (spec) resolve(Wr, hit_radix);
+        }
+        if (hit_hash) {
+            {
+                Prof pr(PROF_LPM_HASH, st, 1);
+                if (spec) k_lpm_hash_spec<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), order, lcp, Wh);
+                else k_lpm_hash<<<warps_grid, LPM_THREADS, 0, st>>>(hashes, blk_off, N, table->t_keys, (u64)(table->S - 1), hit_hash, g_lpm_counters);
+            }
+            if (spec) resolve(Wh, hit_hash);
+        }
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;
 }
 
+
+extern "C" peek_status peek_lpm_counters(uint64_t* counters) {
+    g_lpm_counters = (unsigned long long*)counters;
+    return PEEK_OK;
+}
 
 extern "C" peek_status peek_radix_demand(const int32_t* tokens, const int64_t* tok_off, int64_t N,
                                          const peek_radix* radix, const int32_t* hit_radix,

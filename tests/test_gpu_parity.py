@@ -306,6 +306,54 @@ def test_pending_tree_local_stage(local_cap, grid_limit):
         b.set_option(b.OPT_GRID_LIMIT, 0)
 
 
+def test_lpm_work_counters():
+    """The amortisation claim (Fig. 6(a); SURVEY.md section 4 "work-counter tests"):
+    five requests under a shared system prefix, clusters A x3 and B x2, the cache holds sys and
+    sys+A.  Stock LPM (no tree view) walks from the root once per request and compares every
+    request's whole cached prefix; the dual walk starts ONE walk at the root, compares every cached
+    token once, and reaches the other requests by child lookups below the shared prefixes."""
+    b = _b()
+    rng = np.random.default_rng(66)
+    tok = lambda n: rng.integers(0, 128256, size=n).astype(np.int32)
+    sys_p, a_p, b_p = tok(160), tok(96), tok(64)
+    reqs = [np.concatenate([sys_p, a_p, tok(40)]) for _ in range(3)] + [np.concatenate([sys_p, b_p, tok(40)]) for _ in range(2)]
+    toks, off = _csr(reqs)
+    radix, t_keys = _cache_from([sys_p, np.concatenate([sys_p, a_p])], 256)
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    o_hr = oracle.lpm_radix(toks, off, _orc_radix(radix))
+    d_tok, d_off, d_h, d_bo = _dev(toks), _dev(off), _dev(o_h.view(np.int64), torch.uint64), _dev(o_bo)
+    d_radix, d_keys = _radix_dev(radix), _dev(t_keys.view(np.int64), torch.uint64)
+    tree = b.peek_pending_tree(d_h, d_bo)
+    cnt = torch.zeros(4, dtype=torch.uint64, device=DEV)
+    read = lambda: cnt.cpu().view(torch.int64).tolist()
+    b.lpm_counters(cnt)
+    try:
+        b.set_option(b.OPT_LPM_STRATEGY, b.LPM_DUAL_WALK)
+        b.set_option(b.OPT_LPM_WINDOW, 8)
+        hr, hh = b.peek_lpm(d_tok, d_off, d_h, d_bo, radix=d_radix, t_keys=d_keys, tree=tree)
+        torch.cuda.synchronize()
+        dual = read()
+        cnt.zero_()
+        b.set_option(b.OPT_LPM_STRATEGY, b.LPM_AUTO)
+        hr0, hh0 = b.peek_lpm(d_tok, d_off, d_h, d_bo, radix=d_radix, t_keys=d_keys, tree=None)
+        torch.cuda.synchronize()
+        naive = read()
+    finally:
+        b.lpm_counters(None)
+        b.set_option(b.OPT_LPM_STRATEGY, b.LPM_AUTO)
+        b.set_option(b.OPT_LPM_WINDOW, 0)
+    assert np.array_equal(_np(hr), o_hr) and np.array_equal(_np(hr0), o_hr)
+    assert o_hr.tolist() == [256, 256, 256, 160, 160]
+    # stock LPM: 5 walks from the root in each mode, every request's cached prefix compared in full
+    assert naive[0] == 10
+    assert naive[2] == int(o_hr.sum())               # every walk ends at a node boundary: matched tokens only
+    assert naive[3] == int(np.diff(o_bo).sum())      # a warp probes 32 blocks of a request at once: all of them here
+    # dual walk: one walk from the root per mode; sys and A compared once, B's first token once
+    assert dual[0] == 2
+    assert dual[2] == 160 + 96
+    assert dual[2] * 3 < naive[2] and dual[3] * 2 < naive[3]
+
+
 def test_rank_two_phase_wide_keys():
     """cLPM keys too wide for one 64-bit packed key (full-range hit, cluster size and arrival):
     the arrival sort followed by the stable (hit, cluster size) sort."""
