@@ -256,15 +256,13 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
     u32 parity = 0;           // bit s = parity to wait for on stage s
     int sI = 0, sC = 0;
 
-    auto issue = [&]() {  // next chunk of `im` -> stage sI
+    auto issue = [&]() {  // next chunk of `im` -> stage sI: the owning lane issues its own copy
         const int q = __ffs(im) - 1;
         im &= im - 1;
-        const uintptr_t src = (uintptr_t)__shfl_sync(FULL, (unsigned long long)(uintptr_t)c_src, q);
-        const u32 bytes = __shfl_sync(FULL, c_bytes, q);
-        if (lane == 0) {
+        if (lane == q) {
             const u32 bar = bar0 + 8 * sI;
-            mbar_expect_tx(bar, bytes);
-            if (bytes) tma_load_1d(stage0 + sI * HF_STAGE_BYTES, (const void*)src, bytes, bar);
+            mbar_expect_tx(bar, c_bytes);
+            if (c_bytes) tma_load_1d(stage0 + sI * HF_STAGE_BYTES, (const void*)c_src, c_bytes, bar);
         }
         sI = sI + 1 == HF_STAGES ? 0 : sI + 1;
     };
