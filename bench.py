@@ -24,7 +24,7 @@ import torch
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2607_02525_b200 import workloads as W  # noqa: E402
+from harness import workloads as W  # noqa: E402
 
 METRIC = "lpm_queries_per_s"
 UNIT = "queries/s"
@@ -232,7 +232,7 @@ def gather_ceiling(inp, dev):
     """Random 32-byte-sector gather ceilings: the honest roofline of the probe /
     child-lookup kernels.  Over a buffer far larger than L2 (the token array, capped at 4 GiB) and
     over the table itself (8 S bytes: partly L2 resident)."""
-    from paper_2607_02525_b200 import binding as B
+    from harness import gather_probe as GP
     out = {}
     tok_bytes = inp.tok.numel() * 4
     big = inp.tok[: min(inp.tok.numel(), 1 << 30)] if tok_bytes >= (1 << 28) else None
@@ -242,13 +242,13 @@ def gather_ceiling(inp, dev):
         if buf.data_ptr() % 32:
             continue
         reads = 1 << 26
-        B.bench_random_gather(buf, reads, 1)
+        GP.random_gather(buf, reads, 1)
         torch.cuda.synchronize()
         best = None
         for it in range(3):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            B.bench_random_gather(buf, reads, 2 + it)
+            GP.random_gather(buf, reads, 2 + it)
             e1.record()
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1)

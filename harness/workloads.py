@@ -4,7 +4,7 @@ This module serves BOTH the CUDA path and the CPU oracle and therefore holds non
 of the method's arithmetic: no hash function, no prefix walk, no probe, no sort of
 chains.  It draws random numbers (numpy ``default_rng([seed, config])``; seeds 42,
 142, 242 as in PAPER.md:362), lays requests out as CSR int32 token arrays, and asks
-``csrc/engine_sim.cpp`` (a stand-in for the engine's prefix cache) to
+``harness/engine_sim.cpp`` (a stand-in for the engine's prefix cache) to
 build the read-only cache inputs.  Chained hashes needed for the table keys are
 produced by a ``hash_fn`` the caller passes in (the oracle's in oracle tests, the
 CUDA call in GPU tests and bench.py).
@@ -25,7 +25,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_ESIM_SRC = os.path.join(_HERE, "csrc", "engine_sim.cpp")
+_ESIM_SRC = os.path.join(_HERE, "engine_sim.cpp")
 _ESIM_LIB = os.path.join(_HERE, "libpeek_engine_sim.so")
 _esim = None
 

@@ -331,16 +331,6 @@ const char* peek_profile_name(int32_t slot);
 peek_status peek_profile_read(int32_t slot, double* total_ms, int64_t* groups, int32_t reset);
 int64_t peek_launch_count(void);
 
-/* ---- measurement utility: random 32-byte-sector gather ceiling ------- */
-/* The honest ceiling for the probe / child-lookup / bisection kernels, whose reads are random
- * 32-byte sectors: `reads` independent 16-byte loads at addresses drawn by a counter-based
- * generator (mix64 of seed + read index), uniform over the 32-byte sectors of buf[0 .. bytes)
- * [device, read-only, bytes >= 32]; the xor of everything read goes to sink[0] [device] so the
- * loads cannot be elided.  Enqueues one kernel on `stream`; time it with events.  Not part of the
- * hot path.  Errors: NULL buf or sink, bytes < 32, reads < 0 -> PEEK_ERR_INVALID_ARG. */
-peek_status peek_bench_random_gather(const void* buf, int64_t bytes, int64_t reads, uint64_t seed,
-                                     uint64_t* sink, void* stream);
-
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ CALL_CLPM_SIGNALS, CALL_CLPM_ORDER_FULL, CALL_CLPM_GROUP_MAJOR, CALL_OFFLINE_PHA
 CALL_PENDING_TREE_UPDATE = 8
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
-           "peek_launch_count", "peek_set_option", "peek_bench_random_gather", "peek_lpm_counters",
+           "peek_launch_count", "peek_set_option", "peek_lpm_counters",
            "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
            "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1", "peek_radix_demand",
            "peek_clpm_lane_b", "peek_dynamic_lane", "peek_pending_tree_update",
@@ -96,8 +96,6 @@ def lib():
         L.peek_radix_demand.argtypes = [vp, vp, i64, ctypes.POINTER(_Radix), vp, vp, vp]
         L.peek_offline_phase1.restype = i32
         L.peek_offline_phase1.argtypes = [vp, vp, i64, i32, vp, vp, vp, i64, vp]
-        L.peek_bench_random_gather.restype = i32
-        L.peek_bench_random_gather.argtypes = [vp, i64, i64, u64, vp, vp]
         _lib = L
     return _lib
 
@@ -463,13 +461,3 @@ def launch_count() -> int:
     L = lib()
     L.peek_launch_count.restype = ctypes.c_int64
     return int(L.peek_launch_count())
-
-
-def bench_random_gather(buf: torch.Tensor, reads: int, seed: int = 1) -> torch.Tensor:
-    """Measurement utility (include/peek.h): `reads` random 32-byte-sector loads over `buf`;
-    returns the device sink word.  Time it with CUDA events."""
-    sink = torch.zeros(1, dtype=torch.int64, device=buf.device)
-    st = lib().peek_bench_random_gather(_ptr(buf), buf.numel() * buf.element_size(), int(reads), int(seed),
-                                        _ptr(sink), _stream())
-    _check(st, "peek_bench_random_gather")
-    return sink

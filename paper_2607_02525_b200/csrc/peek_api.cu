@@ -185,48 +185,3 @@ extern "C" peek_status peek_profile_read(int32_t slot, double* total_ms, int64_t
     return PEEK_OK;
 }
 extern "C" int64_t peek_launch_count(void) { return peek::g_launches; }
-
-
-// ---- random-sector gather ceiling (measurement utility) ---------------------------------------
-namespace peek {
-static constexpr int RG_THREADS = 256, RG_PER_THREAD = 8;
-__global__ void __launch_bounds__(RG_THREADS) k_random_gather(const uint4* __restrict__ buf, u64 sectors,
-                                                             i64 reads, u64 seed, u64* __restrict__ sink) {
-    const i64 t = (i64)blockIdx.x * RG_THREADS + threadIdx.x, nthreads = (i64)gridDim.x * RG_THREADS;
-    u64 acc = 0;
-    for (i64 i0 = t; i0 < reads; i0 += nthreads * RG_PER_THREAD) {
-        uint4 v[RG_PER_THREAD];
-#pragma unroll
-        for (int u = 0; u < RG_PER_THREAD; ++u) {  // RG_PER_THREAD independent loads in flight
-            const i64 i = i0 + u * nthreads;
-            const u64 sct = mix64(seed + (u64)i * 0x9E3779B97F4A7C15ull) % sectors;
-            v[u] = i < reads ? __ldg(buf + 2 * sct) : make_uint4(0, 0, 0, 0);
-        }
-#pragma unroll
-        for (int u = 0; u < RG_PER_THREAD; ++u) acc ^= ((u64)v[u].x << 32 | v[u].y) ^ ((u64)v[u].z << 32 | v[u].w);
-    }
-    acc ^= __shfl_xor_sync(0xffffffffu, acc, 16);
-    acc ^= __shfl_xor_sync(0xffffffffu, acc, 8);
-    acc ^= __shfl_xor_sync(0xffffffffu, acc, 4);
-    acc ^= __shfl_xor_sync(0xffffffffu, acc, 2);
-    acc ^= __shfl_xor_sync(0xffffffffu, acc, 1);
-    if ((threadIdx.x & 31) == 0 && acc) atomicXor((unsigned long long*)sink, (unsigned long long)acc);
-}
-}  // namespace peek
-
-extern "C" peek_status peek_bench_random_gather(const void* buf, int64_t bytes, int64_t reads, uint64_t seed,
-                                                uint64_t* sink, void* stream) {
-    if (!buf || !sink || bytes < 32 || reads < 0 || ((uintptr_t)buf & 31)) {
-        peek::set_error("peek_bench_random_gather: bad argument (buf 32-byte aligned, bytes >= 32)");
-        return PEEK_ERR_INVALID_ARG;
-    }
-    if (reads == 0) return PEEK_OK;
-    i64 want = (reads + peek::RG_THREADS * peek::RG_PER_THREAD - 1) / (peek::RG_THREADS * peek::RG_PER_THREAD);
-    i64 cap = (i64)peek::sm_count() * 64;
-    unsigned grid = (unsigned)(want < cap ? want : cap);
-    peek::k_random_gather<<<grid, peek::RG_THREADS, 0, (cudaStream_t)stream>>>(
-        (const uint4*)buf, (u64)(bytes / 32), reads, seed, sink);
-    peek::g_launches += 1;
-    PEEK_CUDA(cudaGetLastError());
-    return PEEK_OK;
-}

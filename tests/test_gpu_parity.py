@@ -6,7 +6,7 @@ import pytest
 import torch
 
 import oracle
-from paper_2607_02525_b200 import workloads as W
+from harness import workloads as W
 
 pytestmark = pytest.mark.gpu
 

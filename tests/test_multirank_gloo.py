@@ -21,7 +21,7 @@ def _worker(rank, world, port, out):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     import bench
-    from paper_2607_02525_b200 import workloads as W
+    from harness import workloads as W
     wl = W.make(1, seed=bench.rank_seed(42, rank))
     toks, off = wl.queue.materialize_np()
     ms = bench.max_over_ranks(10.0 * (rank + 1), torch.device("cpu"), world)

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_2607_02525_b200 import workloads as W
+from harness import workloads as W
 
 B = 16
 

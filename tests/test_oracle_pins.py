@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_2607_02525_b200 import workloads as W
+from harness import workloads as W
 from tests import bruteforce as bf
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden", "hash_vectors.txt")
