@@ -150,8 +150,9 @@ def workspace_bytes(call_id: int, N=0, T=0, NB=0, S=0, V=0) -> int:
 
 
 def _ws(call_id, device, **sizes):
+    """Scratch for one call, cached per (device, stream, call): two streams never share a buffer."""
     need = workspace_bytes(call_id, **sizes)
-    key = (str(device), call_id)
+    key = (str(device), int(torch.cuda.current_stream(device).cuda_stream), call_id)
     buf = _ws_cache.get(key)
     if buf is None or buf.numel() < need:
         buf = torch.empty(need, dtype=torch.uint8, device=device)

@@ -465,12 +465,14 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
         return PEEK_ERR_INVALID_ARG;
     }
     cudaStream_t st = (cudaStream_t)stream;
-    if (demand) PEEK_CUDA(cudaMemsetAsync(demand, 0, sizeof(i32) * (size_t)table->S, st));
-    if (N == 0 || (!demand && !clpm_order)) return PEEK_OK;
-    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < demand_rank_ws_bytes(N, table ? table->S : 0)) {
+    if (N > 0 && (demand || clpm_order) &&
+        (!ws || ((uintptr_t)ws & 255) || ws_bytes < demand_rank_ws_bytes(N, table ? table->S : 0))) {
         set_error("peek_demand_rank: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;
     }
+    // every argument is checked: from here on work is enqueued
+    if (demand) PEEK_CUDA(cudaMemsetAsync(demand, 0, sizeof(i32) * (size_t)table->S, st));
+    if (N == 0 || (!demand && !clpm_order)) return PEEK_OK;
     Arena a(ws);
     RankArgs A;
     rank_layout(a, N, RANK_MAX_GRID, A);

@@ -98,7 +98,13 @@ __global__ void __launch_bounds__(SI_T, 1) k_stride_interleave(const i32* __rest
     int margin = SI_MARGIN;
     while (k0 < N) {
         const int cnt = (int)(N - k0 < SI_T ? N - k0 : SI_T);
-        ++stamp;
+        // the stamp has 22 bits in a table entry: when it wraps, every entry is cleared (0 = never used)
+        if (++stamp >> 22) {
+            __syncthreads();
+            for (int x = tid; x < SI_H; x += SI_T) S.H[x] = 0;
+            __syncthreads();
+            stamp = 1;
+        }
         // ---- 1: slot types ----
         const i64 s = k0 + tid;
         const bool live = tid < cnt;

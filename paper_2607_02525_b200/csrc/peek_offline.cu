@@ -187,7 +187,7 @@ extern "C" peek_status peek_offline_phase1(const uint64_t* hashes, const int64_t
         return PEEK_ERR_INVALID_ARG;
     }
     if (N == 0) return PEEK_OK;
-    if (!blk_off || !order || !guards) { set_error("peek_offline_phase1: NULL argument"); return PEEK_ERR_INVALID_ARG; }
+    if (!hashes || !blk_off || !order || !guards) { set_error("peek_offline_phase1: NULL argument"); return PEEK_ERR_INVALID_ARG; }
     if (!ws || ((uintptr_t)ws & 255) || ws_bytes < offline_phase1_ws_bytes(N)) {
         set_error("peek_offline_phase1: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;

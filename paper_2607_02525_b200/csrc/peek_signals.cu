@@ -364,16 +364,18 @@ extern "C" peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* 
     }
     if (section && N > 0 && !hit) { set_error("peek_clpm_signals: section needs hit"); return PEEK_ERR_INVALID_ARG; }
     cudaStream_t st = (cudaStream_t)stream;
-    if (evict_score) PEEK_CUDA(cudaMemsetAsync(evict_score, 0, sizeof(i64) * (size_t)table->S, st));
-    if (N == 0 || (!section && !score && !evict_score)) return PEEK_OK;
-    if (!blk_off || !order || !lcp || (evict_score && !hashes)) {
+    const bool work = N > 0 && (section || score || evict_score);
+    if (work && (!blk_off || !order || !lcp || (evict_score && !hashes))) {
         set_error("peek_clpm_signals: NULL argument");
         return PEEK_ERR_INVALID_ARG;
     }
-    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < clpm_signals_ws_bytes(N)) {
+    if (work && (!ws || ((uintptr_t)ws & 255) || ws_bytes < clpm_signals_ws_bytes(N))) {
         set_error("peek_clpm_signals: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;
     }
+    // every argument is checked: from here on work is enqueued
+    if (evict_score) PEEK_CUDA(cudaMemsetAsync(evict_score, 0, sizeof(i64) * (size_t)table->S, st));
+    if (!work) return PEEK_OK;
     Arena a(ws);
     SignalsWs W;
     signals_layout(a, N, W);

@@ -175,6 +175,7 @@ __device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb, int wmax) {
         if (kl.sbits + lbits + w <= 64) break;
     }
     kl.total = kl.sbits + kl.lbits + kl.w;
+    if (kl.total > 64) __trap();  // no layout fits (a chain of >= 2^24 blocks): fail loudly, never sort truncated keys
     return kl;
 }
 // The narrowest layout (w = 1: D = 64, LDmax = 64 maxnb + 64, lbits <= bits(192 maxnb + 196)) needs
@@ -1752,7 +1753,7 @@ extern "C" peek_status peek_pending_tree_update(const uint64_t* hashes, const in
         return PEEK_ERR_INVALID_ARG;
     }
     if (N_new == 0) return PEEK_OK;
-    if (!blk_off || !order || !lcp || (N_old > 0 && (!old_order || !old_lcp || !remap))) {
+    if (!hashes || !blk_off || !order || !lcp || (N_old > 0 && (!old_order || !old_lcp || !remap))) {
         set_error("peek_pending_tree_update: NULL argument");
         return PEEK_ERR_INVALID_ARG;
     }

@@ -234,6 +234,39 @@ def test_arg_errors():
         b.peek_lpm(None, off, None, off, radix=None, t_keys=torch.zeros(6, dtype=torch.uint64, device=DEV))
 
 
+def test_errors_leave_outputs_untouched():
+    """include/peek.h: argument and workspace errors are detected before anything is enqueued."""
+    b = _b()
+    L = b.lib()
+    rng = np.random.default_rng(4)
+    reqs = [rng.integers(0, 50, size=64).astype(np.int32) for _ in range(40)]
+    toks, off = _csr(reqs)
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    d_h, d_bo = _dev(o_h.view(np.int64), torch.uint64), _dev(o_bo)
+    tree = b.peek_pending_tree(d_h, d_bo)
+    keys = torch.full((64,), -1, dtype=torch.int64, device=DEV).view(torch.uint64)
+    demand = torch.full((64,), 7, dtype=torch.int32, device=DEV)
+    evict = torch.full((64,), 7, dtype=torch.int64, device=DEV)
+    tbl = b._Table(b._ptr(keys), 64)
+    import ctypes
+    small = torch.zeros(256, dtype=torch.uint8, device=DEV)
+    p = b._ptr
+    st = L.peek_demand_rank(p(d_h), p(d_bo), 40, p(tree.order), p(tree.lcp), ctypes.byref(tbl), None, None, None,
+                            p(demand), None, p(small), 256, None)
+    assert st == -3  # PEEK_ERR_WORKSPACE
+    st2 = L.peek_clpm_signals(p(d_h), p(d_bo), 40, p(tree.order), p(tree.lcp), None, 0, None, ctypes.byref(tbl),
+                              None, None, p(evict), p(small), 256, None)
+    assert st2 == -3
+    st3 = L.peek_clpm_signals(None, p(d_bo), 40, p(tree.order), p(tree.lcp), None, 0, None, ctypes.byref(tbl),
+                              None, None, p(evict), p(small), 256, None)
+    assert st3 == -1  # PEEK_ERR_INVALID_ARG: evict_score needs hashes
+    torch.cuda.synchronize()
+    assert bool((demand == 7).all()) and bool((evict == 7).all())
+    assert L.peek_pending_tree(None, p(d_bo), 40, p(tree.order), p(tree.lcp), None, None, None, None, None, None,
+                               p(small), 256, None) == -1
+    assert L.peek_offline_phase1(None, p(d_bo), 40, 8, p(tree.order), p(evict), p(small), 256, None) == -1
+
+
 def _nested_queue(rng, n, vocab=4):
     """Short requests over a tiny vocabulary: deep nesting, duplicates, prefix-of relations."""
     stems = [rng.integers(0, vocab, size=int(rng.integers(16, 400))).astype(np.int32) for _ in range(40)]
