@@ -46,3 +46,23 @@ def test_world2_independent_batches_and_max_timing():
         assert n == 256
         assert digests[0] != digests[1]        # independent batches
         assert thr == world * 256 * 4 / 20e-3  # whole-job aggregate
+
+
+def test_bench_gpus_flag_spawns_ranks():
+    """`bench.py --gpus 2` outside torchrun re-launches itself with two ranks (the same path the CUDA
+    arm takes); the reference arm runs here on CPU: rank 0 prints the one JSON line, rank 1 exits 0."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference",
+                        "--small", "--config", "1", "--steps", "1", "--warmup", "0", "--cpu-seconds", "0.5"],
+                       capture_output=True, text=True, timeout=600, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    rec = json.loads(lines[0])
+    assert rec["impl"] == "reference" and rec["ranks"] == 2 and rec["value"] > 0
+    assert "torch.distributed.run" in r.stderr and "--nproc-per-node 2" in r.stderr
+    assert rec["config"]["workload"].startswith("configs[0]")
