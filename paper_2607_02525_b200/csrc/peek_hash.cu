@@ -54,6 +54,24 @@ __global__ void __launch_bounds__(1024) k_scan_partials(i64* __restrict__ partia
     }
 }
 
+// small queues: the whole scan in one CTA, one launch (N <= SCAN_SMALL_MAX)
+static constexpr int SCAN_SMALL_MAX = 8192;
+__global__ void __launch_bounds__(1024) k_nb_scan_small(const i64* __restrict__ tok_off, i64 N,
+                                                        i64* __restrict__ blk_off,
+                                                        unsigned long long* __restrict__ counter) {
+    __shared__ i64 sm[34];
+    if (threadIdx.x == 0) { *counter = 0; blk_off[0] = 0; }
+    i64 carry = 0;
+    for (i64 b = 0; b < N; b += 1024) {
+        const i64 r = b + threadIdx.x;
+        const i64 v = r < N ? (tok_off[r + 1] - tok_off[r]) / B16 : 0;
+        i64 tot;
+        const i64 ex = block_exscan_i64(v, sm, &tot);
+        if (r < N) blk_off[r + 1] = carry + ex + v;
+        carry += tot;
+    }
+}
+
 __global__ void __launch_bounds__(SCAN_THREADS) k_nb_apply(const i64* __restrict__ tok_off, i64 N,
                                                           const i64* __restrict__ partial,
                                                           i64* __restrict__ blk_off) {
@@ -425,7 +443,10 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
     i64 nchunks = (N + SCAN_CHUNK - 1) / SCAN_CHUNK;
     i64* partial = a.take<i64>(nchunks + 1);
     unsigned long long* counter = a.take<unsigned long long>(1);
-    {
+    if (N <= SCAN_SMALL_MAX) {
+        Prof pr(PROF_HASH_SCAN, st, 1);
+        k_nb_scan_small<<<1, 1024, 0, st>>>(tok_off, N, blk_off, counter);
+    } else {
         Prof pr(PROF_HASH_SCAN, st, 3);
         k_nb_partial<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial);
         k_scan_partials<<<1, 1024, 0, st>>>(partial, nchunks, counter);

@@ -448,6 +448,32 @@ __device__ __forceinline__ void local_sort(LocalBufs& lb, int n, u64 vary, GsSme
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int Kp = (n + GS_THREADS - 1) / GS_THREADS;
     const int wbase = w * 32 * Kp;
+    if (n <= GS_THREADS) {
+        // Small items (one position per thread; the paper's queues hold 60-200 requests,
+        // PAPER.md:364): no passes at all - every position counts the positions that sort before it
+        // (smaller key, or equal key and earlier) against the keys staged by position, and its
+        // element goes straight to that rank.
+        if (!vary) return;
+        static_assert(sizeof(sm.wcnt) >= GS_THREADS * sizeof(u64), "staging area of the counting sort");
+        u64* kp = (u64*)&sm.wcnt[0][0];
+        const int t = threadIdx.x;
+        unsigned short e = 0;
+        u64 key = ~0ull;
+        if (t < n) { e = lb.idx[t]; key = lb.key[e]; kp[t] = key; }
+        __syncthreads();
+        if (t < n) {
+            u32 rank = 0;
+#pragma unroll 8
+            for (int j = 0; j < n; ++j) {
+                const u64 kj = kp[j];
+                rank += (kj < key || (kj == key && j < t)) ? 1u : 0u;
+            }
+            lb.aux[rank] = e;
+        }
+        __syncthreads();
+        unsigned short* tt = lb.idx; lb.idx = lb.aux; lb.aux = tt;
+        return;
+    }
     while (vary) {
         const int sh = __ffsll((long long)vary) - 1;
         vary &= ~(0xffull << sh);
@@ -742,7 +768,12 @@ __device__ __forceinline__ void tree_phase0(const TreeArgs& A, Grid& g) {
     const i64 C = (N + G - 1) / G;
     const i64 c0 = min((i64)me * C, N), c1 = min(c0 + C, N);
     const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
-    auto IDX = [&](int t, int k) -> i64 { return c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane; };
+    // rows per warp: a chunk of less than a tile is spread over all warps of the CTA (rows beyond KP
+    // are out of range), so small chunks do not leave most warps idle
+    const int KP = ntiles == 1 ? (int)((C + GS_THREADS - 1) / GS_THREADS) : GS_KPT;
+    auto IDX = [&](int t, int k) -> i64 {
+        return k < KP ? c0 + (i64)t * GS_TILE + w * (32 * KP) + k * 32 + lane : (i64)1 << 62;
+    };
     (void)FULL; (void)le_mask; (void)gtid; (void)H; (void)BO; (void)ntiles; (void)c1;
     // ---- phase 0: chain lengths, last words, round-0 digits (leading bits of the first word) ----
     {
@@ -799,7 +830,12 @@ __device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& 
     const i64 C = (N + G - 1) / G;
     const i64 c0 = min((i64)me * C, N), c1 = min(c0 + C, N);
     const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
-    auto IDX = [&](int t, int k) -> i64 { return c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane; };
+    // rows per warp: a chunk of less than a tile is spread over all warps of the CTA (rows beyond KP
+    // are out of range), so small chunks do not leave most warps idle
+    const int KP = ntiles == 1 ? (int)((C + GS_THREADS - 1) / GS_THREADS) : GS_KPT;
+    auto IDX = [&](int t, int k) -> i64 {
+        return k < KP ? c0 + (i64)t * GS_TILE + w * (32 * KP) + k * 32 + lane : (i64)1 << 62;
+    };
     (void)FULL; (void)le_mask; (void)gtid; (void)H; (void)BO; (void)ntiles; (void)c1;
     int cb = 0, round = 0;
     // ---- round 0: stable sort by the round-0 key (generated on the fly from the digits) ----
@@ -1156,7 +1192,12 @@ __device__ __forceinline__ void tree_local_stage(const TreeArgs& A, const KeyLay
 }
 
 // groups and clusters from (order, lcp): three grid-wide phases
-__device__ __forceinline__ void tree_signals(const TreeArgs& A, Grid& g, TreeSmem& tsm, i32* lvl_hi) {
+// SM: LCP and the min hierarchy live in shared memory (one CTA, small queue): plain loads; else they
+// are global arrays other CTAs write between the phases: L2 loads
+template <bool SM>
+__device__ __forceinline__ void tree_signals(const TreeArgs& A, Grid& g, TreeSmem& tsm, i32* lvl_hi,
+                                             const i32* LCP, i32* mt_store) {
+    auto ldl = [&](const i32* p) -> i32 { return SM ? *p : __ldcg(p); };
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const unsigned le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
@@ -1168,13 +1209,18 @@ __device__ __forceinline__ void tree_signals(const TreeArgs& A, Grid& g, TreeSme
     const i64 C = (N + G - 1) / G;
     const i64 c0 = min((i64)me * C, N), c1 = min(c0 + C, N);
     const int ntiles = (int)((C + GS_TILE - 1) / GS_TILE);
-    auto IDX = [&](int t, int k) -> i64 { return c0 + (i64)t * GS_TILE + w * (32 * GS_KPT) + k * 32 + lane; };
+    // rows per warp: a chunk of less than a tile is spread over all warps of the CTA (rows beyond KP
+    // are out of range), so small chunks do not leave most warps idle
+    const int KP = ntiles == 1 ? (int)((C + GS_THREADS - 1) / GS_THREADS) : GS_KPT;
+    auto IDX = [&](int t, int k) -> i64 {
+        return k < KP ? c0 + (i64)t * GS_TILE + w * (32 * KP) + k * 32 + lane : (i64)1 << 62;
+    };
     (void)FULL; (void)le_mask; (void)gtid; (void)H; (void)BO; (void)ntiles; (void)c1;
     const bool want_groups = A.group_id || A.group_size || A.n_groups;
     const bool want_clusters = A.cluster_depth || A.cluster_size || A.cluster_id;
     if (!want_groups && !want_clusters) return;
     MinTree mt;
-    mintree_layout(mt, A.lcp, N, A.mt_buf);
+    mintree_layout(mt, LCP, N, mt_store);
     const i64 gwarp = gtid >> 5, nwarps = ((i64)G * GS_THREADS) >> 5;
 
     // ---- G1: per-CTA count of group starts (lcp == 0) and the last one; min-hierarchy level 1 ----
@@ -1183,7 +1229,7 @@ __device__ __forceinline__ void tree_signals(const TreeArgs& A, Grid& g, TreeSme
         i32 lastw = -1;
         for (int t = 0; t < ntiles; ++t) {
             i32 lv[GS_KPT];
-            ELEMS(k) { const i64 i = IDX(t, k); lv[k] = i < c1 ? __ldcg(A.lcp + i) : 1; }
+            ELEMS(k) { const i64 i = IDX(t, k); lv[k] = i < c1 ? ldl(LCP + i) : 1; }
             ELEMS(k) {
                 const i64 i = IDX(t, k);
                 const unsigned bal = __ballot_sync(FULL, lv[k] == 0);
@@ -1223,7 +1269,7 @@ __device__ __forceinline__ void tree_signals(const TreeArgs& A, Grid& g, TreeSme
             ELEMS(k) {
                 const i64 i = IDX(t, k);
                 lv[k] = 1; ln[k] = 0;
-                if (i < c1) { lv[k] = __ldcg(A.lcp + i); if (i + 1 < N) ln[k] = __ldcg(A.lcp + i + 1); }
+                if (i < c1) { lv[k] = ldl(LCP + i); if (i + 1 < N) ln[k] = ldl(LCP + i + 1); }
             }
             u32 cntw = 0, lastw = 0;
             ELEMS(k) {
@@ -1301,8 +1347,8 @@ __device__ __forceinline__ void tree_signals(const TreeArgs& A, Grid& g, TreeSme
             if (i < c1) {
                 r[k] = (u32)A.order[i];
                 if (want_groups) gid[k] = (i32)A.seg[i];
-                l0[k] = __ldcg(A.lcp + i);
-                if (i + 1 < N) l1[k] = __ldcg(A.lcp + i + 1);
+                l0[k] = ldl(LCP + i);
+                if (i + 1 < N) l1[k] = ldl(LCP + i + 1);
             }
         }
         if (want_groups) {
@@ -1338,9 +1384,9 @@ __device__ __forceinline__ void tree_signals(const TreeArgs& A, Grid& g, TreeSme
         i32 w_prev = 0, w_cur = 0, w_next = 0;
         if (SB == 1) {
             const i64 i = IDX(t, hb * SB);
-            w_cur = i < N ? __ldcg(A.lcp + i) : 0;
-            w_next = i + 32 < N ? __ldcg(A.lcp + i + 32) : 0;
-            w_prev = i >= 32 ? __ldcg(A.lcp + i - 32) : 0;
+            w_cur = i < N ? ldl(LCP + i) : 0;
+            w_next = i + 32 < N ? ldl(LCP + i + 32) : 0;
+            w_prev = (i >= 32 && i - 32 < N) ? ldl(LCP + i - 32) : 0;
             bool g0 = go[0];
             for (int d = 1; d < 64 && __any_sync(FULL, g0); ++d) {
                 const int idx = lane - d;
@@ -1454,7 +1500,7 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_tree_signals(TreeArgs A) {
     __shared__ i32 lvl_hi[LVL_HI_WORDS];
     Grid g{&A.ctl->bar2, 0};
     PEEK_MARK(23);
-    tree_signals(A, g, tsm, lvl_hi);
+    tree_signals<false>(A, g, tsm, lvl_hi, A.lcp, A.mt_buf);
 }
 
 __global__ void __launch_bounds__(GS_THREADS, 1) k_tree_small(TreeArgs A) {
@@ -1463,12 +1509,24 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_tree_small(TreeArgs A) {
     __shared__ TreeSmem tsm;
     Grid g{&A.ctl->bar, 0};  // one CTA: every grid barrier is a CTA barrier
     PEEK_MARK(1);
+    // one CTA: the control block is cleared here instead of by a memset node before the launch
+    for (int i = threadIdx.x; i < (int)(sizeof(TreeCtl) / 4); i += GS_THREADS) ((u32*)A.ctl)[i] = 0;
+    __syncthreads();
     tree_phase0(A, g);
     const KeyLayout kl = make_layout(A.N, __ldcg(&A.ctl->maxnb), LOC_W);
     tree_local_stage(A, kl, kl, true, 0, 0, ssm, tsm, dyn_smem);
     __syncthreads();
     PEEK_MARK(23);
-    tree_signals(A, g, tsm, (i32*)dyn_smem);  // the work item's buffers are free now
+    {   // the work item's buffers are free now: LCP and the min hierarchy move into shared memory, so
+        // the nearest-smaller-value walks of the cluster search cost shared-memory latency
+        i32* slcp = (i32*)dyn_smem;
+        const i64 N = A.N;
+        for (i64 i = threadIdx.x; i < N; i += GS_THREADS) slcp[i] = A.lcp[i];
+        i32* smt = slcp + ((N + 1 + 63) / 64) * 64;
+        i32* shi = smt + mintree_words(N);
+        __syncthreads();
+        tree_signals<true>(A, g, tsm, shi, slcp, smt);
+    }
 }
 
 static void tree_layout(Arena& a, i64 N, int grid, TreeArgs& A) {
@@ -1529,9 +1587,10 @@ static peek_status tree_launch(const u64* hashes, const i64* blk_off, i64 N, i32
     A.cap_seg = (g_tree_local_cap >= 128 && g_tree_local_cap < LOC_CAP) ? g_tree_local_cap : LOC_CAP;
     A.quantum = A.cap_seg / 2;
     tree_layout(a, N, MAX_GRID, A);
-    PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(MAX_GRID)) - (char*)A.ctl), st));
     void* params[] = {&A};
     const bool want_signals = group_id || group_size || n_groups || cluster_depth || cluster_size || cluster_id;
+    if (!(!signals_only && N <= (i64)A.cap_seg))
+        PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(MAX_GRID)) - (char*)A.ctl), st));
     if (!signals_only && N <= (i64)A.cap_seg) {  // the whole queue in one CTA, one launch, no grid barrier
         Prof pr(PROF_TREE, st, 1);
         PEEK_CUDA(func_smem_optin((const void*)k_tree_small, TREE_DYN_SMEM));
