@@ -1,6 +1,6 @@
 """Build libpeek.so (hand-written CUDA for sm_100a) in-tree with nvcc; cross-compiles without a GPU.
 
-    python -m paper_2607_02525_b200.build [--force] [-v]
+    python -m paper_2607_02525_b200.build [--force] [-v] [--checked]
 """
 from __future__ import annotations
 
@@ -12,6 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpeek.so")
+LIB_CHECKED = os.path.join(_HERE, "libpeek_checked.so")
 SOURCES = ["peek_api.cu", "peek_hash.cu", "peek_lpm.cu", "peek_tree.cu", "peek_demand.cu", "peek_signals.cu", "peek_offline.cu",
            "peek_interleave.cu"]
 HEADERS = ["peek_common.cuh", "peek_grid.cuh", "peek_sort.cuh", os.path.join("..", "..", "include", "peek.h")]
@@ -33,9 +34,13 @@ def _stale(out: str, deps) -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_libpeek(force: bool = False, verbose: bool = False) -> str:
+def build_libpeek(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    """checked=True builds libpeek_checked.so (-DPEEK_CHECKED: range checks on every index computed
+    from device data, canaries around the workspace pieces); load it with PEEK_LIB=<path>."""
     hdrs = [os.path.normpath(os.path.join(CSRC, h)) for h in HEADERS]
-    objdir = os.path.join(_HERE, "build")
+    objdir = os.path.join(_HERE, "build_checked" if checked else "build")
+    lib = LIB_CHECKED if checked else LIB
+    extra = ["-DPEEK_CHECKED"] if checked else []
     os.makedirs(objdir, exist_ok=True)
     nvcc = _nvcc()
     jobs = []
@@ -43,7 +48,7 @@ def build_libpeek(force: bool = False, verbose: bool = False) -> str:
         src = os.path.join(CSRC, s)
         obj = os.path.join(objdir, s.replace(".cu", ".o"))
         if force or _stale(obj, [src] + hdrs):
-            jobs.append([nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj])
+            jobs.append([nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj])
 
     def run(cmd):
         r = subprocess.run(cmd, capture_output=True, text=True)
@@ -56,10 +61,10 @@ def build_libpeek(force: bool = False, verbose: bool = False) -> str:
         with ThreadPoolExecutor(max_workers=len(jobs)) as ex:
             list(ex.map(run, jobs))
     objs = [os.path.join(objdir, s.replace(".cu", ".o")) for s in SOURCES]
-    if force or jobs or _stale(LIB, objs):
-        run([nvcc, "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"])
-    return LIB
+    if force or jobs or _stale(lib, objs):
+        run([nvcc, "-shared", "-o", lib] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"])
+    return lib
 
 
 if __name__ == "__main__":
-    print(build_libpeek(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build_libpeek(force="--force" in sys.argv, verbose="-v" in sys.argv, checked="--checked" in sys.argv))

@@ -46,6 +46,42 @@ struct Prof {  // brackets the kernels launched during its lifetime
 
 static inline i64 align_up(i64 x, i64 a) { return (x + a - 1) / a * a; }
 
+// ---- checked build (-DPEEK_CHECKED: libpeek_checked.so) ---------------------------------------
+// compute-sanitizer is closed on this pool, so memory safety gets a build of its own: every index
+// computed from device data is range-checked against the extent the arrays were passed with
+// (PEEK_CHECK: trap), and every piece of workspace is followed by a 256-byte canary that
+// is armed before the call's first kernel and verified after its last one.
+// A failed check traps (the call's stream reports a launch failure at the next synchronisation).
+// -DPEEK_CHECK_PRINT also prints the source line first; a device printf inside the big persistent
+// kernels needs more than the default 1 KB of stack (cudaLimitStackSize), so it is off by default.
+#if defined(PEEK_CHECKED) && defined(PEEK_CHECK_PRINT)
+#define PEEK_CHECK(cond, what)                                                                   \
+    do {                                                                                         \
+        if (!(cond)) {                                                                           \
+            printf("PEEK_CHECKED %s:%d: %s\n", __FILE__, __LINE__, what);                        \
+            __trap();                                                                            \
+        }                                                                                        \
+    } while (0)
+#elif defined(PEEK_CHECKED)
+#define PEEK_CHECK(cond, what) do { if (!(cond)) __trap(); } while (0)
+#endif
+#ifdef PEEK_CHECKED
+static constexpr int CANARY_MAX = 48;
+struct CanaryList { long long off[CANARY_MAX]; int n; };
+static __global__ void k_canary(unsigned char* base, CanaryList L, int verify) {
+    const int p = blockIdx.x;
+    if (p >= L.n) return;
+    unsigned char* c = base + L.off[p] + threadIdx.x;
+    if (!verify) *c = 0xC5;
+    else if (*c != 0xC5) {
+        printf("PEEK_CHECKED workspace canary %d (offset %lld) overwritten at byte %d\n", p, L.off[p], (int)threadIdx.x);
+        __trap();
+    }
+}
+#else
+#define PEEK_CHECK(cond, what) do { } while (0)
+#endif
+
 // Bump allocator over the caller's workspace (256-byte aligned pieces).
 struct Arena {
     char* base;
@@ -55,8 +91,29 @@ struct Arena {
     T* take(i64 n) {
         T* r = (T*)(base ? base + used : nullptr);
         used += align_up((n > 0 ? n : 1) * (i64)sizeof(T), 256);
+#ifdef PEEK_CHECKED
+        if (canaries.n < CANARY_MAX) canaries.off[canaries.n++] = used;
+        used += 256;
+#endif
         return r;
     }
+#ifdef PEEK_CHECKED
+    CanaryList canaries{{0}, 0};
+    cudaStream_t armed_on = nullptr;
+    bool armed = false;
+    // after the call's memsets, before its first kernel
+    void arm(cudaStream_t st) {
+        if (!base || !canaries.n) return;
+        k_canary<<<canaries.n, 256, 0, st>>>((unsigned char*)base, canaries, 0);
+        armed = true;
+        armed_on = st;
+    }
+    ~Arena() {  // after the call's last kernel has been enqueued
+        if (armed) k_canary<<<canaries.n, 256, 0, armed_on>>>((unsigned char*)base, canaries, 1);
+    }
+#else
+    void arm(cudaStream_t) {}
+#endif
 };
 
 // ---- device side -------------------------------------------------------------------------

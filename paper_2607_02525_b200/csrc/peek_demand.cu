@@ -477,6 +477,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
     RankArgs A;
     rank_layout(a, N, RANK_MAX_GRID, A);
     i32* mt_buf = a.take<i32>(mintree_words(N));
+    a.arm(st);
     if (demand) {
         MinTree mt;
         mintree_layout(mt, lcp, N, mt_buf);
@@ -496,6 +497,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
         i64 want = (N + GS_THREADS - 1) / GS_THREADS;
         if (want < grid) grid = (int)(want < 1 ? 1 : want);
         PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(RANK_MAX_GRID)) - (char*)A.ctl), st));
+        a.arm(st);  // the memset spans a canary
         void* params[] = {&A};
         Prof pr(PROF_RANK, st, 1);
         PEEK_CUDA(func_smem_optin((const void*)k_clpm_sort, GS_STAGE_BYTES));
@@ -514,6 +516,7 @@ static peek_status launch_sort_full(FullArgs& A, i64 N, void* ws, cudaStream_t s
     i64 want = (N + GS_THREADS - 1) / GS_THREADS;
     if (want < grid) grid = (int)(want < 1 ? 1 : want);
     PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(1024)) - (char*)A.ctl), st));
+    a.arm(st);
     PEEK_CUDA(func_smem_optin((const void*)k_clpm_sort_full, GS_STAGE_BYTES));
     void* params[] = {&A};
     Prof pr(PROF_RANK_FULL, st, 1);
@@ -619,6 +622,7 @@ extern "C" peek_status peek_clpm_group_major(const int32_t* lane_order, const in
     if (want < grid) grid = (int)(want < 1 ? 1 : want);
     PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(1024)) - (char*)A.ctl), st));
     PEEK_CUDA(cudaMemsetAsync(A.tkeys, 0xff, (size_t)((char*)(A.tfirst + (A.hmask + 1)) - (char*)A.tkeys), st));
+    a.arm(st);
     PEEK_CUDA(func_smem_optin((const void*)k_group_major, GS_STAGE_BYTES));
     void* params[] = {&A};
     Prof pr(PROF_RANK_FULL, st, 1);

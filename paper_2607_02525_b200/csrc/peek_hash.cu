@@ -443,6 +443,7 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
     i64 nchunks = (N + SCAN_CHUNK - 1) / SCAN_CHUNK;
     i64* partial = a.take<i64>(nchunks + 1);
     unsigned long long* counter = a.take<unsigned long long>(1);
+    a.arm(st);
     if (N <= SCAN_SMALL_MAX) {
         Prof pr(PROF_HASH_SCAN, st, 1);
         k_nb_scan_small<<<1, 1024, 0, st>>>(tok_off, N, blk_off, counter);

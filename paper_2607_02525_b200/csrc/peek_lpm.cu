@@ -439,6 +439,7 @@ struct DualArgs {
     RadixDev R; const EdgeInfo* info;                // radix mode (hit_radix != NULL)
     const u64* t_keys; u64 mask;                     // hash mode (hit_hash != NULL)
     const i32* order; const i32* lcp;
+    i32 V, E; i64 CT;  // extents of the radix arrays (range checks of the checked build)
     int win;
     i32 *hit_radix, *hit_hash;
     u32* ctr;             // work-item counter (zero on entry)
@@ -500,6 +501,7 @@ __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_du
                 const i64 jl = jb + lane;
                 const bool valid = jl < end;
                 const i32 r_l = valid ? __ldg(A.order + jl) : 0;
+                PEEK_CHECK(r_l >= 0 && (i64)r_l < N, "order[] entry out of range");
                 const i32 s_l = valid ? 16 * __ldg(A.lcp + jl) : 0;
                 const i64 o_l = valid ? __ldg(A.tok_off + r_l) : 0;
                 const i32 len_l = valid ? (i32)(__ldg(A.tok_off + r_l + 1) - o_l) : 0;
@@ -545,7 +547,10 @@ __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_du
                             const bool sm = at_root && ce1 <= root_staged;
                             const i32 e = find_child_in(sm ? root_ft : A.R.e_first_tok, ce0, ce1, t, lane, sm);
                             if (e < 0) break;
+                            PEEK_CHECK(e < A.E, "edge index out of range");
                             const EdgeInfo ei = A.info[e];
+                            PEEK_CHECK(ei.child > 0 && ei.child < A.V && ei.tok_off >= 0 && ei.tok_off + ei.tok_len <= A.CT &&
+                                       ei.ce0 <= ei.ce1 && ei.ce1 <= A.E, "radix node out of range");
                             if (top < 32) {
                                 if (lane == 0) st[top] = PathEntry{d, ei.tok_len, ei.ce0, ei.ce1, ei.tok_off};
                                 ++top;
@@ -574,6 +579,7 @@ __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_du
                 const i64 jl = jb + lane;
                 const bool valid = jl < end;
                 const i32 r_l = valid ? __ldg(A.order + jl) : 0;
+                PEEK_CHECK(r_l >= 0 && (i64)r_l < N, "order[] entry out of range");
                 const i32 s_l = valid ? __ldg(A.lcp + jl) : 0;
                 const i64 b_l = valid ? __ldg(A.blk_off + r_l) : 0;
                 const i32 nb_l = valid ? (i32)(__ldg(A.blk_off + r_l + 1) - b_l) : 0;
@@ -721,6 +727,7 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
     Fn* partial = a.take<Fn>(nchunks + 1);
     EdgeInfo* info = a.take<EdgeInfo>(VE);
     u32* ctr = a.take<u32>(64);
+    a.arm(st);
     auto resolve = [&](const i32* W, i32* hit) {
         if (N <= 65536) {
             Prof pr(PROF_LPM_RESOLVE, st, 1);
@@ -740,6 +747,7 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
         DualArgs D;
         D.tokens = tokens; D.tok_off = tok_off; D.hashes = hashes; D.blk_off = blk_off; D.N = N;
         D.R = R; D.info = info;
+        D.V = hit_radix ? radix->V : 0; D.E = hit_radix ? radix->E : 0; D.CT = hit_radix ? radix->CT : 0;
         D.t_keys = hit_hash ? table->t_keys : nullptr; D.mask = hit_hash ? (u64)(table->S - 1) : 0;
         D.order = order; D.lcp = lcp; D.win = win; D.hit_radix = hit_radix; D.hit_hash = hit_hash;
         D.counters = g_lpm_counters;

@@ -202,6 +202,7 @@ extern "C" peek_status peek_offline_phase1(const uint64_t* hashes, const int64_t
     PEEK_CUDA(cudaMemsetAsync(A.ncount, 0, sizeof(u32) * (size_t)(A.hmask + 1), st));
     // kand starts as all ones
     PEEK_CUDA(cudaMemsetAsync(A.ctl->kand, 0xff, sizeof(A.ctl->kand), st));
+    a.arm(st);
     Prof pr(PROF_OFFLINE, st, 3);
     i64 work = N * depth_blocks;
     unsigned grid = (unsigned)((work + OF_THREADS - 1) / OF_THREADS);

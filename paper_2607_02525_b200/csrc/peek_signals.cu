@@ -379,6 +379,7 @@ extern "C" peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* 
     Arena a(ws);
     SignalsWs W;
     signals_layout(a, N, W);
+    a.arm(st);
     MinTree mt;
     mintree_layout(mt, lcp, N, W.mt_buf);
     Prof pr(PROF_SIGNALS, st, (mt.levels - 1) + (score ? 4 : 0) + (evict_score ? 3 : 0) + (section ? 2 : 0));

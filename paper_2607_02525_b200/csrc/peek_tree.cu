@@ -524,6 +524,7 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
         u32 r;
         if (mode == LOCAL_FROM_GLOBAL) { lb.key[i] = __ldcg(Kg + p0 + i); r = __ldcg(Vg + p0 + i); }
         else { lb.key[i] = round0_key(kl, __ldcg(A.srank + i)); r = (u32)i; }
+        PEEK_CHECK((i64)r < A.N, "request id of a sorted pair out of range");
         lb.val[i] = r;
         lb.idx[i] = (unsigned short)i;
         if (mode == LOCAL_FROM_GLOBAL) lb.na[i] = __ldcg(A.posna + p0 + i);
@@ -647,6 +648,7 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
                     const u32 a = lb.aux[i];
                     if (a == (0x8000u | (u32)i)) {  // an unresolved segment starts here
                         const unsigned long long hv = __ldcg(&A.segrec[p0 + i].head);
+                        PEEK_CHECK(0xffffffffu - (u32)hv < (u32)n, "segment head position outside the work item");
                         const u32 h = lb.val[lb.idx[0xffffffffu - (u32)hv]];
                         i64 bo; i32 nh; u64 lh, k0b;
                         rec_load(rec, h, bo, nh, lh, k0b);
@@ -683,6 +685,7 @@ __device__ __forceinline__ void tree_local(const TreeArgs& A, const KeyLayout& k
                 LSUBS(k) {
                     rk[k] = 0; hv[k] = 0; ao[k] = 0; na[k] = 0; lo[k] = 0; al[k] = 0; k0a[k] = 0; bo[k] = 0; k0b[k] = 0;
                     if (val_[k]) {
+                        PEEK_CHECK((int)sg[k] < n && p0 + sg[k] < A.N, "segment start outside the work item");
                         const ulonglong2* sp = (const ulonglong2*)(A.segrec + p0 + sg[k]);
                         const ulonglong2 s0 = __ldcg(sp), s1 = __ldcg(sp + 1);
                         hv[k] = s0.x; bo[k] = (i64)s0.y; k0b[k] = s1.x;
@@ -993,10 +996,12 @@ __device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& 
                             max_size = max(max_size, size);
                             if (size > (u32)A.quantum && size <= (u32)A.cap_seg) {
                                 const u32 slot = atomicAdd(&A.ctl->nbig[round % 3], 1u);
+                                PEEK_CHECK((i64)slot < A.N / 64 + 64, "big-segment list overflow");
                                 A.biglist[slot] = (u64)(u32)s | ((u64)size << 32);
                             }
                         }
                         r[k] = un[k] ? __ldcg(cur + i) : 0u;
+                        PEEK_CHECK((i64)r[k] < N, "R1b: request id out of range");
                     }
                     u32 nbr[SB];
                     SUBS(k) nbr[k] = un[k] ? __ldg(&A.rec[r[k]].na) : 0u;
@@ -1064,6 +1069,7 @@ __device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& 
                     sg[k] = 0; r[k] = 0; rk[k] = 0;
                     if (i < c1) { sg[k] = A.seg[i]; r[k] = __ldcg(cur + i); rk[k] = A.srank[i]; }
                     un[k] = (sg[k] >> 31) != 0;
+                    PEEK_CHECK((i64)(sg[k] & 0x7fffffffu) < N, "R2: segment start out of range");
                 }
                 u64 hv[SB], al[SB], k0a[SB], k0b[SB];
                 i64 ao[SB], bo[SB];
@@ -1077,7 +1083,11 @@ __device__ __forceinline__ void tree_global(const TreeArgs& A, const KeyLayout& 
                         rec_load(A.rec, r[k], ao[k], na[k], al[k], k0a[k]);
                     }
                 }
-                SUBS(k) { h[k] = un[k] ? __ldcg(cur + (0xffffffffu - (u32)hv[k])) : 0u; nb[k] = (i32)(hv[k] >> 32); }
+                SUBS(k) {
+                    PEEK_CHECK(!un[k] || (i64)(0xffffffffu - (u32)hv[k]) < N, "R2: segment head position out of range");
+                    h[k] = un[k] ? __ldcg(cur + (0xffffffffu - (u32)hv[k])) : 0u; nb[k] = (i32)(hv[k] >> 32);
+                    PEEK_CHECK((i64)h[k] < N && (i64)r[k] < N, "R2: request id out of range");
+                }
                 SUBS(k) {
                     bo[k] = 0; k0b[k] = 0;
                     if (un[k]) { i32 nh; u64 lh; rec_load(A.rec, h[k], bo[k], nh, lh, k0b[k]); }
@@ -1148,6 +1158,7 @@ __device__ __forceinline__ void tree_local_stage(const TreeArgs& A, const KeyLay
                     const u64 e = __ldcg(A.biglist + it);
                     p0 = (i64)(u32)e;
                     n = (int)(e >> 32);
+                    PEEK_CHECK(n > 0 && n <= LOC_CAP && p0 + n <= N, "big work item out of range");
                 } else {
                     if (it >= nq) break;
                     const i64 a = (i64)it * Q, b = min(a + Q, N);
@@ -1184,6 +1195,7 @@ __device__ __forceinline__ void tree_local_stage(const TreeArgs& A, const KeyLay
                     un_any = __syncthreads_or(un_any);
                     if (!un_any) { tree_direct_output(A, cur, p0, e); continue; }
                     n = (int)(e - p0);
+                    PEEK_CHECK(n > 0 && n <= LOC_CAP && p0 + n <= N, "quantum work item out of range");
                 }
             }
             tree_local(A, kg, kl, K, cur, p0, n, whole ? LOCAL_WHOLE_QUEUE : LOCAL_FROM_GLOBAL, ssm, tsm, lb);
@@ -1591,6 +1603,7 @@ static peek_status tree_launch(const u64* hashes, const i64* blk_off, i64 N, i32
     const bool want_signals = group_id || group_size || n_groups || cluster_depth || cluster_size || cluster_id;
     if (!(!signals_only && N <= (i64)A.cap_seg))
         PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(MAX_GRID)) - (char*)A.ctl), st));
+    a.arm(st);
     if (!signals_only && N <= (i64)A.cap_seg) {  // the whole queue in one CTA, one launch, no grid barrier
         Prof pr(PROF_TREE, st, 1);
         PEEK_CUDA(func_smem_optin((const void*)k_tree_small, TREE_DYN_SMEM));
@@ -1824,6 +1837,7 @@ extern "C" peek_status peek_pending_tree_update(const uint64_t* hashes, const in
     Arena a(ws);
     UpdWs W;
     update_layout(a, N_old, N_new, M, W);
+    a.arm(st);
     if (M > 0) {  // the arrivals' own tree: their chains are requests N_new - M .. N_new - 1
         peek_status rc = tree_launch(hashes, blk_off + (N_new - M), M, W.b_order, W.b_lcp, nullptr, nullptr,
                                      nullptr, nullptr, nullptr, nullptr, 0, W.tree_ws, st);
