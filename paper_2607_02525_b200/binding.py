@@ -151,6 +151,8 @@ def workspace_bytes(call_id: int, N=0, T=0, NB=0, S=0, V=0) -> int:
 
 def _ws(call_id, device, **sizes):
     """Scratch for one call, cached per (device, stream, call): two streams never share a buffer."""
+    if torch.device(device).type != "cuda":
+        raise PeekError("expected CUDA tensors (the library has no CPU path)")
     need = workspace_bytes(call_id, **sizes)
     key = (str(device), int(torch.cuda.current_stream(device).cuda_stream), call_id)
     buf = _ws_cache.get(key)
