@@ -387,6 +387,31 @@ def test_lpm_work_counters():
     assert dual[2] * 3 < naive[2] and dual[3] * 2 < naive[3]
 
 
+@pytest.mark.parametrize("cfg,G", [(2, 2), (5, 3), (4, 4)])
+def test_sharded_queue_emulated(cfg, G):
+    """SURVEY.md section 8(e) through the CUDA calls: the G shards of one queue (by first-block hash) run
+    one after the other on this GPU, demand summed, cLPM keys merged - equal to the oracle on the
+    whole queue (the collectives themselves are covered by tests/test_sharded_gloo.py)."""
+    b = _b()
+    from paper_2607_02525_b200 import sharded
+    wl = W.make(cfg, seed=42, small=True)
+    toks, off = wl.queue.materialize_np()
+    cache = W.build_cache(wl, lambda t, o: oracle.block_hash(t, o, 16, 0))
+    d_keys = _dev(cache.t_keys.view(np.int64), torch.uint64)
+    d_radix = _radix_dev(cache.radix) if cache.radix is not None else None
+    res = sharded.sharded_step_emulated(b, _dev(toks), _dev(off), _dev(wl.arrival), d_radix, d_keys,
+                                        int(d_keys.shape[0]), G)
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    ot = oracle.pending_tree(o_h, o_bo)
+    o_hit = oracle.lpm_radix(toks, off, _orc_radix(cache.radix)) if cache.radix is not None else \
+        oracle.lpm_hash(o_h, o_bo, cache.t_keys)
+    assert np.array_equal(_np(res.hit), o_hit)
+    assert np.array_equal(_np(res.cluster_size), ot.cluster_size)
+    assert np.array_equal(_np(res.demand), oracle.demand(o_h, o_bo, cache.t_keys))
+    assert np.array_equal(_np(res.clpm_order), oracle.clpm_order(o_hit, ot.cluster_size, wl.arrival))
+    assert len(np.unique(_np(res.owner))) > 1 or cfg == 3
+
+
 def test_rank_two_phase_wide_keys():
     """cLPM keys too wide for one 64-bit packed key (full-range hit, cluster size and arrival):
     the arrival sort followed by the stable (hit, cluster size) sort."""
