@@ -83,13 +83,39 @@ __device__ __forceinline__ i64 match_len(const i32* __restrict__ a, const i32* _
     return limit;
 }
 
-// the dual walk's compare: every round trip looks at 32 x 10 tokens (a turn's new segment, the run of
-// tokens a resumed walk usually has to confirm, fits one trip; loads past `limit` are predicated off)
-__device__ __forceinline__ i64 match_len_wide(const i32* __restrict__ a, const i32* __restrict__ b, i64 limit,
+// the dual walk's compare: every round trip looks at up to 32 x 10 tokens (a turn's new segment, the
+// run of tokens a resumed walk usually has to confirm, fits one trip).  Three unrollings - 2, 4 or
+// 10 rows - picked by the remaining length (warp uniform), so a short compare does not pay for the
+// loads and votes of rows past its end; 32-bit indices (a label is shorter than 2^31 tokens).
+template <int U>
+__device__ __forceinline__ bool match_rows(const i32* __restrict__ pa, const i32* __restrict__ pb, i32 mine, i32* f) {
+    i32 x[U], y[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const bool in = u * 32 < mine;  // this lane's token of row u is inside the compare
+        x[u] = in ? __ldg(pa + u * 32) : 0;
+        y[u] = in ? __ldg(pb + u * 32) : 1;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const unsigned neq = __ballot_sync(0xffffffffu, x[u] != y[u]);
+        if (neq) { *f = u * 32 + (__ffs(neq) - 1); return true; }
+    }
+    return false;
+}
+__device__ __forceinline__ i32 match_len_wide(const i32* __restrict__ a, const i32* __restrict__ b, i32 limit,
                                               int lane) {
-    i64 m = limit;
-    for (i64 base = 0; base < limit; base += 320)
-        if (match_step<10>(a, b, base, limit, lane, &m)) return m;
+    for (i32 base = 0; base < limit; base += 320) {
+        const i32* __restrict__ pa = a + base + lane;
+        const i32* __restrict__ pb = b + base + lane;
+        const i32 rem = limit - base, mine = rem - lane;
+        i32 f = 0;
+        bool hit;
+        if (rem <= 64) hit = match_rows<2>(pa, pb, mine, &f);
+        else if (rem <= 128) hit = match_rows<4>(pa, pb, mine, &f);
+        else hit = match_rows<10>(pa, pb, mine, &f);
+        if (hit) { f += base; return f < limit ? f : limit; }
+    }
     return limit > 0 ? limit : 0;
 }
 
@@ -507,14 +533,22 @@ __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_du
                 const i32 len_l = valid ? (i32)(__ldg(A.tok_off + r_l + 1) - o_l) : 0;
                 i32 H_l = 0;
                 const int cnt = (int)min((i64)32, end - jb);
+                // positions that only copy their predecessor's hit are skipped in one vote: the next
+                // position that has to touch the cache is the first one whose shared depth the
+                // current hit reaches (the run's first position always walks)
                 for (int i = 0; i < cnt; ++i) {
-                    i32 s = __shfl_sync(FULL, s_l, i);
                     const bool first = (jb == head && i == 0);
+                    if (!first) {
+                        const unsigned wm = __ballot_sync(FULL, lane >= i && lane < cnt && s_l <= Hprev);
+                        const int nx = wm ? __ffs(wm) - 1 : cnt;
+                        if (lane >= i && lane < nx) H_l = Hprev;
+                        i = nx;
+                        if (i >= cnt) break;
+                    }
+                    i32 s = __shfl_sync(FULL, s_l, i);
                     if (first) s = 0;
                     i32 H;
-                    if (!first && Hprev < s) {
-                        H = Hprev;
-                    } else {
+                    {
                         const i64 o = __shfl_sync(FULL, o_l, i);
                         const i32 len = __shfl_sync(FULL, len_l, i);
                         const i32* __restrict__ q = A.tokens + o;
@@ -586,13 +620,18 @@ __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_du
                 i32 H_l = 0;
                 const int cnt = (int)min((i64)32, end - jb);
                 for (int i = 0; i < cnt; ++i) {
-                    i32 s = __shfl_sync(FULL, s_l, i);
                     const bool first = (jb == head && i == 0);
+                    if (!first) {  // skip the positions that only copy (see the radix loop)
+                        const unsigned wm = __ballot_sync(FULL, lane >= i && lane < cnt && s_l <= Hprev);
+                        const int nx = wm ? __ffs(wm) - 1 : cnt;
+                        if (lane >= i && lane < nx) H_l = Hprev;
+                        i = nx;
+                        if (i >= cnt) break;
+                    }
+                    i32 s = __shfl_sync(FULL, s_l, i);
                     if (first) s = 0;
                     i32 H;
-                    if (!first && Hprev < s) {
-                        H = Hprev;
-                    } else {
+                    {
                         const i64 b0 = __shfl_sync(FULL, b_l, i);
                         const i32 nb = __shfl_sync(FULL, nb_l, i);
                         if (first) ++c_walks;
