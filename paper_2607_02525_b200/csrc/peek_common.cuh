@@ -139,6 +139,20 @@ __device__ __forceinline__ int4 ld_stream_v4(const void* p) {
                  : "l"(p));
     return r;
 }
+// 64-bit loads with an L2 eviction policy: the probed table is re-read by every call and should stay
+// in L2 (evict last); words of the hash array are read once per call (evict first)
+__device__ __forceinline__ u64 ld_u64_keep(const u64* p) {
+    u64 pol, v;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("ld.global.nc.L2::cache_hint.u64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ u64 ld_u64_once(const u64* p) {
+    u64 pol, v;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("ld.global.nc.L2::cache_hint.u64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
+    return v;
+}
 __device__ __forceinline__ u32 ld_acquire_u32(const u32* p) {
     u32 v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");

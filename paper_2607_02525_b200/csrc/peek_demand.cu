@@ -20,7 +20,7 @@ __device__ __forceinline__ i64 table_slot_from(const u64* __restrict__ t_keys, u
         if (tk == key) return (i64)p;
         if (tk == PEEK_EMPTY) return -1;
         p = (p + 1) & mask;
-        tk = __ldg(t_keys + p);
+        tk = ld_u64_keep(t_keys + p);
     }
 }
 
@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(DM_THREADS) k_demand(const u64* __restrict__ h
             }
             const int q = lo;
             const i32 i = M.l0[q] + (itc - __shfl_sync(FULL, excl, q));
-            key[u] = __ldg(hashes + M.b0[q] + i);
+            key[u] = ld_u64_once(hashes + M.b0[q] + i);
             i32 c = 1;
             if (i < M.l1[q]) {
                 if (i >= M.lo1[q]) c = M.cnt1[q];
@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(DM_THREADS) k_demand(const u64* __restrict__ h
 #pragma unroll
         for (int u = 0; u < DM_UNROLL; ++u) {
             slot0[u] = key[u] & mask;
-            tk[u] = __ldg(t_keys + slot0[u]);
+            tk[u] = ld_u64_keep(t_keys + slot0[u]);
         }
 #pragma unroll
         for (int u = 0; u < DM_UNROLL; ++u) {

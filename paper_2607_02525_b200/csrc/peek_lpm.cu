@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(LPM_THREADS) k_lpm_radix(const i32* __restrict
 __device__ __forceinline__ bool table_has(const u64* __restrict__ t_keys, u64 mask, u64 key) {
     u64 p = key & mask;
     for (;;) {
-        u64 tk = __ldg(t_keys + p);
+        u64 tk = ld_u64_keep(t_keys + p);
         if (tk == key) return true;
         if (tk == PEEK_EMPTY) return false;
         p = (p + 1) & mask;
@@ -643,7 +643,7 @@ __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_du
                             const i32 x = i0 + lane;
                             bool miss = false;
                             const bool act = lane < batch && x < nb;
-                            if (act) miss = !table_has(A.t_keys, A.mask, __ldg(A.hashes + b0 + x));
+                            if (act) miss = !table_has(A.t_keys, A.mask, ld_u64_once(A.hashes + b0 + x));
                             c_probe += (u32)__popc(__ballot_sync(FULL, act));
                             const unsigned m = __ballot_sync(FULL, miss);
                             if (m) { H = i0 + (__ffs(m) - 1); break; }
