@@ -157,6 +157,11 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_clpm_sort(RankArgs A) {
     const i64 gtid = (i64)blockIdx.x * GS_THREADS + threadIdx.x, gsize = (i64)gridDim.x * GS_THREADS;
     Grid g{&A.ctl->bar, 0};
     PEEK_MARK(1);
+    if (gridDim.x == 1) {  // one CTA: the control block and the sort's accumulators are cleared here, not by a memset node
+        for (int i = threadIdx.x; i < (int)(sizeof(RankCtl) / 4); i += GS_THREADS) ((u32*)A.ctl)[i] = 0;
+        for (int i = threadIdx.x; i < (int)gs_hist_words(1); i += GS_THREADS) A.bufs.hist[i] = 0;
+        __syncthreads();
+    }
     const i32* __restrict__ hit = A.hit;
     const i32* __restrict__ cs = A.csize;
     const i32* __restrict__ arr = A.arrival;
@@ -481,7 +486,7 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
     if (demand) {
         MinTree mt;
         mintree_layout(mt, lcp, N, mt_buf);
-        Prof pr(PROF_DEMAND, st, mt.levels);
+        Prof pr(PROF_DEMAND, st, mintree_launches(mt) + 1);
         mintree_build(mt, st);
         int ppw = 32;  // at least ~16 K warps when the queue is small
         while (ppw > 1 && N / ppw < 16384) ppw >>= 1;
@@ -496,13 +501,16 @@ extern "C" peek_status peek_demand_rank(const uint64_t* hashes, const int64_t* b
         if (grid > RANK_MAX_GRID) grid = RANK_MAX_GRID;
         i64 want = (N + GS_THREADS - 1) / GS_THREADS;
         if (want < grid) grid = (int)(want < 1 ? 1 : want);
-        PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(RANK_MAX_GRID)) - (char*)A.ctl), st));
-        a.arm(st);  // the memset spans a canary
+        if (grid > 1) {
+            PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(RANK_MAX_GRID)) - (char*)A.ctl), st));
+            a.arm(st);  // the memset spans a canary
+        }
         void* params[] = {&A};
         Prof pr(PROF_RANK, st, 1);
         PEEK_CUDA(func_smem_optin((const void*)k_clpm_sort, GS_STAGE_BYTES));
-        PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort, dim3(grid), dim3(GS_THREADS), params,
-                                              GS_STAGE_BYTES, st));
+        if (grid == 1) k_clpm_sort<<<1, GS_THREADS, GS_STAGE_BYTES, st>>>(A);  // one CTA: no co-residency to ask for
+        else PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_clpm_sort, dim3(grid), dim3(GS_THREADS), params,
+                                                   GS_STAGE_BYTES, st));
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;

@@ -241,7 +241,21 @@ static __global__ void __launch_bounds__(256) k_mintree_level(MinTree mt, int k)
     i64 nw = ((i64)gridDim.x * blockDim.x) >> 5;
     mintree_build_level(mt, k, gw, nw, threadIdx.x & 31);
 }
+// small inputs: every level in one launch of one CTA (a CTA barrier between levels)
+static __global__ void __launch_bounds__(1024) k_mintree_all(MinTree mt) {
+    for (int k = 1; k < mt.levels; ++k) {
+        mintree_build_level(mt, k, (i64)(threadIdx.x >> 5), (i64)(blockDim.x >> 5), threadIdx.x & 31);
+        __syncthreads();
+    }
+}
+static inline int mintree_launches(const MinTree& mt) {
+    return mt.levels <= 1 ? 0 : (mt.n[1] <= 1024 ? 1 : mt.levels - 1);
+}
 static inline void mintree_build(const MinTree& mt, cudaStream_t st) {
+    if (mt.levels > 1 && mt.n[1] <= 1024) {  // N <= 32768
+        k_mintree_all<<<1, 1024, 0, st>>>(mt);
+        return;
+    }
     for (int k = 1; k < mt.levels; ++k) {
         i64 warps = mt.n[k];
         unsigned grid = (unsigned)((warps * 32 + 255) / 256);

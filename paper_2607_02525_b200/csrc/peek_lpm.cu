@@ -17,6 +17,7 @@
 namespace peek {
 
 static constexpr int LPM_THREADS = 256;
+static constexpr int LPM_SMALL_MAX = 2048;  // queues up to this size: one launch, a warp per request, both modes
 static constexpr int CMP_UNROLL = 8;
 
 struct RadixDev {
@@ -201,6 +202,47 @@ __global__ void __launch_bounds__(LPM_THREADS) k_lpm_hash(const u64* __restrict_
     }
     if (lane == 0) out[r] = (i32)(hit * 16);
     if (counters && lane == 0) { atomicAdd(counters + 0, 1ull); atomicAdd(counters + 3, (unsigned long long)c_probe); }
+}
+
+// ---- small queues: both modes in ONE launch, a warp per request ------------------------------------
+// The paper's queues hold 60-200 requests: there the call is bound by launches, not by
+// the walks, so the co-descent machinery (edge table, counters, scans) is skipped: every request
+// walks on its own, radix mode then hash mode, in one kernel.
+__global__ void __launch_bounds__(LPM_THREADS) k_lpm_small(const i32* __restrict__ tokens,
+                                                          const i64* __restrict__ tok_off,
+                                                          const u64* __restrict__ hashes,
+                                                          const i64* __restrict__ blk_off, i64 N, RadixDev R,
+                                                          const u64* __restrict__ t_keys, u64 mask,
+                                                          i32* __restrict__ hit_radix, i32* __restrict__ hit_hash,
+                                                          unsigned long long* counters) {
+    const int lane = threadIdx.x & 31;
+    const i64 r = ((i64)blockIdx.x * LPM_THREADS + threadIdx.x) >> 5;
+    if (r >= N) return;
+    u32 c_look = 0, c_tok = 0, c_probe = 0;
+    if (hit_radix) {
+        const i64 o = tok_off[r];
+        const i32 h = radix_walk(R, tokens + o, tok_off[r + 1] - o, 0, lane, c_look, c_tok);
+        if (lane == 0) hit_radix[r] = h;
+    }
+    if (hit_hash) {
+        const i64 b0 = blk_off[r], nb = blk_off[r + 1] - b0;
+        i64 hit = nb;
+        for (i64 i0 = 0; i0 < nb; i0 += 32) {
+            const i64 i = i0 + lane;
+            bool miss = false;
+            if (i < nb) miss = !table_has(t_keys, mask, hashes[b0 + i]);
+            c_probe += (u32)__popc(__ballot_sync(0xffffffffu, i < nb));
+            const unsigned m = __ballot_sync(0xffffffffu, miss);
+            if (m) { hit = i0 + (__ffs(m) - 1); break; }
+        }
+        if (lane == 0) hit_hash[r] = (i32)(hit * 16);
+    }
+    if (counters && lane == 0) {
+        atomicAdd(counters + 0, (unsigned long long)((hit_radix ? 1 : 0) + (hit_hash ? 1 : 0)));
+        if (c_look) atomicAdd(counters + 1, (unsigned long long)c_look);
+        if (c_tok) atomicAdd(counters + 2, (unsigned long long)c_tok);
+        if (c_probe) atomicAdd(counters + 3, (unsigned long long)c_probe);
+    }
 }
 
 // ---- speculative co-descent (small N, long requests) -----------------------------------------
@@ -781,7 +823,13 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
     RadixDev R{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     if (hit_radix) R = RadixDev{radix->c_tokens, radix->n_tok_off, radix->n_tok_len,
                                 radix->n_child_off, radix->e_first_tok, radix->e_child};
-    if (dual) {  // persistent kernels, one per mode (plus the edge table of the radix cache)
+    if (g_lpm_strategy == PEEK_LPM_AUTO && N <= LPM_SMALL_MAX) {  // small queue: one launch for both modes
+        Prof pr(hit_radix ? PROF_LPM_RADIX : PROF_LPM_HASH, st, 1);
+        k_lpm_small<<<warps_grid, LPM_THREADS, 0, st>>>(tokens, tok_off, hashes, blk_off, N, R,
+                                                        hit_hash ? table->t_keys : nullptr,
+                                                        hit_hash ? (u64)(table->S - 1) : 0, hit_radix, hit_hash,
+                                                        g_lpm_counters);
+    } else if (dual) {  // persistent kernels, one per mode (plus the edge table of the radix cache)
         PEEK_CUDA(cudaMemsetAsync(ctr, 0, 256, st));
         DualArgs D;
         D.tokens = tokens; D.tok_off = tok_off; D.hashes = hashes; D.blk_off = blk_off; D.N = N;

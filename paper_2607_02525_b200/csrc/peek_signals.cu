@@ -382,7 +382,7 @@ extern "C" peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* 
     a.arm(st);
     MinTree mt;
     mintree_layout(mt, lcp, N, W.mt_buf);
-    Prof pr(PROF_SIGNALS, st, (mt.levels - 1) + (score ? 4 : 0) + (evict_score ? 3 : 0) + (section ? 2 : 0));
+    Prof pr(PROF_SIGNALS, st, mintree_launches(mt) + (score ? 4 : 0) + (evict_score ? 3 : 0) + (section ? 2 : 0));
     mintree_build(mt, st);
     unsigned grid = (unsigned)((N + SG_THREADS - 1) / SG_THREADS);
     if (grid > 148u * 16u) grid = 148u * 16u;
