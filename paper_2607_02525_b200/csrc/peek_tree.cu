@@ -1570,7 +1570,8 @@ i64 pending_tree_ws_bytes(i64 N) {
     return a.used;
 }
 
-static int g_tree_local_cap = 0;  // PEEK_OPT_TREE_LOCAL_CAP (0 = LOC_CAP)
+static int g_tree_local_cap = 0;  // PEEK_OPT_TREE_LOCAL_CAP (0 = automatic)
+static constexpr int TREE_SMALL_MAX = 2048;  // queues up to this size run in one CTA from the first step on
 void tree_set_option(int key, i64 v) {
     if (key == PEEK_OPT_TREE_LOCAL_CAP) g_tree_local_cap = (int)v;
 }
@@ -1596,15 +1597,30 @@ static peek_status tree_launch(const u64* hashes, const i64* blk_off, i64 N, i32
     A.signals_only = signals_only;
     // what one CTA finishes alone: segments of up to cap_seg positions; those above the quantum are
     // work items of their own, the others are taken a quantum of positions at a time
-    A.cap_seg = (g_tree_local_cap >= 128 && g_tree_local_cap < LOC_CAP) ? g_tree_local_cap : LOC_CAP;
-    A.quantum = A.cap_seg / 2;
+    if (g_tree_local_cap >= 128 && g_tree_local_cap < LOC_CAP) {  // test hook
+        A.cap_seg = g_tree_local_cap;
+        A.quantum = A.cap_seg / 2;
+    } else if (N <= TREE_SMALL_MAX) {  // the whole queue is one work item of one CTA
+        A.cap_seg = LOC_CAP;
+        A.quantum = LOC_CAP / 2;
+    } else {
+        // a work item occupies one SM: mid-size queues get smaller items (and, for their few big
+        // segments, more grid-wide rounds) so that the local stage has enough of them to fill the GPU
+        const i64 c = N / 8;
+        A.cap_seg = (int)(c < 1024 ? 1024 : (c > LOC_CAP ? LOC_CAP : c));
+        i64 q = ((N / (2 * (i64)sm_count()) + 127) / 128) * 128;
+        if (q < 256) q = 256;
+        if (q > A.cap_seg / 2 || c >= LOC_CAP) q = A.cap_seg / 2;  // big queues: plenty of items anyway, fewer is cheaper
+        A.quantum = (int)q;
+    }
     tree_layout(a, N, MAX_GRID, A);
     void* params[] = {&A};
     const bool want_signals = group_id || group_size || n_groups || cluster_depth || cluster_size || cluster_id;
-    if (!(!signals_only && N <= (i64)A.cap_seg))
+    const bool whole = !signals_only && N <= (i64)A.cap_seg && (N <= TREE_SMALL_MAX || g_tree_local_cap > 0);
+    if (!whole)
         PEEK_CUDA(cudaMemsetAsync(A.ctl, 0, (size_t)((char*)(A.bufs.hist + gs_hist_words(MAX_GRID)) - (char*)A.ctl), st));
     a.arm(st);
-    if (!signals_only && N <= (i64)A.cap_seg) {  // the whole queue in one CTA, one launch, no grid barrier
+    if (whole) {  // the whole queue in one CTA, one launch, no grid barrier
         Prof pr(PROF_TREE, st, 1);
         PEEK_CUDA(func_smem_optin((const void*)k_tree_small, TREE_DYN_SMEM));
         k_tree_small<<<1, GS_THREADS, TREE_DYN_SMEM, st>>>(A);
@@ -1617,7 +1633,11 @@ static peek_status tree_launch(const u64* hashes, const i64* blk_off, i64 N, i32
         PEEK_CUDA(cudaLaunchCooperativeKernel((const void*)k_tree_global, dim3(grid), dim3(GS_THREADS), params,
                                               GS_STAGE_BYTES, st));
         PEEK_CUDA(func_smem_optin((const void*)k_tree_local, TREE_DYN_SMEM));
-        k_tree_local<<<grid, GS_THREADS, TREE_DYN_SMEM, st>>>(A);
+        // the local stage's CTAs draw work items from queues: as many CTAs as there can be items
+        i64 lgrid = (N + A.quantum - 1) / A.quantum + N / (A.quantum + 1) + 1;
+        const int lmax = persistent_ctas() < MAX_GRID ? persistent_ctas() : MAX_GRID;
+        if (lgrid > lmax) lgrid = lmax;
+        k_tree_local<<<(unsigned)lgrid, GS_THREADS, TREE_DYN_SMEM, st>>>(A);
         PEEK_CUDA(cudaGetLastError());
     }
     if (want_signals)
