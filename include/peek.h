@@ -289,8 +289,8 @@ peek_status peek_offline_phase1(const uint64_t* hashes, const int64_t* blk_off, 
 /* ---- options: tuning and test hooks ------------------------------------------------------- */
 /* Process-wide, not thread-safe against concurrent calls; results never depend on them.
  * PEEK_OPT_LPM_STRATEGY  how peek_lpm co-descends when a tree view is given:
- *     PEEK_LPM_AUTO (default)  dual-walk for N >= 32768, speculative below; queues of at most 2048
- *                              requests take one launch of per-request walks (both modes)
+ *     PEEK_LPM_AUTO (default)  dual-walk; queues of at most 2048 requests take one launch of
+ *                              per-request walks (both modes)
  *     PEEK_LPM_DUAL_WALK       a warp walks a run of sorted positions in order, carrying the
  *                              predecessor's hit and cache path (Alg. 1's co-descent)
  *     PEEK_LPM_SPECULATIVE     every position walks in parallel from its shared depth, a scan

@@ -794,7 +794,7 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
     const unsigned warps_grid = (unsigned)((N * 32 + LPM_THREADS - 1) / LPM_THREADS);
     // co-descent strategy: sequential dual-walk needs many runs to fill the machine
     const bool dual = tree && (g_lpm_strategy == PEEK_LPM_DUAL_WALK ||
-                               (g_lpm_strategy == PEEK_LPM_AUTO && N >= 32768));
+                               g_lpm_strategy == PEEK_LPM_AUTO);  // (queues of <= LPM_SMALL_MAX requests took the one-launch path above)
     const bool spec = tree && !dual;
     // sorted positions per dual-walk window: enough windows to fill the machine (~8K warps), at
     // most 32 positions (a run head pays a full walk from the root)
