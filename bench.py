@@ -591,7 +591,10 @@ def run_reference(args):
         return
     import oracle
     wl, cache = cpu_inputs(args.config, args.seed, args.small)
-    n = size_sample(wl, cache, args.cpu_seconds)  # the same sample rule as the cpu_baseline leg
+    # the same sample rule as the cpu_baseline leg (size_sample); the per-pass budget shrinks with the
+    # number of passes so that warm-up + timed steps end within a few minutes
+    budget = min(args.cpu_seconds, 150.0 / max(args.steps + args.warmup, 1))
+    n = size_sample(wl, cache, budget)
     for _ in range(args.warmup):
         oracle_pass(wl, cache, n)
     t = 0.0
