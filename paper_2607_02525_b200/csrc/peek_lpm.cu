@@ -8,8 +8,10 @@
 // consecutive blocks probed per step in the open-addressed table, first miss wins.
 //
 // Without a peek_tree_view every request walks on its own (k_lpm_radix / k_lpm_hash, one warp per
-// request).  With it the calls co-descend over the sorted order: k_lpm_radix_dual /
-// k_lpm_hash_dual below ("one cache walk per pending edge").
+// request).  With it the call co-descends over the sorted order: k_lpm_dual<RADIX> below
+// ("one cache walk per pending edge"), one persistent kernel per mode.  Queues of
+// at most LPM_SMALL_MAX requests take one launch for both modes (k_lpm_small).  The speculative
+// variant (k_lpm_*_spec + the resolve scan) is kept as an explicit strategy.
 #include <stdlib.h>
 
 #include "peek_common.cuh"

@@ -2,19 +2,22 @@
 // a batch: lexicographic order of the requests' hash chains (= DFS order of the compressed trie),
 // adjacent LCP (= its branching depths), flat groups and per-request clusters.
 //
-// ONE persistent cooperative kernel (one CTA of GS_THREADS per SM), in two stages:
-//   GLOBAL stage - grid-wide partition.  Round 0 sorts the requests by the leading bits of their
-//     first hash word (stable LSD pair sort of peek_sort.cuh); further grid-wide rounds of the
-//     refinement below run only while some unresolved segment is larger than what one CTA can
-//     finish alone (cap_seg positions).
-//   LOCAL stage - every unresolved segment (a run of sorted positions whose chains share a prefix
-//     and are not ordered yet) is finished by ONE CTA out of shared memory: all further refinement
-//     rounds, their sorts and their scans cost CTA barriers instead of grid barriers, and
-//     segments are independent, so the tail of one does not hold up the others.  Work items are
-//     handed out through two atomic queues (big segments first, then fixed quanta of positions
-//     holding the small ones); which CTA takes which item never changes a result.
-//   Queues of at most LOC_CAP requests (the paper's hold 60-200) run in one CTA from
-//   the first step on and see no grid barrier at all.
+// Two stages, three kernels on one stream (k_tree_global -> k_tree_local -> k_tree_signals):
+//   GLOBAL stage (cooperative, one CTA of GS_THREADS per SM) - grid-wide partition.  Round 0 sorts the
+//     requests by the leading bits of their first hash word (stable LSD pair sort of
+//     peek_sort.cuh); further grid-wide rounds of the refinement below run only while some
+//     unresolved segment is larger than what one CTA should finish alone (cap_seg positions).
+//   LOCAL stage (persistent, no CTA waits for another) - every unresolved segment (a run of sorted
+//     positions whose chains share a prefix and are not ordered yet) is finished by ONE CTA out of
+//     shared memory: all further refinement rounds, their sorts and their scans cost CTA barriers
+//     instead of grid barriers, and segments are independent, so the tail of one does not hold up
+//     the others.  Work items are handed out through two atomic queues (the segments above the
+//     quantum first, then fixed quanta of positions holding the small ones); which CTA takes
+//     which item never changes a result.  A work item occupies one SM, so cap_seg and the quantum
+//     scale with the queue (tree_launch): mid-size queues get enough items to fill the GPU.
+//   SIGNALS (cooperative) - groups and clusters from (order, lcp).
+//   Queues of at most TREE_SMALL_MAX requests (the paper's hold 60-200) run in one CTA
+//   and one launch from the first step on (k_tree_small) and see no grid barrier at all.
 //
 // Refinement = path peeling.  Every unresolved segment picks its LONGEST chain as head h.  A member
 // r is classified by its LCP with h in units of w-bit digits (a 64-bit hash word = D digits, most
