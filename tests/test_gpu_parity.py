@@ -412,6 +412,41 @@ def test_sharded_queue_emulated(cfg, G):
     assert len(np.unique(_np(res.owner))) > 1 or cfg == 3
 
 
+def test_pending_tree_scale_shapes():
+    """peek_pending_tree at the sizes where its launch plan changes (one CTA up to 2048 requests, item
+    capacity and quantum growing with the queue, full capacity from ~90 000 on) and on shapes that
+    stress each stage: deep tries (several grid-wide rounds), a few giant clusters (segments far above
+    the local capacity), 250 000 requests over 200 distinct chains (huge resolved segments), and a
+    multi-turn queue (conversations whose turns are prefixes of one another under shared prompts)."""
+    b = _b()
+    rng = np.random.default_rng(7)
+    for n in (2048, 2049, 11265, 90113):
+        reqs, _ = _nested_queue(rng, n)
+        _tree_only(b, reqs)
+    bases = [rng.integers(0, 50000, size=int(rng.integers(200, 3000))).astype(np.int32) for _ in range(5)]
+    reqs = []
+    for _ in range(70000):
+        k = int(rng.integers(0, 8))
+        if k < 5:
+            bse = bases[k]
+            reqs.append(np.concatenate([bse[: int(rng.integers(len(bse) // 2, len(bse) + 1))],
+                                        rng.integers(0, 50000, size=int(rng.integers(0, 100))).astype(np.int32)]))
+        else:
+            reqs.append(rng.integers(0, 50000, size=int(rng.integers(0, 300))).astype(np.int32))
+    _tree_only(b, reqs)
+    pool = [rng.integers(0, 1000, size=int(rng.integers(0, 400))).astype(np.int32) for _ in range(200)]
+    _tree_only(b, [pool[int(i)] for i in rng.integers(0, 200, size=250000)])
+    prompts = [rng.integers(0, 128256, size=1024).astype(np.int32) for _ in range(12)]
+    reqs = []
+    for c in range(3000):
+        ctx = prompts[int(rng.integers(0, 12))]
+        for t in range(int(rng.integers(1, 24))):
+            ctx = np.concatenate([ctx, rng.integers(0, 128256, size=int(rng.integers(64, 512))).astype(np.int32)])
+            reqs.append(ctx)
+    perm = rng.permutation(len(reqs))
+    _tree_only(b, [reqs[i] for i in perm])
+
+
 def test_rank_two_phase_wide_keys():
     """cLPM keys too wide for one 64-bit packed key (full-range hit, cluster size and arrival):
     the arrival sort followed by the stable (hit, cluster size) sort."""
