@@ -105,21 +105,26 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_nb_apply(const i64* __restrict
 //      staged in shared memory by ONE 1-D bulk TMA copy (cp.async.bulk + mbarrier, HF_STAGES deep
 //      ring per warp), then lane j computes block j of the chunk on its own: 16 multiply-adds from
 //      four conflict-free 128-bit shared loads, no cross-lane reduction; c = mix64(S) goes to the
-//      warp's c-buffer in shared memory
-//   B  every lane runs the serial chain k = mix64(k ^ c) over ITS request's chunk (32 requests per
-//      warp in parallel - the chain is inherently serial per request, so lanes = requests)
+//      warp's c-buffer in shared memory.  The loop is unrolled over the ring (stage addresses,
+//      barriers and parities are static) and a chunk's mix64 runs one trip late, inside the next
+//      chunk's multiply-adds, where its dependent chain costs no stalls
+//   B  every owning lane runs the serial chain k = mix64(k ^ c) over ITS request's chunk (the chain
+//      is inherently serial per request, so lanes = requests)
 //   C  the chunk's k values are written to `hashes` with coalesced 256-byte stores
 // so tokens are read from HBM once and only the final hashes are written: 4T + 8NB bytes.
+// HF_LANES requests per warp: the c-buffer (HF_LANES x 32 values) and the ring share the warp's
+// slice of shared memory, and 20 warps x 16 requests beat 15 x 32 (more copies in flight; the chain
+// phase runs half empty, but phase A is 70 % of the instructions).
 //
 // Alignment: a request starts at an arbitrary token, so a chunk starts `a` = 0..3 words past a
 // 16-byte boundary.  The copy fetches the 16-byte aligned superset; row j = staged bytes
-// [64j, 64j+64).  Block j is words a..15 of row j plus words 0..a-1 of row j+1; lane j computes
-// both parts of ITS row (U_j for block j, Q_j for block j-1) with the multipliers rotated by a,
-// and S_j = U_j + Q_{j+1} takes one shuffle.
+// [64j, 64j+64).  Block j is words a..15 of row j plus words 0..a-1 of row j+1: lane j also loads
+// the first vector of row j+1, which stands in for the first a words of its own row, and the
+// multipliers are rotated by a (block_sum<a>).
 // Bank conflicts: rows are 64 bytes apart, so lane j reads its four 16-byte vectors in the rotated
 // order (c + (j>>1)) & 3 and keeps its multipliers pre-rotated the same way (M[c][e] below).
 #ifndef PEEK_HF_WARPS
-#define PEEK_HF_WARPS 15
+#define PEEK_HF_WARPS 20
 #endif
 #ifndef PEEK_HF_STAGES
 #define PEEK_HF_STAGES 3
@@ -130,7 +135,7 @@ static constexpr int HF_STAGES = PEEK_HF_STAGES;
 static constexpr int HF_STAGE_BYTES = 2176;          // 2048 + 16 rounded up to a multiple of 128
 static constexpr int HF_CROW = 33;                   // c-buffer row pitch in u64 (32 + 1: no conflicts)
 #ifndef PEEK_HF_LANES
-#define PEEK_HF_LANES 32
+#define PEEK_HF_LANES 16
 #endif
 static constexpr int HF_LANES = PEEK_HF_LANES;       // owning lanes (requests) per warp = c-buffer rows
 static constexpr int HF_WARP_BYTES = HF_STAGES * HF_STAGE_BYTES + HF_LANES * HF_CROW * 8 + 64;
@@ -164,58 +169,35 @@ __device__ __forceinline__ uint4 lds128(u32 addr) {
     return v;
 }
 
-// Sum over this lane's 64-byte row with the multipliers rotated by A words: returns U (the part
-// of block j) and *qown (the part of block j-1: the first A words of the row).  V[c] is the row's
-// physical vector (c + x) & 3, M[c][e] = pos_mult(4 * ((c + x) & 3) + e), c0 = (4 - x) & 3 is the
-// register that holds physical vector 0.
+// Content sum (without SUM_M) of block `lane` of a staged chunk whose first token sits A words past a
+// 16-byte boundary.  V[c] is physical vector (c + x) & 3 of row `lane`, M[c][e] = pos_mult(4 * ((c + x) & 3)
+// + e).  The block is words A..15 of the row followed by words 0..A-1 of the NEXT row: X (vector 0 of
+// row lane + 1) stands in for the first A words of this row's physical vector 0, which V[c0] holds.
+// The previous chunk's mix64 rides in the same basic block so that its dependent chain fills the
+// multiply-add latencies.
 template <int A>
-__device__ __forceinline__ u64 row_sum(const uint4 (&V)[4], const u64 (&M)[4][4], int c0, u64* qown) {
+__device__ __forceinline__ u64 block_sum(const uint4 (&V)[4], u32 xaddr, const u64 (&M)[4][4], int c0,
+                                         u64 Uprev, u64* cprev) {
+    u32 xw[4] = {0, 0, 0, 0};
+    if (A > 0) {
+        const uint4 X = lds128(xaddr);
+        xw[0] = X.x; xw[1] = X.y; xw[2] = X.z; xw[3] = X.w;
+    }
     u64 acc0 = 0, acc1 = 0;
-    u64 W[4] = {0, 0, 0, 0};
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
         const u32 w[4] = {V[c].x, V[c].y, V[c].z, V[c].w};
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            if (e >= A) {
-                if (e & 1) acc1 += (u64)w[e] * M[c][e - A];
-                else acc0 += (u64)w[e] * M[c][e - A];
-            } else {
-                W[c] += (u64)w[e] * M[(c + 3) & 3][4 + e - A];
-            }
+            u64 p;
+            if (e >= A) p = (u64)w[e] * M[c][e - A];
+            else p = (u64)(c == c0 ? xw[e] : w[e]) * M[(c + 3) & 3][4 + e - A];
+            if (e & 1) acc1 += p;
+            else acc0 += p;
         }
     }
-    u64 tot = acc0 + acc1;
-    if (A > 0) {
-        u64 q = c0 == 0 ? W[0] : (c0 == 1 ? W[1] : (c0 == 2 ? W[2] : W[3]));
-        tot += (W[0] + W[1]) + (W[2] + W[3]) - q;
-        *qown = q;
-    } else {
-        *qown = 0;
-    }
-    return tot;
-}
-
-// S - SUM_M of block `lane` of the staged chunk: own row's part plus the next row's first A words.
-template <int A>
-__device__ __forceinline__ u64 block_sum(const uint4 (&V)[4], const u64 (&M)[4][4], int c0, u32 sbase,
-                                         int lane, int n) {
-    u64 qown;
-    u64 U = row_sum<A>(V, M, c0, &qown);
-    if (A > 0) {
-        u64 qn = __shfl_down_sync(0xffffffffu, qown, 1);
-        if (lane == 31 && n == 32) {
-            // row 32 belongs to no lane: its first A words carry positions 16-A..15, which for
-            // lane 31 (x = 3) are M[0][4-A..3]
-            uint4 X = lds128(sbase + 2048u);
-            const u32 w[4] = {X.x, X.y, X.z, X.w};
-            qn = 0;
-#pragma unroll
-            for (int e = 0; e < A; ++e) qn += (u64)w[e] * M[0][4 - A + e];
-        }
-        U += qn;
-    }
-    return U;
+    *cprev = mix64(Uprev + SUM_M);
+    return acc0 + acc1;
 }
 
 struct HashArgs {
@@ -271,21 +253,24 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
     const char* c_src = nullptr;
     u32 c_bytes = 0, c_meta = 0;
     unsigned im = 0, cm = 0;  // lanes whose chunk is still to be issued / consumed
-    u32 parity = 0;           // bit s = parity to wait for on stage s
-    int sI = 0, sC = 0;
+    u32 par[HF_STAGES];       // parity to wait for on each stage
+#pragma unroll
+    for (int s = 0; s < HF_STAGES; ++s) par[s] = 0;
+    const u32 xoff = 64u * lane + 64u;
 
-    auto issue = [&]() {  // next chunk of `im` -> stage sI: the owning lane issues its own copy
+    // next chunk of `im` -> stage S (static): the owning lane issues its own copy
+    auto issue = [&](const int S) {
         const int q = __ffs(im) - 1;
         im &= im - 1;
         if (lane == q) {
-            const u32 bar = bar0 + 8 * sI;
+            const u32 bar = bar0 + 8 * S;
             mbar_expect_tx(bar, c_bytes);
-            if (c_bytes) tma_load_1d(stage0 + sI * HF_STAGE_BYTES, (const void*)c_src, c_bytes, bar);
+            if (c_bytes) tma_load_1d(stage0 + S * HF_STAGE_BYTES, (const void*)c_src, c_bytes, bar);
         }
-        sI = sI + 1 == HF_STAGES ? 0 : sI + 1;
     };
     // Take requests for the lanes that have none, describe every owning lane's next chunk and put
-    // the first HF_STAGES - 1 copies of the round in flight.  Returns false when nothing is left.
+    // the first HF_STAGES - 1 copies of the round in flight (every round starts at stage 0: all
+    // stages are drained when phase A ends).  Returns false when nothing is left.
     auto next_round = [&]() -> bool {
         bool need = !own && lane < A.lanes_cap && !exhausted;
         for (;;) {
@@ -329,44 +314,52 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
         im = cm = active;
 #pragma unroll
         for (int s = 0; s < HF_STAGES - 1; ++s)
-            if (im) issue();
+            if (im) issue(s);
         return true;
     };
 
     bool more = next_round();
     while (more) {
-        // ---- phase A: one thread per block of each staged chunk ----
+        // ---- phase A: one thread per block of each staged chunk; the loop is unrolled over the
+        //      ring so that stage addresses, barriers and parities are static ----
+        u64 Uprev = 0;
+        u64* cprev = cbuf + 32;  // first trip: the pad slot of row 0
         while (cm) {
-            if (im) issue();
-            const int q = __ffs(cm) - 1;
-            cm &= cm - 1;
-            const u32 meta = __shfl_sync(FULL, c_meta, q);
-            const int n = meta & 0xff, a = (meta >> 8) & 3;
-            const u32 sbase = stage0 + sC * HF_STAGE_BYTES;
-            mbar_wait(bar0 + 8 * sC, (parity >> sC) & 1u);
-            parity ^= 1u << sC;
-            sC = sC + 1 == HF_STAGES ? 0 : sC + 1;
-            if (meta >> 16) {  // last words of the pool, past its last 16-byte boundary: by hand
-                const u32 src_lo = __shfl_sync(FULL, (u32)(uintptr_t)c_src, q);
-                if (lane < (int)(meta >> 16)) {
-                    const u32 v = *(const u32*)(pool_end16 + 4 * lane);
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(sbase + ((u32)(uintptr_t)pool_end16 - src_lo) + 4u * lane), "r"(v) : "memory");
-                }
-                __syncwarp();
-            }
-            uint4 V[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) V[c] = lds128(sbase + voff[c]);
-            u64 U;
-            switch (a) {
-                case 0: U = block_sum<0>(V, M, c0, sbase, lane, n); break;
-                case 1: U = block_sum<1>(V, M, c0, sbase, lane, n); break;
-                case 2: U = block_sum<2>(V, M, c0, sbase, lane, n); break;
-                default: U = block_sum<3>(V, M, c0, sbase, lane, n); break;
+            for (int S = 0; S < HF_STAGES; ++S) {
+                if (!cm) break;
+                if (im) issue((S + HF_STAGES - 1) % HF_STAGES);
+                const int q = __ffs(cm) - 1;
+                cm &= cm - 1;
+                const u32 meta = __shfl_sync(FULL, c_meta, q);
+                const int a = (meta >> 8) & 3;
+                const u32 sbase = stage0 + S * HF_STAGE_BYTES;
+                mbar_wait(bar0 + 8 * S, par[S]);
+                par[S] ^= 1u;
+                if (meta >> 16) {  // last words of the pool, past its last 16-byte boundary: by hand
+                    const u32 src_lo = __shfl_sync(FULL, (u32)(uintptr_t)c_src, q);
+                    if (lane < (int)(meta >> 16)) {
+                        const u32 v = *(const u32*)(pool_end16 + 4 * lane);
+                        asm volatile("st.shared.u32 [%0], %1;" ::"r"(sbase + ((u32)(uintptr_t)pool_end16 - src_lo) + 4u * lane), "r"(v) : "memory");
+                    }
+                    __syncwarp();
+                }
+                uint4 V[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) V[c] = lds128(sbase + voff[c]);
+                u64 U;
+                switch (a) {
+                    case 0: U = block_sum<0>(V, sbase + xoff, M, c0, Uprev, cprev); break;
+                    case 1: U = block_sum<1>(V, sbase + xoff, M, c0, Uprev, cprev); break;
+                    case 2: U = block_sum<2>(V, sbase + xoff, M, c0, Uprev, cprev); break;
+                    default: U = block_sum<3>(V, sbase + xoff, M, c0, Uprev, cprev); break;
+                }
+                Uprev = U;
+                cprev = cbuf + q * HF_CROW + lane;
+                __syncwarp();  // the stage is fully read before it is refilled
             }
-            if (lane < n) cbuf[q * HF_CROW + lane] = mix64(U + SUM_M);
-            __syncwarp();  // the stage is fully read before it is refilled; cbuf row visible
         }
+        *cprev = mix64(Uprev + SUM_M);
 
         // ---- advance, and put the next round's first copies in flight before the chain ----
         const i32 nB = (i32)(c_meta & 0xff);  // this round: chain steps of this lane, output position
@@ -378,6 +371,7 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
             if (pos == nb) { own = false; fresh = true; }
         }
         more = next_round();
+        __syncwarp();  // c-buffer rows visible
 
         // ---- phase B: serial chain, lane = request ----
         const i32 nmax = __reduce_max_sync(FULL, nB);
