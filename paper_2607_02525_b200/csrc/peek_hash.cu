@@ -328,7 +328,7 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
 #pragma unroll
             for (int S = 0; S < HF_STAGES; ++S) {
                 if (!cm) break;
-                if (im) issue((S + HF_STAGES - 1) % HF_STAGES);
+                issue((S + HF_STAGES - 1) % HF_STAGES);  // no chunk left: no lane matches
                 const int q = __ffs(cm) - 1;
                 cm &= cm - 1;
                 const u32 meta = __shfl_sync(FULL, c_meta, q);
@@ -374,16 +374,25 @@ __global__ void __launch_bounds__(HF_THREADS, 1) k_block_hash_fused(HashArgs A) 
         __syncwarp();  // c-buffer rows visible
 
         // ---- phase B: serial chain, lane = request ----
+        // steps every owner has run unguarded (lanes without a request chain row 0 and store nothing)
+        const bool ownr = (done >> lane) & 1u;
         const i32 nmax = __reduce_max_sync(FULL, nB);
-        u64* crow = cbuf + lane * HF_CROW;
-        for (i32 s = 0; s < nmax; ++s) {
+        const i32 nmin = __reduce_min_sync(FULL, ownr ? nB : 32);
+        u64* crow = cbuf + (ownr ? lane : 0) * HF_CROW;
+        i32 s = 0;
+        for (; s < nmin; ++s) {
+            k = mix64(k ^ crow[s]);
+            if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1;
+            if (ownr) crow[s] = k;
+        }
+        for (; s < nmax; ++s) {
             if (s < nB) {
                 k = mix64(k ^ crow[s]);
                 if (k == PEEK_EMPTY) k = PEEK_EMPTY - 1;
                 crow[s] = k;
             }
         }
-        if (fresh) k = A.seed;
+        if (fresh || !ownr) k = A.seed;
         __syncwarp();
 
         // ---- phase C: coalesced stores of the round's hashes ----
