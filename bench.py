@@ -35,7 +35,7 @@ UNIT = "queries/s"
 CONFIG_NAMES = {1: "configs[0] tiny_shared_prompt_chat", 2: "configs[1] shared_prompt_chat_at_scale",
                 3: "configs[2] long_prefix_rag", 4: "configs[3] singleton_chat_table_only",
                 5: "configs[4] agentic_multi_turn_at_scale"}
-PAIR_SLOTS = ("tree.persistent", "lpm.radix_walk", "lpm.hash_probe")  # north_star: peek_pending_tree + peek_lpm
+PAIR_SLOTS = ("tree.persistent", "lpm.radix_walk", "lpm.hash_probe", "lpm.dual_walk")  # north_star: peek_pending_tree + peek_lpm
 
 
 def log(*a):
@@ -239,6 +239,8 @@ def algorithmic_bytes(inp, out: dict) -> dict:
         else:
             hb = int(torch.clamp(hs // 16 - lcp, min=0).sum().item())
             res[name] = 40 * (hb + R) + 16 * N
+    if "lpm.radix" in res and "lpm.hash" in res:  # both modes side by side (one profile slot)
+        res["lpm.both"] = res["lpm.radix"] + res["lpm.hash"]
     dplus = int((out["demand"] > 0).sum().item()) if out["demand"] is not None else 0
     res["demand"] = 40 * U + 32 * dplus + 4 * S
     res["rank"] = 208 * N
@@ -246,7 +248,8 @@ def algorithmic_bytes(inp, out: dict) -> dict:
 
 
 SLOT_TO_CALL = {"hash.nb_scan": "hash.nb_scan", "hash.content": "hash", "tree.persistent": "tree",
-                "lpm.radix_walk": "lpm.radix", "lpm.hash_probe": "lpm.hash", "lpm.resolve_scan": None,
+                "lpm.radix_walk": "lpm.radix", "lpm.hash_probe": "lpm.hash", "lpm.dual_walk": "lpm.both",
+                "lpm.resolve_scan": None,
                 "demand.count": "demand", "rank.clpm_sort": "rank"}
 
 
@@ -447,7 +450,7 @@ def measured_peak():
 def kernel_source_sha(slot: str):
     """sha256 (first 12 hex digits) of the source file of the slot's kernel: stamps an ncu capture."""
     files = {"hash.content": "peek_hash.cu", "tree.persistent": "peek_tree.cu", "lpm.radix_walk": "peek_lpm.cu",
-             "lpm.hash_probe": "peek_lpm.cu"}
+             "lpm.hash_probe": "peek_lpm.cu", "lpm.dual_walk": "peek_lpm.cu"}
     f = files.get(slot)
     if not f:
         return None
@@ -782,7 +785,7 @@ def run_peek(args):
     calls = calls_table(inp, prof, out, args.steps, t_ms)
     ceil = gather_ceiling(inp, dev)
     if "hbm" in ceil:
-        for slot in ("lpm.radix_walk", "lpm.hash_probe", "demand.count"):
+        for slot in ("lpm.radix_walk", "lpm.hash_probe", "lpm.dual_walk", "demand.count"):
             if slot in calls and "alg_GBps" in calls[slot]:
                 calls[slot]["frac_of_random_sector_ceiling"] = calls[slot]["alg_GBps"] / ceil["hbm"]["GBps"]
     dom = max(calls, key=lambda s: calls[s]["ms_per_step"])

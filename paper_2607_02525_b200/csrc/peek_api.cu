@@ -44,6 +44,48 @@ cudaError_t func_smem_optin(const void* func, int bytes) {
     return e;
 }
 
+static std::mutex g_side_mu;
+bool side_fork(cudaStream_t st, SideStream* ss) {
+    struct PerDev { int dev; SideStream s; };
+    static std::vector<PerDev> made;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        return false;
+    }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    g_side_mu.lock();
+    const SideStream* found = nullptr;
+    for (const PerDev& d : made)
+        if (d.dev == dev) found = &d.s;
+    if (!found) {
+        SideStream n{};
+        if (cudaStreamCreateWithFlags(&n.side, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&n.fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&n.join, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            g_side_mu.unlock();
+            return false;
+        }
+        made.push_back(PerDev{dev, n});
+        found = &made.back().s;
+    }
+    *ss = *found;
+    if (cudaEventRecord(ss->fork, st) != cudaSuccess || cudaStreamWaitEvent(ss->side, ss->fork, 0) != cudaSuccess) {
+        cudaGetLastError();
+        g_side_mu.unlock();
+        return false;
+    }
+    return true;  // side_join unlocks
+}
+cudaError_t side_join(cudaStream_t st, const SideStream& ss) {
+    cudaError_t e = cudaEventRecord(ss.join, ss.side);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ss.join, 0);
+    g_side_mu.unlock();
+    return e;
+}
+
 int sm_count() {
     int dev = 0, n = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 148;

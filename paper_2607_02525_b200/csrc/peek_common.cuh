@@ -23,6 +23,14 @@ int persistent_ctas();  // grid of the persistent cooperative kernels (PEEK_OPT_
 // opt `func` in to `bytes` of dynamic shared memory on the CURRENT device (the attribute belongs to the
 // device's context, so it is remembered per device; thread-safe)
 cudaError_t func_smem_optin(const void* func, int bytes);
+// A library-owned side stream per device for calls that run two independent kernels side by side
+// (fork: `side` waits for `fork` recorded on the caller's stream; join: the caller's stream waits
+// for `join` recorded on `side`).  side_fork returns false when the call must stay on one stream
+// (a stream under capture, or no side stream could be made); on true it
+// holds side_mutex() until side_join, so two host threads never interleave their record/wait pairs.
+struct SideStream { cudaStream_t side; cudaEvent_t fork, join; };
+bool side_fork(cudaStream_t st, SideStream* ss);
+cudaError_t side_join(cudaStream_t st, const SideStream& ss);
 
 // tracing slots (peek_profile_*)
 enum ProfSlot {

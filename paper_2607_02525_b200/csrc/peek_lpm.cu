@@ -844,16 +844,29 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
         i64 ctas = (items + DW_WARPS - 1) / DW_WARPS;
         const i64 cap = (i64)sm_count() * PEEK_DW_CAP;  // resident CTAs per SM - the warps loop over the items
         if (ctas > cap) ctas = cap;
-        if (hit_radix) {
-            Prof pr(PROF_LPM_RADIX, st, radix->E > 0 ? 2 : 1);
+        // both modes: the two walks are independent, so the hash probes run on the library's side
+        // stream next to the radix walk (each is bound by dependent trips, not by the machine)
+        SideStream ss;
+        if (hit_radix && hit_hash && side_fork(st, &ss)) {
+            Prof pr(PROF_LPM_DUAL, st, radix->E > 0 ? 3 : 2);
+            D.ctr = ctr + 32;
+            k_lpm_dual<false><<<(unsigned)ctas, DW_THREADS, 0, ss.side>>>(D);
             if (radix->E > 0) k_lpm_prep<<<(unsigned)((radix->E + 255) / 256), 256, 0, st>>>(R, radix->E, info);
             D.ctr = ctr;
             k_lpm_dual<true><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
-        }
-        if (hit_hash) {
-            Prof pr(PROF_LPM_HASH, st, 1);
-            D.ctr = ctr + 32;
-            k_lpm_dual<false><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
+            PEEK_CUDA(side_join(st, ss));
+        } else {
+            if (hit_radix) {
+                Prof pr(PROF_LPM_RADIX, st, radix->E > 0 ? 2 : 1);
+                if (radix->E > 0) k_lpm_prep<<<(unsigned)((radix->E + 255) / 256), 256, 0, st>>>(R, radix->E, info);
+                D.ctr = ctr;
+                k_lpm_dual<true><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
+            }
+            if (hit_hash) {
+                Prof pr(PROF_LPM_HASH, st, 1);
+                D.ctr = ctr + 32;
+                k_lpm_dual<false><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
+            }
         }
     } else {
         if (hit_radix) {

@@ -387,6 +387,45 @@ def test_lpm_work_counters():
     assert dual[2] * 3 < naive[2] and dual[3] * 2 < naive[3]
 
 
+def test_lpm_both_modes_side_stream():
+    """peek_lpm with both modes and a tree view runs the hash probes on the library's side stream
+    next to the radix walk (fork/join around the caller's stream).  Same hits as the oracle on the
+    default stream, on a user stream, back to back, and under CUDA-graph capture (where the call must
+    stay on the capturing stream)."""
+    b = _b()
+    wl = W.make(5, seed=77, small=True)
+    toks, off = wl.queue.materialize_np()
+    cache = W.build_cache(wl, lambda t, o: oracle.block_hash(t, o, 16, 0))
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    o_hr = oracle.lpm_radix(toks, off, _orc_radix(cache.radix))
+    o_hh = oracle.lpm_hash(o_h, o_bo, cache.t_keys)
+    d_tok, d_off, d_h, d_bo = _dev(toks), _dev(off), _dev(o_h.view(np.int64), torch.uint64), _dev(o_bo)
+    d_radix, d_keys = _radix_dev(cache.radix), _dev(cache.t_keys.view(np.int64), torch.uint64)
+    tree = b.peek_pending_tree(d_h, d_bo)
+    call = lambda: b.peek_lpm(d_tok, d_off, d_h, d_bo, radix=d_radix, t_keys=d_keys, tree=tree)
+    b.set_option(b.OPT_LPM_STRATEGY, b.LPM_DUAL_WALK)  # the small case would take the one-launch path
+    try:
+        for _ in range(3):
+            hr, hh = call()
+            assert np.array_equal(_np(hr), o_hr) and np.array_equal(_np(hh), o_hh)
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            outs = [call() for _ in range(4)]
+        side.synchronize()
+        for hr, hh in outs:
+            assert np.array_equal(_np(hr), o_hr) and np.array_equal(_np(hh), o_hh)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            ghr, ghh = call()
+        ghr.zero_(); ghh.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(_np(ghr), o_hr) and np.array_equal(_np(ghh), o_hh)
+    finally:
+        b.set_option(b.OPT_LPM_STRATEGY, b.LPM_AUTO)
+
+
 @pytest.mark.parametrize("cfg,G", [(2, 2), (5, 3), (4, 4)])
 def test_sharded_queue_emulated(cfg, G):
     """SURVEY.md section 8(e) through the CUDA calls: the G shards of one queue (by first-block hash) run
