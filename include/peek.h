@@ -106,6 +106,21 @@ peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok_off, int64
                             int32_t block_size, uint64_t seed, int64_t* blk_off, uint64_t* hashes,
                             int64_t hashes_capacity, void* ws, int64_t ws_bytes, void* stream);
 
+/* The same operation for callers that cannot allocate device memory (code under CUDA-graph capture,
+ * serving loops and harnesses that forbid cudaMalloc): no `ws` - the scratch is a 32 KB file-scope
+ * `static __device__` array inside the library, which every GPU that loads the library holds until
+ * the process exits.  Arguments, layouts, outputs and error behaviour are those of peek_block_hash;
+ * in addition N > PEEK_BLOCK_HASH_STATIC_MAX_N is rejected with PEEK_ERR_CAPACITY (nothing is
+ * touched).  The call makes no cudaMalloc / cudaFree and no allocating library call.  ALL calls on
+ * a device share the one array: two calls that overlap on the GPU (different streams, or two host
+ * threads on different streams) race and corrupt each other - serialise them on one stream or use
+ * peek_block_hash with separate workspaces.  The array keeps the last call's contents; the kernels
+ * rewrite everything they read from it, so nothing has to be cleared between calls. */
+#define PEEK_BLOCK_HASH_STATIC_MAX_N 4194304
+peek_status peek_block_hash_static(const int32_t* tokens, const int64_t* tok_off, int64_t N,
+                                   int32_t block_size, uint64_t seed, int64_t* blk_off,
+                                   uint64_t* hashes, int64_t hashes_capacity, void* stream);
+
 /* ---- the engine's prefix cache, read-only --------------------------------- */
 /* Radix cache flattened to arrays.  Node 0 is the root (empty label).  Node u's label is
  * c_tokens[n_tok_off[u] .. + n_tok_len[u]).  The children of node v are edges

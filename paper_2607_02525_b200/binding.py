@@ -24,7 +24,7 @@ CALL_PENDING_TREE_UPDATE = 8
 EXPORTS = ["peek_status_string", "peek_last_error", "peek_version", "peek_workspace_bytes",
            "peek_profile_enable", "peek_profile_slots", "peek_profile_name", "peek_profile_read",
            "peek_launch_count", "peek_set_option", "peek_lpm_counters",
-           "peek_block_hash", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
+           "peek_block_hash", "peek_block_hash_static", "peek_lpm", "peek_pending_tree", "peek_demand_rank",
            "peek_clpm_signals", "peek_clpm_order_full", "peek_clpm_group_major", "peek_offline_phase1", "peek_radix_demand",
            "peek_clpm_lane_b", "peek_dynamic_lane", "peek_pending_tree_update",
            "peek_stride_interleave"]
@@ -69,6 +69,8 @@ def lib():
         L.peek_set_option.argtypes = [i32, i64]
         L.peek_block_hash.restype = i32
         L.peek_block_hash.argtypes = [vp, vp, i64, i32, u64, vp, vp, i64, vp, i64, vp]
+        L.peek_block_hash_static.restype = i32
+        L.peek_block_hash_static.argtypes = [vp, vp, i64, i32, u64, vp, vp, i64, vp]
         L.peek_lpm.restype = i32
         L.peek_lpm.argtypes = [vp, vp, vp, vp, i64, i32, ctypes.POINTER(_Radix), ctypes.POINTER(_Table),
                                ctypes.POINTER(_TreeView), vp, vp, vp, i64, vp]
@@ -213,6 +215,22 @@ def peek_block_hash(tokens: torch.Tensor, tok_off: torch.Tensor, NB: int, block_
                                _ptr(tok_off, torch.int64), N, block_size, ctypes.c_uint64(seed),
                                _ptr(blk_off, torch.int64), _ptr(hashes, U64), NB, _ptr(ws), nbytes, _stream())
     _check(st, "peek_block_hash")
+    return blk_off, hashes[:NB]
+
+
+BLOCK_HASH_STATIC_MAX_N = 4194304  # include/peek.h PEEK_BLOCK_HASH_STATIC_MAX_N
+
+
+def peek_block_hash_static(tokens: torch.Tensor, tok_off: torch.Tensor, NB: int, blk_off: torch.Tensor,
+                           hashes: torch.Tensor, block_size: int = 16, seed: int = 0):
+    """peek_block_hash without a workspace: the scratch is a static device array inside the library
+    (at most BLOCK_HASH_STATIC_MAX_N requests; calls that overlap on the GPU race).  Nothing is
+    allocated here either: the caller passes both outputs.  Returns (blk_off, hashes[:NB])."""
+    N = int(tok_off.shape[0]) - 1
+    st = lib().peek_block_hash_static(_ptr(tokens, torch.int32) if tokens.numel() else None,
+                                      _ptr(tok_off, torch.int64), N, block_size, ctypes.c_uint64(seed),
+                                      _ptr(blk_off, torch.int64), _ptr(hashes, U64), NB, _stream())
+    _check(st, "peek_block_hash_static")
     return blk_off, hashes[:NB]
 
 

@@ -4,6 +4,8 @@
 //   nb_scan   blk_off = exclusive prefix sum of floor(len_r / B)                 (3 small launches)
 //   fused     k_block_hash_fused: tokens -> per-block sums -> chained hashes in ONE pass over HBM
 //             (1-D bulk TMA staging, thread-per-block sums, lane-per-request chain; see below)
+#include <mutex>
+
 #include "peek_common.cuh"
 
 namespace peek {
@@ -472,4 +474,62 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
     }
     PEEK_CUDA(cudaGetLastError());
     return PEEK_OK;
+}
+
+// ---- peek_block_hash_static: the same call, its scratch in a file-scope device array -------------
+// For callers that cannot allocate device memory (CUDA-graph capture, serving loops and harnesses
+// that forbid cudaMalloc).  The scratch of peek_block_hash (the per-chunk partial sums of the block
+// scan and the request counter of k_block_hash_fused) lives in g_hash_static_scratch: every GPU that
+// loads the library holds these 32 KB until the process exits.  In host code the array's name is a
+// host-side stand-in, not a device address, so the address the kernels get comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+static constexpr i64 HASH_STATIC_BYTES = 32 * 1024;
+static __device__ __align__(256) unsigned char g_hash_static_scratch[HASH_STATIC_BYTES];
+
+static peek_status hash_static_scratch(void** out) {
+    static std::mutex mu;
+    static void* known[64];  // by device ordinal; no host allocation either
+    int dev = 0;
+    PEEK_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < 64 && known[dev]) {
+        *out = known[dev];
+        return PEEK_OK;
+    }
+    void* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_hash_static_scratch);
+    if (e != cudaSuccess || !p) return cuda_fail(e, "cudaGetSymbolAddress(g_hash_static_scratch)");
+    if (dev >= 0 && dev < 64) known[dev] = p;
+    *out = p;
+    return PEEK_OK;
+}
+
+extern "C" peek_status peek_block_hash_static(const int32_t* tokens, const int64_t* tok_off, int64_t N,
+                                              int32_t block_size, uint64_t seed, int64_t* blk_off,
+                                              uint64_t* hashes, int64_t hashes_capacity, void* stream) {
+    // host-side checks first (they answer before any CUDA call), in the order of peek_block_hash
+    if (N < 0) { set_error("peek_block_hash_static: N out of range"); return PEEK_ERR_INVALID_ARG; }
+    if (N > PEEK_BLOCK_HASH_STATIC_MAX_N || block_hash_ws_bytes(N) > HASH_STATIC_BYTES) {
+        set_error("peek_block_hash_static: N = %lld exceeds the static scratch (at most %lld requests); "
+                  "use peek_block_hash with a caller-provided workspace",
+                  (long long)N, (long long)PEEK_BLOCK_HASH_STATIC_MAX_N);
+        return PEEK_ERR_CAPACITY;
+    }
+    if (block_size != B16) { set_error("peek_block_hash_static: block_size must be 16"); return PEEK_ERR_UNSUPPORTED; }
+    if (N == 0) return PEEK_OK;
+    if (!tok_off || !blk_off || hashes_capacity < 0 || (hashes_capacity > 0 && (!hashes || !tokens))) {
+        set_error("peek_block_hash_static: NULL argument");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    if ((uintptr_t)tokens & 15) {
+        set_error("peek_block_hash_static: tokens must be 16-byte aligned");
+        return PEEK_ERR_INVALID_ARG;
+    }
+    void* scratch = nullptr;
+    const peek_status s = hash_static_scratch(&scratch);
+    if (s != PEEK_OK) return s;
+    // Nothing in the scratch has to start at zero: the scan kernels write every partial sum they
+    // later read and reset the request counter, so the previous call's contents are harmless.
+    return peek_block_hash(tokens, tok_off, N, block_size, seed, blk_off, hashes, hashes_capacity, scratch,
+                           HASH_STATIC_BYTES, stream);
 }
