@@ -24,6 +24,7 @@ peek_status cuda_fail(cudaError_t e, const char* what) {
 }
 
 static int g_grid_limit = 0;  // PEEK_OPT_GRID_LIMIT
+bool grid_limited() { return g_grid_limit > 0; }  // the test hook is set: small-queue shortcuts stand aside
 int persistent_ctas() {       // CTAs of a persistent cooperative kernel: one per SM unless capped
     int n = sm_count();
     return (g_grid_limit > 0 && g_grid_limit < n) ? g_grid_limit : n;

@@ -22,6 +22,7 @@ int sm_count();  // SMs of the current device (148 on B200)
 int persistent_ctas();  // grid of the persistent cooperative kernels (PEEK_OPT_GRID_LIMIT)
 // opt `func` in to `bytes` of dynamic shared memory on the CURRENT device (the attribute belongs to the
 // device's context, so it is remembered per device; thread-safe)
+bool grid_limited();
 cudaError_t func_smem_optin(const void* func, int bytes);
 // A library-owned side stream per device for calls that run two independent kernels side by side
 // (fork: `side` waits for `fork` recorded on the caller's stream; join: the caller's stream waits

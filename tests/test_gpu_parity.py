@@ -504,6 +504,28 @@ def test_rank_two_phase_wide_keys():
         assert np.array_equal(_np(g_ord), oracle.clpm_order(hit, cs, a))
 
 
+@pytest.mark.parametrize("n", [1, 2, 31, 200, 511, 512, 513])
+def test_rank_small_queue_path(n):
+    """Queues of at most 512 requests rank by counting (one CTA, `k_clpm_rank_small`); 513 takes the sort.
+    Extreme and heavily tied keys, with and without arrival; the grid-limit test hook must give the
+    same order through the general path."""
+    b = _b()
+    rng = np.random.default_rng(900 + n)
+    hit = rng.choice(np.array([-2**31, -1, 0, 16, 160, 2**31 - 1], dtype=np.int64), size=n).astype(np.int32)
+    cs = rng.integers(1, 4, size=n).astype(np.int32)
+    arr = rng.integers(-5, 5, size=n).astype(np.int32)
+    for a in (arr, None):
+        want = oracle.clpm_order(hit, cs, a)
+        for limit in (0, 1):
+            b.set_option(b.OPT_GRID_LIMIT, limit)
+            try:
+                _, g_ord = b.peek_demand_rank(None, None, tree=None, t_keys=None, hit=_dev(hit),
+                                              cluster_size=_dev(cs), arrival=_dev(a) if a is not None else None)
+            finally:
+                b.set_option(b.OPT_GRID_LIMIT, 0)
+            assert np.array_equal(_np(g_ord), want)
+
+
 @pytest.mark.parametrize("cfg,seed", [(2, 42), (2, 142), (3, 42), (3, 242), (4, 42), (4, 142), (5, 42)])
 def test_full_size_configs(cfg, seed):
     """BASELINE.json configs[1..4] at FULL size in the launch configuration bench.py times (config 5:
