@@ -540,7 +540,7 @@ __device__ __forceinline__ i32 find_child_in(const i32* ft, i32 e0, i32 e1, i32 
 #endif
 // RADIX selects the mode at compile time: the two instantiations get their own register budgets
 // (the hash probe loop is lean and wants every warp slot of the SM; the radix walk is not)
-template <bool RADIX>
+template <bool RADIX, bool UPFRONT>
 __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_dual(DualArgs A) {
     __shared__ i32 root_ft[DW_ROOT_STAGE];
     __shared__ PathEntry stack[DW_WARPS][32];
@@ -663,6 +663,16 @@ __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_du
                 const i32 nb_l = valid ? (i32)(__ldg(A.blk_off + r_l + 1) - b_l) : 0;
                 i32 H_l = 0;
                 const int cnt = (int)min((i64)32, end - jb);
+                // A walk resumed at the shared depth often misses at once (the branch below the shared
+                // prefix is not cached), and that first probe does not depend on the predecessor's hit.
+                // When the queue has too few windows to fill the machine (UPFRONT: the call is bound by
+                // the chain of dependent trips inside a window, not by throughput), every position of the
+                // batch makes it up front, side by side, and a miss there costs the sequential loop no
+                // memory round trip.  On a full machine the extra probes cost more than they save.
+                const bool up_l = UPFRONT && valid && s_l < nb_l;
+                bool miss0_l = false;
+                if (UPFRONT && up_l) miss0_l = !table_has(A.t_keys, A.mask, ld_u64_once(A.hashes + b_l + s_l));
+                if (UPFRONT) c_probe += (u32)__popc(__ballot_sync(FULL, up_l));
                 for (int i = 0; i < cnt; ++i) {
                     const bool first = (jb == head && i == 0);
                     if (!first) {  // skip the positions that only copy (see the radix loop)
@@ -680,10 +690,13 @@ __global__ void __launch_bounds__(DW_THREADS, RADIX ? PEEK_DW_MINB : 8) k_lpm_du
                         const i32 nb = __shfl_sync(FULL, nb_l, i);
                         if (first) ++c_walks;
                         H = nb;
-                        // a resumed walk mostly misses at once (the branch below the shared prefix
-                        // is not cached): its first batch is 8 probes, later ones 32
+                        i32 from = s;
+                        if (UPFRONT && !first && s < nb) {  // the block at the shared depth was probed up front
+                            if (__shfl_sync(FULL, (int)miss0_l, i)) { H = s; from = nb; }
+                            else from = s + 1;
+                        }
                         int batch = 32;
-                        for (i32 i0 = s; i0 < nb; i0 += batch, batch = 32) {
+                        for (i32 i0 = from; i0 < nb; i0 += batch, batch = 32) {
                             const i32 x = i0 + lane;
                             bool miss = false;
                             const bool act = lane < batch && x < nb;
@@ -841,6 +854,7 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
         D.order = order; D.lcp = lcp; D.win = win; D.hit_radix = hit_radix; D.hit_hash = hit_hash;
         D.counters = g_lpm_counters;
         const i64 items = (N + win - 1) / win;
+        const bool upfront = items <= (i64)sm_count() * 64;  // fewer windows than warp slots: the call is latency bound
         i64 ctas = (items + DW_WARPS - 1) / DW_WARPS;
         const i64 cap = (i64)sm_count() * PEEK_DW_CAP;  // resident CTAs per SM - the warps loop over the items
         if (ctas > cap) ctas = cap;
@@ -850,22 +864,24 @@ extern "C" peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, c
         if (hit_radix && hit_hash && side_fork(st, &ss)) {
             Prof pr(PROF_LPM_DUAL, st, radix->E > 0 ? 3 : 2);
             D.ctr = ctr + 32;
-            k_lpm_dual<false><<<(unsigned)ctas, DW_THREADS, 0, ss.side>>>(D);
+            if (upfront) k_lpm_dual<false, true><<<(unsigned)ctas, DW_THREADS, 0, ss.side>>>(D);
+            else k_lpm_dual<false, false><<<(unsigned)ctas, DW_THREADS, 0, ss.side>>>(D);
             if (radix->E > 0) k_lpm_prep<<<(unsigned)((radix->E + 255) / 256), 256, 0, st>>>(R, radix->E, info);
             D.ctr = ctr;
-            k_lpm_dual<true><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
+            k_lpm_dual<true, false><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
             PEEK_CUDA(side_join(st, ss));
         } else {
             if (hit_radix) {
                 Prof pr(PROF_LPM_RADIX, st, radix->E > 0 ? 2 : 1);
                 if (radix->E > 0) k_lpm_prep<<<(unsigned)((radix->E + 255) / 256), 256, 0, st>>>(R, radix->E, info);
                 D.ctr = ctr;
-                k_lpm_dual<true><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
+                k_lpm_dual<true, false><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
             }
             if (hit_hash) {
                 Prof pr(PROF_LPM_HASH, st, 1);
                 D.ctr = ctr + 32;
-                k_lpm_dual<false><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
+                if (upfront) k_lpm_dual<false, true><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
+                else k_lpm_dual<false, false><<<(unsigned)ctas, DW_THREADS, 0, st>>>(D);
             }
         }
     } else {
