@@ -162,7 +162,14 @@ typedef struct {
  * hit_hash  int32[N] OUT (NULL to skip; needs table, hashes, blk_off): block_size * number of
  *           leading blocks whose chained hash is in the table, scanning to the FIRST miss.
  * tree      optional (NULL = naive per-request walk; needs hashes/blk_off as given to
- *           peek_pending_tree). */
+ *           peek_pending_tree).
+ * Streams   With a tree view and BOTH modes requested (queues above 2048 requests) the two walks are
+ *           independent kernels: the hash probes run on a side stream that the library creates once
+ *           per device (one non-blocking stream and two events, kept until the process exits; no
+ *           device memory), forked from and joined back into `stream`, so for the caller the call is
+ *           still ordered on `stream` alone.  If `stream` is being captured into a CUDA graph, or the
+ *           side stream cannot be made, both kernels stay on `stream`.  Calls from several host
+ *           threads share the side stream: they stay correct and serialise on it. */
 peek_status peek_lpm(const int32_t* tokens, const int64_t* tok_off, const uint64_t* hashes,
                      const int64_t* blk_off, int64_t N, int32_t block_size,
                      const peek_radix* radix /*host struct*/, const peek_table* table /*host struct*/,
