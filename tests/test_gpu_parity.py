@@ -504,6 +504,43 @@ def test_rank_two_phase_wide_keys():
         assert np.array_equal(_np(g_ord), oracle.clpm_order(hit, cs, a))
 
 
+def test_demand_tagged_probe_dense_table():
+    """Tables of 65 536 slots and more are probed through one-byte tags, eight at a time
+    (`k_demand<true>`).  A 93 %-full table makes long probe runs that wrap around the end; filler keys
+    share the tag (top byte) and the home slot of pending hashes, so tag matches with a different key,
+    runs that cross tag words and absent keys behind a matching tag all occur.  demand against the oracle."""
+    b = _b()
+    rng = np.random.default_rng(4242)
+    base = rng.integers(0, 1000, size=16 * 40).astype(np.int32)
+    reqs = [np.concatenate([base[:16 * int(rng.integers(1, 40))], rng.integers(0, 1000, size=int(rng.integers(0, 400))).astype(np.int32)])
+            for _ in range(3000)]
+    toks, off = _csr(reqs)
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    S = 1 << 16
+    mask = np.uint64(S - 1)
+    uniq = np.unique(o_h)
+    cached = uniq[rng.random(uniq.shape[0]) < 0.5]                    # half of the pending blocks are cached
+    absent = uniq[~np.isin(uniq, cached)]
+    # fillers: same top byte and same home slot as an absent pending hash, different middle bits
+    pick = absent[rng.integers(0, absent.shape[0], size=20000)]
+    mid = rng.integers(1, 1 << 30, size=pick.shape[0], dtype=np.uint64) << np.uint64(20)
+    fill_same = (pick ^ mid) & ~np.uint64(0)
+    fill_same = fill_same[~np.isin(fill_same, uniq)]
+    # fillers that pile up in the last slots of the table (runs wrap around to slot 0)
+    tail = (rng.integers(0, 1 << 40, size=3000, dtype=np.uint64) << np.uint64(16)) | (np.uint64(S - 1) - rng.integers(0, 8, size=3000, dtype=np.uint64))
+    rest = rng.integers(0, 2**63, size=S, dtype=np.uint64)
+    keys = np.concatenate([cached, fill_same, tail, rest])
+    keys = keys[keys != np.uint64(0xFFFFFFFFFFFFFFFF)]
+    t_keys = W.build_table(keys, S, max_keys=int(0.93 * S))
+    assert (t_keys != np.uint64(0xFFFFFFFFFFFFFFFF)).sum() >= int(0.9 * S)
+    d_h, d_bo = _dev(o_h.view(np.int64), torch.uint64), _dev(o_bo)
+    tree = b.peek_pending_tree(d_h, d_bo)
+    g_dem, _ = b.peek_demand_rank(d_h, d_bo, tree=tree, t_keys=_dev(t_keys.view(np.int64), torch.uint64))
+    want = oracle.demand(o_h, o_bo, t_keys)
+    assert want.sum() > 0
+    assert np.array_equal(_np(g_dem), want)
+
+
 @pytest.mark.parametrize("n", [1, 2, 31, 200, 511, 512, 513])
 def test_rank_small_queue_path(n):
     """Queues of at most 512 requests rank by counting (one CTA, `k_clpm_rank_small`); 513 takes the sort.
