@@ -132,7 +132,7 @@ i64 block_hash_ws_bytes(i64 N);
 i64 lpm_ws_bytes(i64 N, i64 V);
 i64 pending_tree_ws_bytes(i64 N);
 i64 demand_rank_ws_bytes(i64 N, i64 S);
-i64 clpm_signals_ws_bytes(i64 N);
+i64 clpm_signals_ws_bytes(i64 N, i64 S);
 i64 clpm_order_full_ws_bytes(i64 N);
 i64 group_major_ws_bytes(i64 N);
 i64 offline_phase1_ws_bytes(i64 N);
@@ -170,7 +170,7 @@ extern "C" peek_status peek_workspace_bytes(int32_t call_id, int64_t N, int64_t 
         case PEEK_CALL_LPM: *out_bytes = peek::lpm_ws_bytes(N, V > 0 ? V : 0); break;
         case PEEK_CALL_PENDING_TREE: *out_bytes = peek::pending_tree_ws_bytes(N); break;
         case PEEK_CALL_DEMAND_RANK: *out_bytes = peek::demand_rank_ws_bytes(N, S); break;
-        case PEEK_CALL_CLPM_SIGNALS: *out_bytes = peek::clpm_signals_ws_bytes(N); break;
+        case PEEK_CALL_CLPM_SIGNALS: *out_bytes = peek::clpm_signals_ws_bytes(N, S); break;
         case PEEK_CALL_CLPM_ORDER_FULL: *out_bytes = peek::clpm_order_full_ws_bytes(N); break;
         case PEEK_CALL_CLPM_GROUP_MAJOR: *out_bytes = peek::group_major_ws_bytes(N); break;
         case PEEK_CALL_OFFLINE_PHASE1: *out_bytes = peek::offline_phase1_ws_bytes(N); break;

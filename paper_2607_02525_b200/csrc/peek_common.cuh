@@ -162,6 +162,66 @@ __device__ __forceinline__ u64 ld_u64_once(const u64* p) {
     asm volatile("ld.global.nc.L2::cache_hint.u64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
     return v;
 }
+// ---- tagged table probes (peek_demand_rank, peek_lpm, peek_clpm_signals) -------------------------
+// Tables of at least TAGS_MIN_S slots get a
+// one-byte tag per slot first - 0 for an empty slot, else a fingerprint of its key (k_table_tags: one
+// streaming pass over the table).  A probe then walks the TAGS, which do stay in L2, and reads a key only
+// where the fingerprint matches: most pending blocks are not cached, and an absent key now costs a
+// byte from an L2-resident array instead of a random sector of the table.
+static constexpr i64 TAGS_MIN_S = (i64)1 << 16;
+__device__ __forceinline__ u32 key_tag(u64 key) { const u32 t = (u32)(key >> 56); return t ? t : 1u; }
+__device__ __forceinline__ u64 ld_tagword(const unsigned char* p) { return ld_u64_keep((const u64*)p); }
+static __global__ void __launch_bounds__(256) k_table_tags(const u64* __restrict__ t_keys, i64 S, unsigned char* __restrict__ tags,
+                                                    i32* __restrict__ demand) {
+    // thread = 8 consecutive slots (64 bytes of keys in, 8 bytes of tags out, the slots' 8 counters
+    // cleared when `demand` is given: that call's memset rides along); S is a power of two >= 8 here
+    const i64 g = (i64)blockIdx.x * 256 + threadIdx.x;
+    if (g * 8 >= S) return;
+    const ulonglong2* kp = (const ulonglong2*)(t_keys + g * 8);
+    u64 out = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const ulonglong2 v = __ldg(kp + q);
+        const u64 t0 = v.x == PEEK_EMPTY ? 0u : key_tag(v.x), t1 = v.y == PEEK_EMPTY ? 0u : key_tag(v.y);
+        out |= (t0 << (16 * q)) | (t1 << (16 * q + 8));
+    }
+    *(u64*)(tags + g * 8) = out;
+    if (demand) {
+        int4* d = (int4*)(demand + g * 8);
+        d[0] = make_int4(0, 0, 0, 0);
+        d[1] = make_int4(0, 0, 0, 0);
+    }
+}
+// slot of `key` or -1.  The probe sequence p, p+1, ... is walked eight tags at a time: `w` is the aligned
+// tag word that holds slot p (already loaded); bytes below p & 7 are not on the sequence.  zero_bytes()
+// marks (0x80) exactly the zero bytes of a word - the 7-bit adds cannot carry across bytes - so the
+// markers of the empty slots (w) and of the slots whose tag equals the key's (w ^ want) are both
+// exact, and the first marker on the sequence decides: empty -> absent, tag match -> compare the key.
+__device__ __forceinline__ u64 zero_bytes(u64 v) {
+    const u64 m7 = 0x7f7f7f7f7f7f7f7full;
+    return ~(((v & m7) + m7) | v | m7);
+}
+__device__ __forceinline__ i64 table_slot_tagged(const u64* __restrict__ t_keys, const unsigned char* __restrict__ tags,
+                                                 u64 mask, u64 key, u64 p, u64 w) {
+    const u64 want = (u64)key_tag(key) * 0x0101010101010101ull;
+    u64 base = p & ~7ull;
+    u64 live = ~0ull << (8 * (p & 7));  // bytes on the probe sequence
+    for (;;) {
+        const u64 zw = zero_bytes(w) & live;
+        u64 ev = zw | (zero_bytes(w ^ want) & live);
+        while (ev) {
+            const u64 first = ev & (~ev + 1);  // lowest marker
+            if (zw & first) return -1;         // an empty slot comes first: the key is absent
+            const u64 slot = base + (u64)((__ffsll((long long)first) - 1) >> 3);
+            if (ld_u64_keep(t_keys + slot) == key) return (i64)slot;
+            ev ^= first;                       // another key with the same tag
+        }
+        base = (base + 8) & mask;
+        live = ~0ull;
+        w = ld_tagword(tags + base);
+    }
+}
+
 __device__ __forceinline__ u32 ld_acquire_u32(const u32* p) {
     u32 v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");

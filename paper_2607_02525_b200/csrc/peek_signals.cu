@@ -195,6 +195,7 @@ __global__ void __launch_bounds__(SG_THREADS) k_evict_write(const u64* __restric
                                                            const i64* ein_a, const i64* ein_b,
                                                            const i32* __restrict__ which,
                                                            const u64* __restrict__ t_keys, u64 mask,
+                                                           const unsigned char* __restrict__ tags,
                                                            i64* __restrict__ evict, int ppw) {
     __shared__ EvictMeta sm[EV_WARPS];
     const unsigned FULL = 0xffffffffu;
@@ -269,7 +270,8 @@ __global__ void __launch_bounds__(SG_THREADS) k_evict_write(const u64* __restric
             val = own > eq ? own : eq;
         }
         if (act) {
-            const i64 p = sg_table_slot(t_keys, mask, key);
+            const i64 p = tags ? table_slot_tagged(t_keys, tags, mask, key, key & mask, ld_tagword(tags + ((key & mask) & ~7ull)))
+                               : sg_table_slot(t_keys, mask, key);
             if (p >= 0) evict[p] = val;
         }
     }
@@ -341,10 +343,12 @@ static void signals_layout(Arena& a, i64 N, SignalsWs& W) {
     W.start = a.take<i32>(N);
     W.runmin = a.take<unsigned long long>(N);
 }
-i64 clpm_signals_ws_bytes(i64 N) {
+// S > 0: room for the table's tags (peek_common.cuh), used when the workspace has it
+i64 clpm_signals_ws_bytes(i64 N, i64 S) {
     Arena a(nullptr);
     SignalsWs W;
     signals_layout(a, N, W);
+    if (S >= TAGS_MIN_S) a.take<unsigned char>(S);
     return a.used;
 }
 
@@ -369,7 +373,7 @@ extern "C" peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* 
         set_error("peek_clpm_signals: NULL argument");
         return PEEK_ERR_INVALID_ARG;
     }
-    if (work && (!ws || ((uintptr_t)ws & 255) || ws_bytes < clpm_signals_ws_bytes(N))) {
+    if (work && (!ws || ((uintptr_t)ws & 255) || ws_bytes < clpm_signals_ws_bytes(N, 0))) {
         set_error("peek_clpm_signals: workspace NULL, misaligned or too small");
         return PEEK_ERR_WORKSPACE;
     }
@@ -379,10 +383,14 @@ extern "C" peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* 
     Arena a(ws);
     SignalsWs W;
     signals_layout(a, N, W);
+    unsigned char* tags = nullptr;  // big table: absent keys (most pending blocks) are answered by its tags
+    if (evict_score && table->S >= TAGS_MIN_S && ((uintptr_t)table->t_keys & 15) == 0 &&
+        ws_bytes >= clpm_signals_ws_bytes(N, table->S))
+        tags = a.take<unsigned char>(table->S);
     a.arm(st);
     MinTree mt;
     mintree_layout(mt, lcp, N, W.mt_buf);
-    Prof pr(PROF_SIGNALS, st, mintree_launches(mt) + (score ? 4 : 0) + (evict_score ? 3 : 0) + (section ? 2 : 0));
+    Prof pr(PROF_SIGNALS, st, mintree_launches(mt) + (score ? 4 : 0) + (evict_score ? (tags ? 4 : 3) : 0) + (section ? 2 : 0));
     mintree_build(mt, st);
     unsigned grid = (unsigned)((N + SG_THREADS - 1) / SG_THREADS);
     if (grid > 148u * 16u) grid = 148u * 16u;
@@ -407,8 +415,9 @@ extern "C" peek_status peek_clpm_signals(const uint64_t* hashes, const int64_t* 
         while (ppw > 1 && N / ppw < 16384) ppw >>= 1;
         const i64 ewarps = (N + ppw - 1) / ppw;
         const unsigned wgrid = (unsigned)((ewarps * 32 + SG_THREADS - 1) / SG_THREADS);
+        if (tags) k_table_tags<<<(unsigned)((table->S / 8 + 255) / 256), 256, 0, st>>>(table->t_keys, table->S, tags, nullptr);
         k_evict_write<<<wgrid, SG_THREADS, 0, st>>>(hashes, blk_off, N, order, lcp, mt, W.ein[0], W.ein[1], W.which,
-                                                   table->t_keys, (u64)(table->S - 1), evict_score, ppw);
+                                                   table->t_keys, (u64)(table->S - 1), tags, evict_score, ppw);
     }
     if (section) {
         PEEK_CUDA(cudaMemsetAsync(W.runmin, 0xff, sizeof(unsigned long long) * (size_t)N, st));
