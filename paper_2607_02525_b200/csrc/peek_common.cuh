@@ -152,13 +152,13 @@ __device__ __forceinline__ int4 ld_stream_v4(const void* p) {
 // in L2 (evict last); words of the hash array are read once per call (evict first)
 __device__ __forceinline__ u64 ld_u64_keep(const u64* p) {
     u64 pol, v;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));  // not volatile: one per thread, hoisted out of loops
     asm volatile("ld.global.nc.L2::cache_hint.u64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
     return v;
 }
 __device__ __forceinline__ u64 ld_u64_once(const u64* p) {
     u64 pol, v;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     asm volatile("ld.global.nc.L2::cache_hint.u64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
     return v;
 }
@@ -169,7 +169,8 @@ __device__ __forceinline__ u64 ld_u64_once(const u64* p) {
 // where the fingerprint matches: most pending blocks are not cached, and an absent key now costs a
 // byte from an L2-resident array instead of a random sector of the table.
 static constexpr i64 TAGS_MIN_S = (i64)1 << 16;
-__device__ __forceinline__ u32 key_tag(u64 key) { const u32 t = (u32)(key >> 56); return t ? t : 1u; }
+// 7-bit tags (1..127): with the top bit of every byte clear, "byte == 0" is a carry-free add per byte
+__device__ __forceinline__ u32 key_tag(u64 key) { const u32 t = (u32)(key >> 57); return t ? t : 1u; }
 __device__ __forceinline__ u64 ld_tagword(const unsigned char* p) { return ld_u64_keep((const u64*)p); }
 static __global__ void __launch_bounds__(256) k_table_tags(const u64* __restrict__ t_keys, i64 S, unsigned char* __restrict__ tags,
                                                     i32* __restrict__ demand) {
@@ -194,12 +195,14 @@ static __global__ void __launch_bounds__(256) k_table_tags(const u64* __restrict
 }
 // slot of `key` or -1.  The probe sequence p, p+1, ... is walked eight tags at a time: `w` is the aligned
 // tag word that holds slot p (already loaded); bytes below p & 7 are not on the sequence.  zero_bytes()
-// marks (0x80) exactly the zero bytes of a word - the 7-bit adds cannot carry across bytes - so the
-// markers of the empty slots (w) and of the slots whose tag equals the key's (w ^ want) are both
-// exact, and the first marker on the sequence decides: empty -> absent, tag match -> compare the key.
+// marks (0x80) exactly the zero bytes of a word whose bytes are all <= 0x7f - byte + 0x7f sets the top
+// bit iff the byte is not 0 and never carries into its neighbour - so the markers of the empty slots
+// (w) and of the slots whose tag equals the key's (w ^ want) are both exact, and the first marker on
+// the sequence decides: empty -> absent, tag match -> compare the key.
 __device__ __forceinline__ u64 zero_bytes(u64 v) {
-    const u64 m7 = 0x7f7f7f7f7f7f7f7full;
-    return ~(((v & m7) + m7) | v | m7);
+    const u32 m7 = 0x7f7f7f7fu, hi = 0x80808080u;
+    const u32 lo32 = ~((u32)v + m7) & hi, hi32 = ~((u32)(v >> 32) + m7) & hi;  // no carries: halves are independent
+    return ((u64)hi32 << 32) | lo32;
 }
 __device__ __forceinline__ i64 table_slot_tagged(const u64* __restrict__ t_keys, const unsigned char* __restrict__ tags,
                                                  u64 mask, u64 key, u64 p, u64 w) {

@@ -87,7 +87,7 @@ __device__ __forceinline__ void rec_load(const ReqRec* __restrict__ rec, u32 r, 
 // a word of the hash array: read-once random sector, first in line for eviction from L2
 __device__ __forceinline__ u64 ldh(const u64* p) {
     u64 pol, v;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     asm volatile("ld.global.nc.L2::cache_hint.u64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
     return v;
 }
