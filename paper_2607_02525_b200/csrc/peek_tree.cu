@@ -186,6 +186,11 @@ __device__ __forceinline__ KeyLayout make_layout(i64 N, u64 maxnb, int wmax) {
 // chains of up to 2.6e8 tokens.  The entry point rejects longer chains (PEEK_ERR_UNSUPPORTED is
 // reported through the status word; see tree_launch).
 
+// Digit width of the grid-wide rounds.  A sort pass there costs two grid barriers whatever the queue
+// holds, so queues of at most 65 536 requests take 16-bit digits (two passes fewer per round): 16 bits
+// already tell that many branches apart, and the few that collide are finished by the local stage.
+__device__ __forceinline__ int global_wmax(i64 N) { return N <= 65536 ? 16 : 32; }
+
 // round-0 key of a request: d0 = (leading W0_BITS of its first word) | 1 << 31, or 0 for an empty chain
 __device__ __forceinline__ u64 round0_key(const KeyLayout& kl, u32 d0) {
     const int w0 = kl.w < W0_BITS ? kl.w : W0_BITS;
@@ -1495,7 +1500,7 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_tree_global(TreeArgs A) {
     Grid g{&A.ctl->bar, 0};
     PEEK_MARK(1);
     tree_phase0(A, g);
-    const KeyLayout kl = make_layout(A.N, __ldcg(&A.ctl->maxnb), 32);
+    const KeyLayout kl = make_layout(A.N, __ldcg(&A.ctl->maxnb), global_wmax(A.N));
     tree_global(A, kl, g, ssm, tsm, gs_stage(dyn_smem));
     PEEK_MARK(14);
 }
@@ -1505,7 +1510,7 @@ __global__ void __launch_bounds__(GS_THREADS, 1) k_tree_local(TreeArgs A) {
     __shared__ GsSmem ssm;
     __shared__ TreeSmem tsm;
     PEEK_MARK(15);
-    const KeyLayout kg = make_layout(A.N, __ldcg(&A.ctl->maxnb), 32), kl = make_layout(A.N, __ldcg(&A.ctl->maxnb), LOC_W);
+    const KeyLayout kg = make_layout(A.N, __ldcg(&A.ctl->maxnb), global_wmax(A.N)), kl = make_layout(A.N, __ldcg(&A.ctl->maxnb), LOC_W);
     tree_local_stage(A, kg, kl, false, (int)__ldcg(&A.ctl->fin_cb), (int)__ldcg(&A.ctl->fin_round), ssm, tsm, dyn_smem);
     PEEK_MARK(20);
 }
