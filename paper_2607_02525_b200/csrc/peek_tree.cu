@@ -1701,16 +1701,27 @@ struct UpdArgs {
     u64* agg;                    // gridDim scratch of the grid scans
 };
 
-// ordered grid-wide inclusive scan (associative op, NOT necessarily commutative)
+// ordered grid-wide inclusive scan (associative op, NOT necessarily commutative).  A thread owns
+// UP_ITEMS consecutive elements of a step and has all their loads in flight at once (the loads of
+// the compaction are dependent gathers), so a CTA's chunk takes a quarter of the steps - and of the
+// CTA barriers - that one element per thread would.  xch: blockDim.x elements of shared memory.
+static constexpr int UP_ITEMS = 4;
 template <typename T, typename Op, typename Load, typename Store>
-__device__ void grid_inscan_ordered(i64 n, Load load, Store store, Op op, T ident, T* agg, T* smem, Grid& g) {
-    const i64 chunk = (((n + gridDim.x - 1) / gridDim.x) + blockDim.x - 1) / blockDim.x * blockDim.x;
+__device__ void grid_inscan_ordered(i64 n, Load load, Store store, Op op, T ident, T* agg, T* smem, T* xch, Grid& g) {
+    const i64 step = (i64)blockDim.x * UP_ITEMS;
+    const i64 chunk = (((n + gridDim.x - 1) / gridDim.x) + step - 1) / step * step;
     const i64 c0 = min((i64)blockIdx.x * chunk, n), c1 = min(c0 + chunk, n);
     T carry = ident;
-    for (i64 b = c0; b < c1; b += blockDim.x) {
-        const i64 i = b + threadIdx.x;
+    for (i64 b = c0; b < c1; b += step) {
+        const i64 i0 = b + (i64)threadIdx.x * UP_ITEMS;
+        T v[UP_ITEMS];
+#pragma unroll
+        for (int k = 0; k < UP_ITEMS; ++k) v[k] = i0 + k < c1 ? load(i0 + k) : ident;
+        T t = v[0];
+#pragma unroll
+        for (int k = 1; k < UP_ITEMS; ++k) t = op(t, v[k]);
         T tt;
-        block_inscan(i < c1 ? load(i) : ident, op, ident, smem, &tt);
+        block_inscan(t, op, ident, smem, &tt);
         carry = op(carry, tt);
     }
     if (threadIdx.x == 0) agg[blockIdx.x] = carry;
@@ -1721,11 +1732,22 @@ __device__ void grid_inscan_ordered(i64 n, Load load, Store store, Op op, T iden
         for (int c = (int)threadIdx.x * per; c < min(((int)threadIdx.x + 1) * per, (int)blockIdx.x); ++c) acc = op(acc, agg[c]);
         block_inscan(acc, op, ident, smem, &carry);
     }
-    for (i64 b = c0; b < c1; b += blockDim.x) {
-        const i64 i = b + threadIdx.x;
+    for (i64 b = c0; b < c1; b += step) {
+        const i64 i0 = b + (i64)threadIdx.x * UP_ITEMS;
+        T v[UP_ITEMS];
+#pragma unroll
+        for (int k = 0; k < UP_ITEMS; ++k) v[k] = i0 + k < c1 ? load(i0 + k) : ident;
+#pragma unroll
+        for (int k = 1; k < UP_ITEMS; ++k) v[k] = op(v[k - 1], v[k]);  // inclusive inside the thread
         T tt;
-        const T inc = block_inscan(i < c1 ? load(i) : ident, op, ident, smem, &tt);
-        if (i < c1) store(i, op(carry, inc));
+        const T inc = block_inscan(v[UP_ITEMS - 1], op, ident, smem, &tt);
+        xch[threadIdx.x] = inc;  // the threads before this one = the inclusive value of its left neighbour
+        __syncthreads();
+        const T before = op(carry, threadIdx.x ? xch[threadIdx.x - 1] : ident);
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < UP_ITEMS; ++k)
+            if (i0 + k < c1) store(i0 + k, op(before, v[k]));
         carry = op(carry, tt);
     }
     g.sync();
@@ -1755,6 +1777,7 @@ static constexpr int UP_THREADS = 512;
 
 __global__ void __launch_bounds__(UP_THREADS) k_tree_update(UpdArgs A) {
     __shared__ u64 s64[UP_THREADS / 32 + 2];
+    __shared__ u64 xch[UP_THREADS];
     Grid g{&A.ctl->bar, 0};
     const i64 gtid = (i64)blockIdx.x * UP_THREADS + threadIdx.x, gsize = (i64)gridDim.x * UP_THREADS;
     const u64* __restrict__ H = A.hashes;
@@ -1776,11 +1799,48 @@ __global__ void __launch_bounds__(UP_THREADS) k_tree_update(UpdArgs A) {
             if (j == A.N_old - 1) A.ctl->S = (i64)(v >> 32);
         };
         grid_inscan_ordered<u64>(A.N_old, load, store, [](u64 a, u64 b) { return upd_op(a, b); },
-                                 upd_pack(0, 0x7fffffffu, 0), A.agg, s64, g);
+                                 upd_pack(0, 0x7fffffffu, 0), A.agg, s64, xch, g);
     }
     const i64 S = A.N_old > 0 ? __ldcg(&A.ctl->S) : 0;
     // ---- 3: every arrival bisects for its place among the survivors ----
     const i64 first_new = A.N_new - A.M;
+    if (A.M * 32 <= gsize) {
+        // few arrivals (the steady state of a serving loop): a warp per arrival, 32 pivots per step.
+        // A comparison is ~10 dependent trips (offsets, the depth bisection of chain_lcp, the branch
+        // words); 4 steps of 32 side by side instead of 20 one after the other.
+        const unsigned FULL = 0xffffffffu;
+        const int lane = threadIdx.x & 31;
+        const i64 q = gtid >> 5;
+        if (q < A.M) {
+            const i64 x = first_new + __ldg(A.b_order + q);
+            i64 lo = 0, hi = S;  // survivors before lo sort at or before x, from hi on after x
+            while (lo < hi) {
+                const i64 len = hi - lo;
+                const bool wide = len >= 32;
+                auto pivot = [&](int l) -> i64 { return wide ? lo + (len * (l + 1)) / 33 : lo + l; };
+                bool before = false;  // this lane's survivor sorts at or before x
+                if (wide || lane < len) {
+                    i32 l;
+                    before = upd_cmp(H, BO, x, __ldcg(A.s_order + pivot(lane)), &l) > 0;
+                }
+                const int c = __popc(__ballot_sync(FULL, before));  // sorted survivors: a prefix of the lanes
+                if (wide) {
+                    const i64 nlo = c ? pivot(c - 1) + 1 : lo, nhi = c < 32 ? pivot(c) : hi;
+                    lo = nlo; hi = nhi;
+                } else {
+                    lo += c; hi = lo;
+                }
+            }
+            i32 l = 0;
+            if (lane == 0 && lo > 0) upd_cmp(H, BO, x, __ldcg(A.s_order + lo - 1), &l);
+            if (lane == 1 && lo < S) upd_cmp(H, BO, x, __ldcg(A.s_order + lo), &l);
+            const i32 lR = __shfl_sync(FULL, l, 1);
+            if (lane == 0) {
+                A.ins[q] = (i32)lo; A.lcpL[q] = l; A.lcpR[q] = lR;
+                atomicAdd((unsigned long long*)(A.hist + lo), 1ull);
+            }
+        }
+    } else
     for (i64 q = gtid; q < A.M; q += gsize) {
         const i64 x = first_new + __ldg(A.b_order + q);
         i64 lo = 0, hi = S;
@@ -1814,7 +1874,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_tree_update(UpdArgs A) {
                 A.lcp[pos] = fix >= 0 ? fix : __ldcg(A.s_lcp + p);
             }
         };
-        grid_inscan_ordered<u64>(S + 1, load, store, [](u64 a, u64 b) { return a + b; }, (u64)0, A.agg, s64, g);
+        grid_inscan_ordered<u64>(S + 1, load, store, [](u64 a, u64 b) { return a + b; }, (u64)0, A.agg, s64, xch, g);
     }
 }
 
