@@ -449,6 +449,7 @@ __device__ __forceinline__ LocalBufs local_bufs(unsigned char* dyn_smem) {
                      (unsigned short*)(dyn_smem + (size_t)LOC_CAP * 16)};
 }
 
+static constexpr int LOC_COUNT_MAX = 512;  // items up to this size rank by counting (quadratic: 21 us at 1024, 5 us at 512)
 // Stable LSD sort of the item's n <= LOC_CAP positions by the key bits set in `vary` (8-bit
 // digits): permutes lb.idx (ping-pong with lb.aux; the roles are swapped in place).  Warp w owns
 // positions [w*32*Kp, (w+1)*32*Kp), Kp = ceil(n / GS_THREADS) rows.
@@ -456,7 +457,7 @@ __device__ __forceinline__ void local_sort(LocalBufs& lb, int n, u64 vary, GsSme
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int Kp = (n + GS_THREADS - 1) / GS_THREADS;
     const int wbase = w * 32 * Kp;
-    if (n <= GS_THREADS) {
+    if (n <= LOC_COUNT_MAX) {
         // Small items (one position per thread; the paper's queues hold 60-200 requests,
         // PAPER.md:364): no passes at all - every position counts the positions that sort before it
         // (smaller key, or equal key and earlier) against the keys staged by position, and its
