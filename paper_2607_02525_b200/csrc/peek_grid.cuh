@@ -248,20 +248,33 @@ static __global__ void __launch_bounds__(1024) k_mintree_all(MinTree mt) {
         __syncthreads();
     }
 }
+// big inputs: level 1 by the whole grid, then every further level (<= 1/1024 of the input) by one CTA
+static __global__ void __launch_bounds__(1024) k_mintree_from(MinTree mt, int k0) {
+    for (int k = k0; k < mt.levels; ++k) {
+        mintree_build_level(mt, k, (i64)(threadIdx.x >> 5), (i64)(blockDim.x >> 5), threadIdx.x & 31);
+        __syncthreads();
+    }
+}
+static constexpr i64 MINTREE_TAIL_MAX = 32768;  // entries of level 2 that one CTA still builds (N <= 2^25)
 static inline int mintree_launches(const MinTree& mt) {
-    return mt.levels <= 1 ? 0 : (mt.n[1] <= 1024 ? 1 : mt.levels - 1);
+    if (mt.levels <= 1) return 0;
+    if (mt.n[1] <= 1024) return 1;
+    if (mt.levels > 2 && mt.n[2] <= MINTREE_TAIL_MAX) return 2;
+    return mt.levels - 1;
 }
 static inline void mintree_build(const MinTree& mt, cudaStream_t st) {
     if (mt.levels > 1 && mt.n[1] <= 1024) {  // N <= 32768
         k_mintree_all<<<1, 1024, 0, st>>>(mt);
         return;
     }
-    for (int k = 1; k < mt.levels; ++k) {
+    const bool tail = mt.levels > 2 && mt.n[2] <= MINTREE_TAIL_MAX;
+    for (int k = 1; k < (tail ? 2 : mt.levels); ++k) {
         i64 warps = mt.n[k];
         unsigned grid = (unsigned)((warps * 32 + 255) / 256);
         if (grid > 148u * 8u) grid = 148u * 8u;
         k_mintree_level<<<grid, 256, 0, st>>>(mt, k);
     }
+    if (tail) k_mintree_from<<<1, 1024, 0, st>>>(mt, 2);
 }
 
 // largest p <= j with L0x[p] < cd   (requires one to exist, e.g. L0x[0] = 0 < cd)
