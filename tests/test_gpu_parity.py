@@ -426,6 +426,53 @@ def test_lpm_both_modes_side_stream():
         b.set_option(b.OPT_LPM_STRATEGY, b.LPM_AUTO)
 
 
+def test_lpm_side_stream_two_host_threads():
+    """Two host threads, each on its own stream with its own outputs and workspace, call peek_lpm (both
+    modes, dual walk) at the same time: they share the library's side stream and its events, which a
+    mutex keeps consistent between fork and join.  Every result equals the oracle."""
+    import threading
+    b = _b()
+    wl = W.make(2, seed=91, small=True)
+    toks, off = wl.queue.materialize_np()
+    cache = W.build_cache(wl, lambda t, o: oracle.block_hash(t, o, 16, 0))
+    o_bo, o_h = oracle.block_hash(toks, off, 16, 0)
+    o_hr = oracle.lpm_radix(toks, off, _orc_radix(cache.radix))
+    o_hh = oracle.lpm_hash(o_h, o_bo, cache.t_keys)
+    d_tok, d_off, d_h, d_bo = _dev(toks), _dev(off), _dev(o_h.view(np.int64), torch.uint64), _dev(o_bo)
+    d_radix, d_keys = _radix_dev(cache.radix), _dev(cache.t_keys.view(np.int64), torch.uint64)
+    tree = b.peek_pending_tree(d_h, d_bo)
+    torch.cuda.synchronize()
+    b.set_option(b.OPT_LPM_STRATEGY, b.LPM_DUAL_WALK)
+    errors = []
+
+    def worker(tid):
+        try:
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                for it in range(25):
+                    hr, hh = b.peek_lpm(d_tok, d_off, d_h, d_bo, radix=d_radix, t_keys=d_keys, tree=tree)
+                    if it % 6 == 0:
+                        st.synchronize()
+                        if not (np.array_equal(_np(hr), o_hr) and np.array_equal(_np(hh), o_hh)):
+                            errors.append("thread %d call %d differs" % (tid, it))
+                st.synchronize()
+                if not (np.array_equal(_np(hr), o_hr) and np.array_equal(_np(hh), o_hh)):
+                    errors.append("thread %d last call differs" % tid)
+        except Exception as e:  # noqa: BLE001 - reported below
+            errors.append("thread %d: %r" % (tid, e))
+
+    try:
+        ts = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+        for t in ts:
+            t.start()
+        for t in ts:
+            t.join(timeout=120)
+        assert not any(t.is_alive() for t in ts), "a thread hangs"
+    finally:
+        b.set_option(b.OPT_LPM_STRATEGY, b.LPM_AUTO)
+    assert not errors, errors
+
+
 @pytest.mark.parametrize("cfg,G", [(2, 2), (5, 3), (4, 4)])
 def test_sharded_queue_emulated(cfg, G):
     """SURVEY.md section 8(e) through the CUDA calls: the G shards of one queue (by first-block hash) run
