@@ -74,29 +74,54 @@ __global__ void __launch_bounds__(1024) k_nb_scan_small(const i64* __restrict__ 
     }
 }
 
+// PRESCANNED: partial[] holds exclusive prefixes (k_scan_partials ran); else it holds the chunks' own
+// sums and every CTA adds up the chunks before its own itself (up to SCAN_DIRECT_MAX of them: one
+// launch less), CTA 0 also resetting the request counter of k_block_hash_fused
+static constexpr int SCAN_DIRECT_MAX = 1024;
+template <bool PRESCANNED>
 __global__ void __launch_bounds__(SCAN_THREADS) k_nb_apply(const i64* __restrict__ tok_off, i64 N,
                                                           const i64* __restrict__ partial,
-                                                          i64* __restrict__ blk_off) {
+                                                          i64* __restrict__ blk_off,
+                                                          unsigned long long* __restrict__ counter) {
     __shared__ i64 sm[34];
-    // thread t owns SCAN_ITEMS consecutive requests so the scan is a plain blocked scan
-    i64 r0 = (i64)blockIdx.x * SCAN_CHUNK + (i64)threadIdx.x * SCAN_ITEMS;
+    i64 base = 0;
+    if (PRESCANNED) {
+        base = partial[blockIdx.x];
+    } else {
+        if (blockIdx.x == 0 && threadIdx.x == 0) *counter = 0;
+        i64 acc = 0;
+        for (int c = threadIdx.x; c < (int)blockIdx.x; c += SCAN_THREADS) acc += partial[c];
+        i64 tot0;
+        block_exscan_i64(acc, sm, &tot0);
+        base = tot0;
+        __syncthreads();
+    }
+    // thread t owns SCAN_ITEMS consecutive requests so the scan is a plain blocked scan; the offsets
+    // come in and the results go out through a shared-memory tile, so both global streams are coalesced
+    __shared__ i64 tile[SCAN_CHUNK + 1];
+    const i64 c0 = (i64)blockIdx.x * SCAN_CHUNK;
+    for (int x = threadIdx.x; x <= SCAN_CHUNK; x += SCAN_THREADS) tile[x] = c0 + x <= N ? tok_off[c0 + x] : 0;
+    __syncthreads();
+    const int t0 = threadIdx.x * SCAN_ITEMS;
     i64 nb[SCAN_ITEMS];
     i64 s = 0;
 #pragma unroll
     for (int it = 0; it < SCAN_ITEMS; ++it) {
-        i64 r = r0 + it;
-        nb[it] = r < N ? (tok_off[r + 1] - tok_off[r]) / B16 : 0;
+        nb[it] = c0 + t0 + it < N ? (tile[t0 + it + 1] - tile[t0 + it]) / B16 : 0;
         s += nb[it];
     }
     i64 tot;
-    i64 ex = block_exscan_i64(s, sm, &tot) + partial[blockIdx.x];
-    if (blockIdx.x == 0 && threadIdx.x == 0) blk_off[0] = 0;
+    i64 ex = block_exscan_i64(s, sm, &tot) + base;
+    __syncthreads();  // every thread has read its offsets: the tile now takes the results
 #pragma unroll
     for (int it = 0; it < SCAN_ITEMS; ++it) {
-        i64 r = r0 + it;
         ex += nb[it];
-        if (r < N) blk_off[r + 1] = ex;
+        tile[t0 + it] = ex;
     }
+    __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) blk_off[0] = 0;
+    for (int x = threadIdx.x; x < SCAN_CHUNK; x += SCAN_THREADS)
+        if (c0 + x < N) blk_off[c0 + x + 1] = tile[x];
 }
 
 // ---- fused content + chain ----------------------------------------------------------------
@@ -456,10 +481,15 @@ extern "C" peek_status peek_block_hash(const int32_t* tokens, const int64_t* tok
         Prof pr(PROF_HASH_SCAN, st, 1);
         k_nb_scan_small<<<1, 1024, 0, st>>>(tok_off, N, blk_off, counter);
     } else {
-        Prof pr(PROF_HASH_SCAN, st, 3);
+        const bool direct = nchunks <= SCAN_DIRECT_MAX;
+        Prof pr(PROF_HASH_SCAN, st, direct ? 2 : 3);
         k_nb_partial<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial);
-        k_scan_partials<<<1, 1024, 0, st>>>(partial, nchunks, counter);
-        k_nb_apply<<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial, blk_off);
+        if (direct) {
+            k_nb_apply<false><<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial, blk_off, counter);
+        } else {
+            k_scan_partials<<<1, 1024, 0, st>>>(partial, nchunks, counter);
+            k_nb_apply<true><<<(unsigned)nchunks, SCAN_THREADS, 0, st>>>(tok_off, N, partial, blk_off, counter);
+        }
     }
     if (hashes_capacity > 0) {
         PEEK_CUDA(func_smem_optin((const void*)k_block_hash_fused, HF_SMEM_BYTES));
