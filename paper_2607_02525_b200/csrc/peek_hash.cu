@@ -1,7 +1,7 @@
 // peek_hash.cu — a1 peek_block_hash: chained per-block hashes (R1).
 //
 // Two steps:
-//   nb_scan   blk_off = exclusive prefix sum of floor(len_r / B)                 (3 small launches)
+//   nb_scan   blk_off = exclusive prefix sum of floor(len_r / B)                 (2 small launches; 3 beyond 2 M requests; 1 up to 8192)
 //   fused     k_block_hash_fused: tokens -> per-block sums -> chained hashes in ONE pass over HBM
 //             (1-D bulk TMA staging, thread-per-block sums, lane-per-request chain; see below)
 #include <mutex>
